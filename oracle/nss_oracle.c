@@ -1,0 +1,839 @@
+/*
+ * nss_oracle.c — the ORACLE.  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, scalar CPU implementation (C99, libm, fp64 throughout) of the hot path of
+ * "Parallel Nested Slice Sampling for Gravitational Wave Parameter Estimation"
+ * (arxiv 2509.24949; /root/reference/PAPER.md):
+ *   - a heterodyned (relative-binning) frequency-domain GW log-likelihood
+ *   - the same log-likelihood on the full frequency grid
+ *   - one batched nested-slice-sampling replacement step and the NS loop
+ * The paper prints no equations; every formula below is the reading fixed in SURVEY.md §8(c)
+ * (O1..O16, A1..A24), restated in DESIGN.md §3, and cited by that label.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * call this file.  It shares no source, header, table or helper with the CUDA path under
+ * paper_2509_24949_b200/csrc/, and neither includes the other.
+ *
+ * No blocking, fusion or reordering: loops run in the order the definitions are written.
+ * OpenMP is used only to run independent points / independent chains on several host cores;
+ * every per-point and per-chain computation is the same scalar code (results do not depend on
+ * the thread count, since every random draw is a Philox counter, O11).
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): see DESIGN.md §5.  Unpinned by any external
+ * source: the higher PN phase coefficients phi_2..phi_7 (P2: "parity unpinned"; only sanity
+ * identities), and the sampler conventions A12/A14/A15/A17 (validity pinned by P13/P15 only).
+ */
+#include <complex.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifndef M_PI
+#define M_PI 3.14159265358979323846
+#endif
+
+/* ---- O1 constants ------------------------------------------------------------------------ */
+#define ORC_GMSUN_S 4.925490947641267e-6   /* G Msun / c^3  [s]  */
+#define ORC_MPC_M   3.085677581491367e22   /* 1 Mpc [m]          */
+#define ORC_C_MS    299792458.0            /* c [m/s]            */
+#define ORC_EULER   0.5772156649015329     /* Euler gamma        */
+
+#define ORC_NSLOT 11          /* canonical slots, O2 */
+#define ORC_MAXDET 4
+#define ORC_W 2.0             /* slice width scale w, O12.4a / A14 */
+#define ORC_MAX_EXPAND 32     /* per side, A15 */
+#define ORC_MAX_SHRINK 64     /* A15 */
+
+typedef struct { double vertex[3], xarm[3], yarm[3]; } orc_detector;
+
+typedef struct orc_problem {
+  int d;
+  int param_index[ORC_NSLOT];
+  double theta_fixed[ORC_NSLOT];
+  double lo[ORC_NSLOT], hi[ORC_NSLOT];
+  int n_det;
+  orc_detector det[ORC_MAXDET];
+  double gmst;
+  int n_freq;
+  double f_min, df;
+  double *psd;              /* [n_det][n_freq] */
+  double complex *data;     /* [n_det][n_freq] */
+  double theta_fid[ORC_NSLOT];
+  int n_bins;
+  int kind;                 /* 0 RB, 1 full grid, 2 Gaussian test */
+  double gauss_mu[ORC_NSLOT], gauss_sigma[ORC_NSLOT];
+  /* derived (O7..O9) */
+  double DD;                /* sum_det <d,d> */
+  int *edge_idx;            /* [B+1] grid indices i_e */
+  double *edge_f;           /* [B+1] F_e */
+  double complex *A0, *A1;  /* [n_det][B] */
+  double *B0, *B1;          /* [n_det][B] */
+  double complex *h0_edge;  /* [n_det][B+1] */
+} orc_problem;
+
+/* ---- O2 parameters ------------------------------------------------------------------------ */
+/* canonical order: 0 Mc, 1 q, 2 chi1z, 3 chi2z, 4 dL[Mpc], 5 tc, 6 phic, 7 iota, 8 psi, 9 ra, 10 dec */
+int orc_domain_ok(const double th[ORC_NSLOT])
+{
+  for (int j = 0; j < ORC_NSLOT; ++j) if (!isfinite(th[j])) return 0;
+  if (!(th[0] > 0.0)) return 0;
+  if (!(th[1] > 0.0 && th[1] <= 1.0)) return 0;
+  if (!(fabs(th[2]) < 1.0 && fabs(th[3]) < 1.0)) return 0;
+  if (!(th[4] > 0.0)) return 0;
+  return 1;
+}
+
+/* ---- O3 waveform: TaylorF2 3.5PN phase + 1.5PN spin-orbit, Newtonian amplitude ------------ */
+double orc_phase(double f, const double th[ORC_NSLOT])
+{
+  const double Mc = th[0], q = th[1], chi1 = th[2], chi2 = th[3], tc = th[5], phic = th[6];
+  const double eta = q / ((1.0 + q) * (1.0 + q));
+  const double M = Mc * pow(eta, -3.0 / 5.0) * ORC_GMSUN_S;      /* total mass [s] */
+  const double m1 = 1.0 / (1.0 + q), m2 = q / (1.0 + q);         /* m_i / M */
+  const double v = cbrt(M_PI * M * f);
+  const double vlso = 1.0 / sqrt(6.0);
+  const double beta = (113.0 / 12.0 * m1 * m1 + 25.0 / 4.0 * eta) * chi1
+                    + (113.0 / 12.0 * m2 * m2 + 25.0 / 4.0 * eta) * chi2;
+  double phi[8];
+  phi[0] = 1.0;
+  phi[1] = 0.0;
+  phi[2] = 3715.0 / 756.0 + 55.0 * eta / 9.0;
+  phi[3] = -16.0 * M_PI + 4.0 * beta;
+  phi[4] = 15293365.0 / 508032.0 + 27145.0 * eta / 504.0 + 3085.0 * eta * eta / 72.0;
+  phi[5] = M_PI * (38645.0 / 756.0 - 65.0 * eta / 9.0) * (1.0 + 3.0 * log(v / vlso));
+  phi[6] = 11583231236531.0 / 4694215680.0 - 640.0 * M_PI * M_PI / 3.0 - 6848.0 * ORC_EULER / 21.0
+         + eta * (-15737765635.0 / 3048192.0 + 2255.0 * M_PI * M_PI / 12.0)
+         + 76055.0 * eta * eta / 1728.0 - 127825.0 * eta * eta * eta / 1296.0
+         - 6848.0 / 21.0 * log(4.0 * v);
+  phi[7] = M_PI * (77096675.0 / 254016.0 + 378515.0 * eta / 1512.0 - 74045.0 * eta * eta / 756.0);
+  double s = 0.0;
+  for (int k = 0; k < 8; ++k) s += phi[k] * pow(v, (double)k);
+  return 2.0 * M_PI * f * tc - phic - M_PI / 4.0 + 3.0 / (128.0 * eta * pow(v, 5.0)) * s;
+}
+
+/* test hook (P1): same phase with phi_2..phi_7 zeroed = Newtonian chirp */
+double orc_phase_newtonian(double f, const double th[ORC_NSLOT])
+{
+  const double Mc = th[0], q = th[1], tc = th[5], phic = th[6];
+  const double eta = q / ((1.0 + q) * (1.0 + q));
+  const double M = Mc * pow(eta, -3.0 / 5.0) * ORC_GMSUN_S;
+  const double v = cbrt(M_PI * M * f);
+  return 2.0 * M_PI * f * tc - phic - M_PI / 4.0 + 3.0 / (128.0 * eta * pow(v, 5.0)) * 1.0;
+}
+
+/* plus / cross polarisations, O3 */
+void orc_polarisations(double f, const double th[ORC_NSLOT], double complex *hp, double complex *hc)
+{
+  const double Mc = th[0], dL = th[4], iota = th[7];
+  const double amp = sqrt(5.0 / 24.0) * pow(M_PI, -2.0 / 3.0) * pow(Mc * ORC_GMSUN_S, 5.0 / 6.0)
+                   * ORC_C_MS / (dL * ORC_MPC_M);
+  const double psi = orc_phase(f, th);
+  const double complex e = cexp(-I * psi);
+  const double a = amp * pow(f, -7.0 / 6.0);
+  const double ci = cos(iota);
+  *hp = a * (1.0 + ci * ci) / 2.0 * e;
+  *hc = -I * a * ci * e;
+}
+
+/* ---- O4 detector response ----------------------------------------------------------------- */
+void orc_antenna(const orc_detector *det, double gmst, double ra, double dec, double psi,
+                 double *Fp, double *Fc, double *dt)
+{
+  double D[3][3];
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b)
+      D[a][b] = 0.5 * (det->xarm[a] * det->xarm[b] - det->yarm[a] * det->yarm[b]);
+  const double g = gmst - ra;
+  const double X[3] = { -cos(psi) * sin(g) - sin(psi) * cos(g) * sin(dec),
+                        -cos(psi) * cos(g) + sin(psi) * sin(g) * sin(dec),
+                         sin(psi) * cos(dec) };
+  const double Y[3] = {  sin(psi) * sin(g) - cos(psi) * cos(g) * sin(dec),
+                         sin(psi) * cos(g) + cos(psi) * sin(g) * sin(dec),
+                         cos(psi) * cos(dec) };
+  double XDX = 0, YDY = 0, XDY = 0, YDX = 0;
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b) {
+      XDX += X[a] * D[a][b] * X[b];
+      YDY += Y[a] * D[a][b] * Y[b];
+      XDY += X[a] * D[a][b] * Y[b];
+      YDX += Y[a] * D[a][b] * X[b];
+    }
+  *Fp = XDX - YDY;
+  *Fc = XDY + YDX;
+  const double n[3] = { cos(dec) * cos(ra - gmst), cos(dec) * sin(ra - gmst), sin(dec) };
+  *dt = -(det->vertex[0] * n[0] + det->vertex[1] * n[1] + det->vertex[2] * n[2]) / ORC_C_MS;
+}
+
+/* strain in one detector at frequencies f[0..n): h_det = [F+ h+ + Fx hx] e^{-2 pi i f dt} */
+void orc_waveform_det(const double th[ORC_NSLOT], const orc_detector *det, double gmst,
+                      const double *f, int n, double complex *out)
+{
+  double Fp, Fc, dt;
+  orc_antenna(det, gmst, th[9], th[10], th[8], &Fp, &Fc, &dt);
+  for (int k = 0; k < n; ++k) {
+    double complex hp, hc;
+    orc_polarisations(f[k], th, &hp, &hc);
+    out[k] = (Fp * hp + Fc * hc) * cexp(-2.0 * M_PI * I * f[k] * dt);
+  }
+}
+
+/* ---- O7 inner product --------------------------------------------------------------------- */
+/* <a,b> = 4 df Re sum_k conj(a_k) b_k / S_k, every grid point, no end weights */
+double orc_inner(const double complex *a, const double complex *b, const double *S, int n, double df)
+{
+  double s = 0.0;
+  for (int k = 0; k < n; ++k) s += creal(conj(a[k]) * b[k]) / S[k];
+  return 4.0 * df * s;
+}
+
+static void canon_from_sampled(const orc_problem *p, const double *theta, double th[ORC_NSLOT])
+{
+  for (int j = 0; j < ORC_NSLOT; ++j) th[j] = p->theta_fixed[j];
+  for (int j = 0; j < p->d; ++j) th[p->param_index[j]] = theta[j];
+}
+
+/* O7: logL = -1/2 sum_det <d-h, d-h>, written as the definition */
+double orc_loglike_full_canon(const orc_problem *p, const double th[ORC_NSLOT])
+{
+  if (!orc_domain_ok(th)) return -INFINITY;
+  const int n = p->n_freq;
+  double *f = (double *)malloc(sizeof(double) * n);
+  double complex *h = (double complex *)malloc(sizeof(double complex) * n);
+  double complex *r = (double complex *)malloc(sizeof(double complex) * n);
+  for (int k = 0; k < n; ++k) f[k] = p->f_min + k * p->df;
+  double logL = 0.0;
+  for (int a = 0; a < p->n_det; ++a) {
+    orc_waveform_det(th, &p->det[a], p->gmst, f, n, h);
+    const double complex *dat = p->data + (size_t)a * n;
+    for (int k = 0; k < n; ++k) r[k] = dat[k] - h[k];
+    logL += -0.5 * orc_inner(r, r, p->psd + (size_t)a * n, n, p->df);
+  }
+  free(f); free(h); free(r);
+  return logL;
+}
+
+/* the same logL in the expanded form sum_det [<d,h> - 1/2 <h,h>] - 1/2 DD, plus its two parts
+ * (test hook for P7) */
+void orc_full_parts_canon(const orc_problem *p, const double th[ORC_NSLOT], double *dh, double *hh)
+{
+  const int n = p->n_freq;
+  double *f = (double *)malloc(sizeof(double) * n);
+  double complex *h = (double complex *)malloc(sizeof(double complex) * n);
+  for (int k = 0; k < n; ++k) f[k] = p->f_min + k * p->df;
+  *dh = 0.0; *hh = 0.0;
+  for (int a = 0; a < p->n_det; ++a) {
+    orc_waveform_det(th, &p->det[a], p->gmst, f, n, h);
+    *dh += orc_inner(p->data + (size_t)a * n, h, p->psd + (size_t)a * n, n, p->df);
+    *hh += orc_inner(h, h, p->psd + (size_t)a * n, n, p->df);
+  }
+  free(f); free(h);
+}
+
+/* ---- O8 bin edges -------------------------------------------------------------------------- */
+static double dephasing(double f, double fmin, double fmax)
+{
+  static const double gam[5] = { -5.0 / 3.0, -2.0 / 3.0, 1.0, 5.0 / 3.0, 7.0 / 3.0 };
+  double s = 0.0;
+  for (int i = 0; i < 5; ++i) {
+    const double fs = gam[i] > 0 ? fmax : fmin;
+    s += (gam[i] > 0 ? 1.0 : -1.0) * pow(f / fs, gam[i]);
+  }
+  return s;
+}
+
+static int build_edges(orc_problem *p)
+{
+  const int n = p->n_freq, B = p->n_bins;
+  if (B < 1 || B > n - 1) return -1;
+  const double fmin = p->f_min, fmax = p->f_min + (n - 1) * p->df;
+  double *del = (double *)malloc(sizeof(double) * n);
+  for (int k = 0; k < n; ++k) del[k] = dephasing(p->f_min + k * p->df, fmin, fmax);
+  int *ie = p->edge_idx;
+  for (int e = 0; e <= B; ++e) {
+    const double target = del[0] + ((double)e / (double)B) * (del[n - 1] - del[0]);
+    int best = 0; double bd = fabs(del[0] - target);
+    for (int k = 1; k < n; ++k) {
+      const double dd = fabs(del[k] - target);
+      if (dd < bd) { bd = dd; best = k; }        /* ties -> lower index */
+    }
+    ie[e] = best;
+  }
+  ie[0] = 0; ie[B] = n - 1;
+  for (int e = 1; e <= B; ++e) if (ie[e] < ie[e - 1] + 1) ie[e] = ie[e - 1] + 1;
+  ie[B] = n - 1;
+  for (int e = B - 1; e >= 0; --e) if (ie[e] > ie[e + 1] - 1) ie[e] = ie[e + 1] - 1;
+  for (int e = 0; e <= B; ++e) p->edge_f[e] = p->f_min + ie[e] * p->df;
+  free(del);
+  return 0;
+}
+
+/* ---- O9 summary data ----------------------------------------------------------------------- */
+static void build_summary(orc_problem *p)
+{
+  const int n = p->n_freq, B = p->n_bins;
+  double *f = (double *)malloc(sizeof(double) * n);
+  double complex *h0 = (double complex *)malloc(sizeof(double complex) * n);
+  for (int k = 0; k < n; ++k) f[k] = p->f_min + k * p->df;
+  for (int a = 0; a < p->n_det; ++a) {
+    orc_waveform_det(p->theta_fid, &p->det[a], p->gmst, f, n, h0);
+    const double complex *dat = p->data + (size_t)a * n;
+    const double *S = p->psd + (size_t)a * n;
+    for (int b = 0; b < B; ++b) {
+      const int k0 = p->edge_idx[b];
+      const int k1 = (b == B - 1) ? p->edge_idx[B] + 1 : p->edge_idx[b + 1];   /* A8 */
+      const double fbar = 0.5 * (p->edge_f[b] + p->edge_f[b + 1]);
+      double complex a0 = 0, a1 = 0; double b0 = 0, b1 = 0;
+      for (int k = k0; k < k1; ++k) {
+        const double complex dh = dat[k] * conj(h0[k]) / S[k];
+        const double hh = creal(h0[k] * conj(h0[k])) / S[k];
+        a0 += dh; a1 += dh * (f[k] - fbar);
+        b0 += hh; b1 += hh * (f[k] - fbar);
+      }
+      p->A0[(size_t)a * B + b] = 4.0 * p->df * a0;
+      p->A1[(size_t)a * B + b] = 4.0 * p->df * a1;
+      p->B0[(size_t)a * B + b] = 4.0 * p->df * b0;
+      p->B1[(size_t)a * B + b] = 4.0 * p->df * b1;
+    }
+    for (int e = 0; e <= B; ++e) p->h0_edge[(size_t)a * (B + 1) + e] = h0[p->edge_idx[e]];
+  }
+  free(f); free(h0);
+}
+
+/* ---- O10 relative-binning logL ------------------------------------------------------------- */
+void orc_rb_parts_canon(const orc_problem *p, const double th[ORC_NSLOT], double *dh, double *hh)
+{
+  const int B = p->n_bins;
+  double complex *h = (double complex *)malloc(sizeof(double complex) * (B + 1));
+  double complex *r = (double complex *)malloc(sizeof(double complex) * (B + 1));
+  *dh = 0.0; *hh = 0.0;
+  for (int a = 0; a < p->n_det; ++a) {
+    orc_waveform_det(th, &p->det[a], p->gmst, p->edge_f, B + 1, h);      /* same O3/O4 routine */
+    for (int e = 0; e <= B; ++e) r[e] = h[e] / p->h0_edge[(size_t)a * (B + 1) + e];
+    for (int b = 0; b < B; ++b) {
+      const double complex r0 = 0.5 * (r[b] + r[b + 1]);
+      const double complex r1 = (r[b + 1] - r[b]) / (p->edge_f[b + 1] - p->edge_f[b]);
+      const size_t ib = (size_t)a * B + b;
+      *dh += creal(p->A0[ib] * conj(r0) + p->A1[ib] * conj(r1));
+      *hh += p->B0[ib] * creal(r0 * conj(r0)) + 2.0 * p->B1[ib] * creal(r0 * conj(r1));
+    }
+  }
+  free(h); free(r);
+}
+
+double orc_loglike_rb_canon(const orc_problem *p, const double th[ORC_NSLOT])
+{
+  if (!orc_domain_ok(th)) return -INFINITY;
+  double dh, hh;
+  orc_rb_parts_canon(p, th, &dh, &hh);
+  return dh - 0.5 * hh - 0.5 * p->DD;
+}
+
+/* ---- O16 Gaussian test likelihood ---------------------------------------------------------- */
+static double loglike_gauss(const orc_problem *p, const double *theta)
+{
+  double s = 0.0;
+  for (int j = 0; j < p->d; ++j) {
+    if (!isfinite(theta[j])) return -INFINITY;
+    const double z = (theta[j] - p->gauss_mu[j]) / p->gauss_sigma[j];
+    s += z * z;
+  }
+  return -0.5 * s;
+}
+
+/* logL of a sampled-coordinate vector theta[d], according to p->kind */
+double orc_loglike(const orc_problem *p, const double *theta)
+{
+  if (p->kind == 2) return loglike_gauss(p, theta);
+  double th[ORC_NSLOT];
+  canon_from_sampled(p, theta, th);
+  return p->kind == 0 ? orc_loglike_rb_canon(p, th) : orc_loglike_full_canon(p, th);
+}
+
+double orc_loglike_kind(const orc_problem *p, const double *theta, int kind)
+{
+  if (kind == 2) return loglike_gauss(p, theta);
+  double th[ORC_NSLOT];
+  canon_from_sampled(p, theta, th);
+  return kind == 0 ? orc_loglike_rb_canon(p, th) : orc_loglike_full_canon(p, th);
+}
+
+void orc_loglike_batch(const orc_problem *p, const double *theta, int64_t N, double *out, int nthreads)
+{
+  if (nthreads < 1) nthreads = 1;
+#pragma omp parallel for schedule(static) num_threads(nthreads)
+  for (int64_t i = 0; i < N; ++i) out[i] = orc_loglike(p, theta + (size_t)i * p->d);
+}
+
+/* ---- create / destroy ---------------------------------------------------------------------- */
+void orc_destroy(orc_problem *p)
+{
+  if (!p) return;
+  free(p->psd); free(p->data); free(p->edge_idx); free(p->edge_f);
+  free(p->A0); free(p->A1); free(p->B0); free(p->B1); free(p->h0_edge);
+  free(p);
+}
+
+/* det_flat: [n_det][9] = vertex(3), xarm(3), yarm(3); data: [n_det][n_freq][2] (re, im).
+ * kind 2 needs no detectors/data (n_det = 0, n_freq = 0 allowed).  Returns NULL on bad input. */
+orc_problem *orc_create(int d, const int *param_index, const double *theta_fixed,
+                        const double *lo, const double *hi,
+                        int n_det, const double *det_flat, double gmst,
+                        int n_freq, double f_min, double df,
+                        const double *psd, const double *data,
+                        const double *theta_fid, int n_bins, int kind,
+                        const double *gauss_mu, const double *gauss_sigma)
+{
+  if (d < 1 || d > ORC_NSLOT || kind < 0 || kind > 2) return NULL;
+  orc_problem *p = (orc_problem *)calloc(1, sizeof(orc_problem));
+  p->d = d; p->kind = kind;
+  for (int j = 0; j < d; ++j) {
+    p->param_index[j] = param_index ? param_index[j] : j;
+    p->lo[j] = lo[j]; p->hi[j] = hi[j];
+    if (!(lo[j] < hi[j])) { orc_destroy(p); return NULL; }
+    if (gauss_mu) p->gauss_mu[j] = gauss_mu[j];
+    if (gauss_sigma) p->gauss_sigma[j] = gauss_sigma[j];
+  }
+  if (kind == 2) return p;
+  if (n_det < 1 || n_det > ORC_MAXDET || n_freq < 2) { orc_destroy(p); return NULL; }
+  for (int j = 0; j < ORC_NSLOT; ++j) { p->theta_fixed[j] = theta_fixed[j]; p->theta_fid[j] = theta_fid[j]; }
+  p->n_det = n_det; p->gmst = gmst; p->n_freq = n_freq; p->f_min = f_min; p->df = df; p->n_bins = n_bins;
+  for (int a = 0; a < n_det; ++a)
+    for (int c = 0; c < 3; ++c) {
+      p->det[a].vertex[c] = det_flat[a * 9 + c];
+      p->det[a].xarm[c] = det_flat[a * 9 + 3 + c];
+      p->det[a].yarm[c] = det_flat[a * 9 + 6 + c];
+    }
+  const size_t nn = (size_t)n_det * n_freq;
+  p->psd = (double *)malloc(sizeof(double) * nn);
+  p->data = (double complex *)malloc(sizeof(double complex) * nn);
+  for (size_t k = 0; k < nn; ++k) {
+    if (!(psd[k] > 0.0)) { orc_destroy(p); return NULL; }
+    p->psd[k] = psd[k];
+    p->data[k] = data[2 * k] + I * data[2 * k + 1];
+  }
+  p->DD = 0.0;
+  for (int a = 0; a < n_det; ++a)
+    p->DD += orc_inner(p->data + (size_t)a * n_freq, p->data + (size_t)a * n_freq,
+                       p->psd + (size_t)a * n_freq, n_freq, df);
+  if (kind == 0) {
+    if (!orc_domain_ok(p->theta_fid)) { orc_destroy(p); return NULL; }
+    const int B = n_bins;
+    if (B < 1 || B > n_freq - 1) { orc_destroy(p); return NULL; }
+    p->edge_idx = (int *)malloc(sizeof(int) * (B + 1));
+    p->edge_f = (double *)malloc(sizeof(double) * (B + 1));
+    p->A0 = (double complex *)malloc(sizeof(double complex) * n_det * B);
+    p->A1 = (double complex *)malloc(sizeof(double complex) * n_det * B);
+    p->B0 = (double *)malloc(sizeof(double) * n_det * B);
+    p->B1 = (double *)malloc(sizeof(double) * n_det * B);
+    p->h0_edge = (double complex *)malloc(sizeof(double complex) * n_det * (B + 1));
+    build_edges(p);
+    build_summary(p);
+  }
+  return p;
+}
+
+/* accessors for tests */
+double orc_get_DD(const orc_problem *p) { return p->DD; }
+void orc_get_edges(const orc_problem *p, int *idx, double *f)
+{
+  for (int e = 0; e <= p->n_bins; ++e) { idx[e] = p->edge_idx[e]; f[e] = p->edge_f[e]; }
+}
+/* out: [n_det][B][6] = A0re, A0im, A1re, A1im, B0, B1 */
+void orc_get_summary(const orc_problem *p, double *out)
+{
+  for (int a = 0; a < p->n_det; ++a)
+    for (int b = 0; b < p->n_bins; ++b) {
+      const size_t ib = (size_t)a * p->n_bins + b;
+      out[ib * 6 + 0] = creal(p->A0[ib]); out[ib * 6 + 1] = cimag(p->A0[ib]);
+      out[ib * 6 + 2] = creal(p->A1[ib]); out[ib * 6 + 3] = cimag(p->A1[ib]);
+      out[ib * 6 + 4] = p->B0[ib];        out[ib * 6 + 5] = p->B1[ib];
+    }
+}
+/* waveform of a canonical parameter vector on an arbitrary frequency list; out [n][2] */
+void orc_waveform(const double *th, const double *det9, double gmst, const double *f, int n, double *out)
+{
+  orc_detector det;
+  for (int c = 0; c < 3; ++c) { det.vertex[c] = det9[c]; det.xarm[c] = det9[3 + c]; det.yarm[c] = det9[6 + c]; }
+  double complex *h = (double complex *)malloc(sizeof(double complex) * n);
+  orc_waveform_det(th, &det, gmst, f, n, h);
+  for (int k = 0; k < n; ++k) { out[2 * k] = creal(h[k]); out[2 * k + 1] = cimag(h[k]); }
+  free(h);
+}
+void orc_antenna_flat(const double *det9, double gmst, double ra, double dec, double psi, double *out3)
+{
+  orc_detector det;
+  for (int c = 0; c < 3; ++c) { det.vertex[c] = det9[c]; det.xarm[c] = det9[3 + c]; det.yarm[c] = det9[6 + c]; }
+  orc_antenna(&det, gmst, ra, dec, psi, &out3[0], &out3[1], &out3[2]);
+}
+void orc_parts(const orc_problem *p, const double *theta, double *out4)
+{
+  double th[ORC_NSLOT];
+  canon_from_sampled(p, theta, th);
+  orc_full_parts_canon(p, th, &out4[0], &out4[1]);
+  if (p->kind == 0) orc_rb_parts_canon(p, th, &out4[2], &out4[3]);
+}
+
+/* ============================================================================================ */
+/* ---- O11 random numbers: Philox4x32-10 (Salmon, Moraes, Dror, Shaw 2011) -------------------- */
+void orc_philox4x32_10(const uint32_t key_in[2], const uint32_t ctr_in[4], uint32_t out[4])
+{
+  uint32_t k0 = key_in[0], k1 = key_in[1];
+  uint32_t c0 = ctr_in[0], c1 = ctr_in[1], c2 = ctr_in[2], c3 = ctr_in[3];
+  for (int round = 0; round < 10; ++round) {
+    const uint64_t p0 = (uint64_t)0xD2511F53u * (uint64_t)c0;
+    const uint64_t p1 = (uint64_t)0xCD9E8D57u * (uint64_t)c2;
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+    const uint32_t n1 = (uint32_t)p1;
+    const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+    const uint32_t n3 = (uint32_t)p0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* one counter block -> two 53-bit integers ka, kb (O11) */
+void orc_draw53(uint64_t seed, uint32_t block, uint32_t step, uint32_t chain, uint32_t iteration,
+                uint64_t *ka, uint64_t *kb)
+{
+  const uint32_t key[2] = { (uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32) };
+  const uint32_t ctr[4] = { block, step, chain, iteration };
+  uint32_t w[4];
+  orc_philox4x32_10(key, ctr, w);
+  *ka = ((uint64_t)(w[0] >> 5) << 26) + (uint64_t)(w[1] >> 6);
+  *kb = ((uint64_t)(w[2] >> 5) << 26) + (uint64_t)(w[3] >> 6);
+}
+static const double TWO_M53 = 1.0 / 9007199254740992.0;
+/* u in [0,1) */
+double orc_uniform_a(uint64_t seed, uint32_t block, uint32_t step, uint32_t chain, uint32_t iteration)
+{
+  uint64_t ka, kb; orc_draw53(seed, block, step, chain, iteration, &ka, &kb);
+  return (double)ka * TWO_M53;
+}
+/* Box-Muller pair from one block: z0 = sqrt(-2 ln u+_a) cos(2 pi u_b), z1 = ... sin(...) */
+void orc_normal_pair(uint64_t seed, uint32_t block, uint32_t step, uint32_t chain, uint32_t iteration,
+                     double *z0, double *z1)
+{
+  uint64_t ka, kb; orc_draw53(seed, block, step, chain, iteration, &ka, &kb);
+  const double up = (double)(ka + 1) * TWO_M53;     /* (0,1] */
+  const double ub = (double)kb * TWO_M53;           /* [0,1) */
+  const double r = sqrt(-2.0 * log(up));
+  *z0 = r * cos(2.0 * M_PI * ub);
+  *z1 = r * sin(2.0 * M_PI * ub);
+}
+
+#define ORC_ITER_INIT 0xFFFFFFFFu
+#define ORC_ITER_ERR  0xFFFFFFFEu
+#define ORC_STEP_START 0xFFFFFFFFu
+
+/* ---- O13 initial live points --------------------------------------------------------------- */
+void orc_init_live(const orc_problem *p, int n, uint64_t seed, double *live, double *logL, int nthreads)
+{
+  const int d = p->d;
+  for (int i = 0; i < n; ++i)
+    for (int j = 0; j < d; ++j) {
+      uint64_t ka, kb; orc_draw53(seed, (uint32_t)(j / 2), 0u, (uint32_t)i, ORC_ITER_INIT, &ka, &kb);
+      const double u = (double)((j & 1) ? kb : ka) * TWO_M53;
+      live[(size_t)i * d + j] = p->lo[j] + (p->hi[j] - p->lo[j]) * u;
+    }
+  orc_loglike_batch(p, live, n, logL, nthreads);
+}
+
+/* ---- O12.1 delete select ------------------------------------------------------------------- */
+/* dead_idx: the k lowest logL ascending, ties by lower slot; surv_idx: the rest, ascending slot */
+void orc_select_lowest(const double *logL, int n, int k, int *dead_idx, int *surv_idx)
+{
+  char *taken = (char *)calloc(n, 1);
+  for (int j = 0; j < k; ++j) {                 /* selection, written as the definition */
+    int best = -1;
+    for (int i = 0; i < n; ++i) {
+      if (taken[i]) continue;
+      if (best < 0 || logL[i] < logL[best]) best = i;     /* strict <  => ties keep lower slot */
+    }
+    taken[best] = 1; dead_idx[j] = best;
+  }
+  int m = 0;
+  for (int i = 0; i < n; ++i) if (!taken[i]) surv_idx[m++] = i;
+  free(taken);
+}
+
+static double logaddexp(double a, double b)
+{
+  if (a == -INFINITY) return b;
+  if (b == -INFINITY) return a;
+  const double m = a > b ? a : b;
+  return m + log(exp(a - m) + exp(b - m));
+}
+double orc_logaddexp(double a, double b) { return logaddexp(a, b); }
+
+/* ---- O12.2 evidence bookkeeping ------------------------------------------------------------ */
+void orc_evidence_update(const double *dead_logL, int n, int k, double *logX, double *logZ, double *logw)
+{
+  for (int j = 0; j < k; ++j) {
+    const double m = (double)(n - j);
+    logw[j] = *logX + log(1.0 - exp(-1.0 / m));
+    *logX = *logX - 1.0 / m;
+    *logZ = logaddexp(*logZ, dead_logL[j] + logw[j]);
+  }
+}
+
+/* ---- O12.3 tuning: mean, covariance (two-pass, 1/(n-1)), lower Cholesky --------------------- */
+int orc_tune(const double *live, int n, int d, double *mean, double *cov, double *chol)
+{
+  for (int j = 0; j < d; ++j) {
+    double s = 0.0;
+    for (int i = 0; i < n; ++i) s += live[(size_t)i * d + j];
+    mean[j] = s / n;
+  }
+  for (int a = 0; a < d; ++a)
+    for (int b = 0; b < d; ++b) {
+      double s = 0.0;
+      for (int i = 0; i < n; ++i) s += (live[(size_t)i * d + a] - mean[a]) * (live[(size_t)i * d + b] - mean[b]);
+      cov[a * d + b] = s / (n - 1);
+    }
+  for (int a = 0; a < d * d; ++a) chol[a] = 0.0;
+  for (int i = 0; i < d; ++i)
+    for (int j = 0; j <= i; ++j) {
+      double s = cov[i * d + j];
+      for (int m = 0; m < j; ++m) s -= chol[i * d + m] * chol[j * d + m];
+      if (i == j) {
+        if (!(s > 0.0)) return -1;
+        chol[i * d + i] = sqrt(s);
+      } else chol[i * d + j] = s / chol[j * d + j];
+    }
+  return 0;
+}
+
+/* ---- O12.4 one slice-sampling chain --------------------------------------------------------- */
+typedef struct {
+  const orc_problem *p; double Lstar; const double *chol;
+  int64_t n_evals; double margin;
+} chain_ctx;
+
+/* inside(t): box test first (inclusive), then logL(x + t v) > L*  (strict) */
+static int inside(chain_ctx *c, const double *x, const double *v, double t, double *y, double *ly)
+{
+  const int d = c->p->d;
+  for (int j = 0; j < d; ++j) {
+    y[j] = x[j] + t * v[j];
+    if (!(y[j] >= c->p->lo[j] && y[j] <= c->p->hi[j])) return 0;
+  }
+  const double l = orc_loglike(c->p, y);
+  c->n_evals += 1;
+  const double mg = fabs(l - c->Lstar);
+  if (mg < c->margin) c->margin = mg;
+  *ly = l;
+  return l > c->Lstar;
+}
+
+/* trace (optional): [n_repeats][3] = left expansions, right expansions, accepted shrink index (-1: none) */
+static void run_chain(chain_ctx *c, uint64_t seed, uint32_t iteration, uint32_t chain, int n_repeats,
+                      double *x, double *lx, int32_t *trace)
+{
+  const int d = c->p->d;
+  double z[ORC_NSLOT + 1], v[ORC_NSLOT], y[ORC_NSLOT];
+  for (int s = 0; s < n_repeats; ++s) {
+    /* a. direction: n = z/|z|, v = w L n */
+    for (int b = 0; b < (d + 1) / 2; ++b)
+      orc_normal_pair(seed, (uint32_t)(1 + b), (uint32_t)s, chain, iteration, &z[2 * b], &z[2 * b + 1]);
+    double nz = 0.0;
+    for (int j = 0; j < d; ++j) nz += z[j] * z[j];
+    nz = sqrt(nz);
+    for (int i = 0; i < d; ++i) {
+      double a = 0.0;
+      for (int j = 0; j <= i; ++j) a += c->chol[i * d + j] * (z[j] / nz);
+      v[i] = ORC_W * a;
+    }
+    /* b. stepping out */
+    const double u = orc_uniform_a(seed, 0u, (uint32_t)s, chain, iteration);
+    double l = -u, r = 1.0 - u, ly;
+    int nl = 0, nr = 0;
+    while (nl < ORC_MAX_EXPAND && inside(c, x, v, l, y, &ly)) { l -= 1.0; ++nl; }
+    while (nr < ORC_MAX_EXPAND && inside(c, x, v, r, y, &ly)) { r += 1.0; ++nr; }
+    /* c. shrinkage */
+    int acc = -1;
+    for (int kk = 0; kk < ORC_MAX_SHRINK; ++kk) {
+      const double uk = orc_uniform_a(seed, (uint32_t)(64 + kk), (uint32_t)s, chain, iteration);
+      const double t = l + (r - l) * uk;
+      if (inside(c, x, v, t, y, &ly)) {
+        for (int j = 0; j < d; ++j) x[j] = y[j];
+        *lx = ly; acc = kk;
+        break;
+      }
+      if (t < 0.0) l = t; else r = t;
+    }
+    if (trace) { trace[3 * s] = nl; trace[3 * s + 1] = nr; trace[3 * s + 2] = acc; }
+  }
+}
+
+/* ---- O12 one NS iteration -------------------------------------------------------------------
+ * live [n][d], logL [n] updated in place.  logLstar_in = NaN -> threshold selected internally
+ * (= highest deleted logL); otherwise it is used as given (teacher-forced form, §8(b)).
+ * Outputs (caller-allocated): dead_theta [k][d], dead_logL [k], dead_idx [k] (ascending logL),
+ * *logLstar_out, *n_evals_out; optional trace [k][n_repeats][3], margin [k].
+ * Returns 0, -1 (Cholesky pivot <= 0), -2 (bad sizes / survivor below threshold). */
+int orc_replace_step(const orc_problem *p, double *live, double *logL, int n, int k,
+                     double logLstar_in, int n_repeats, uint64_t seed, uint32_t iteration,
+                     double *dead_theta, double *dead_logL, int *dead_idx,
+                     double *logLstar_out, int64_t *n_evals_out,
+                     int32_t *trace, double *margin, int nthreads)
+{
+  const int d = p->d;
+  if (n < 2 || k < 1 || k >= n || n_repeats < 0) return -2;
+  int *surv = (int *)malloc(sizeof(int) * (n - k));
+  orc_select_lowest(logL, n, k, dead_idx, surv);
+  double Lstar = logL[dead_idx[k - 1]];
+  if (!isnan(logLstar_in)) {
+    Lstar = logLstar_in;
+    for (int i = 0; i < n - k; ++i) if (logL[surv[i]] < Lstar) { free(surv); return -2; }
+  }
+  for (int j = 0; j < k; ++j) {
+    for (int a = 0; a < d; ++a) dead_theta[(size_t)j * d + a] = live[(size_t)dead_idx[j] * d + a];
+    dead_logL[j] = logL[dead_idx[j]];
+  }
+  double mean[ORC_NSLOT], cov[ORC_NSLOT * ORC_NSLOT], chol[ORC_NSLOT * ORC_NSLOT];
+  if (orc_tune(live, n, d, mean, cov, chol) != 0) { free(surv); return -1; }
+
+  double *newx = (double *)malloc(sizeof(double) * (size_t)k * d);
+  double *newl = (double *)malloc(sizeof(double) * k);
+  int64_t total = 0;
+  if (nthreads < 1) nthreads = 1;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads) reduction(+ : total)
+  for (int c = 0; c < k; ++c) {
+    chain_ctx ctx = { p, Lstar, chol, 0, INFINITY };
+    const double u = orc_uniform_a(seed, 0u, ORC_STEP_START, (uint32_t)c, iteration);
+    int si = (int)floor(u * (double)(n - k));
+    if (si > n - k - 1) si = n - k - 1;
+    const int slot = surv[si];
+    double x[ORC_NSLOT], lx = logL[slot];
+    for (int a = 0; a < d; ++a) x[a] = live[(size_t)slot * d + a];
+    run_chain(&ctx, seed, iteration, (uint32_t)c, n_repeats, x, &lx,
+              trace ? trace + (size_t)c * n_repeats * 3 : NULL);
+    for (int a = 0; a < d; ++a) newx[(size_t)c * d + a] = x[a];
+    newl[c] = lx;
+    if (margin) margin[c] = ctx.margin;
+    total += ctx.n_evals;
+  }
+  for (int c = 0; c < k; ++c) {                                 /* O12.5 replace */
+    for (int a = 0; a < d; ++a) live[(size_t)dead_idx[c] * d + a] = newx[(size_t)c * d + a];
+    logL[dead_idx[c]] = newl[c];
+  }
+  *logLstar_out = Lstar;
+  *n_evals_out = total;
+  free(surv); free(newx); free(newl);
+  return 0;
+}
+
+static double logsumexp(const double *a, int n)
+{
+  double m = -INFINITY;
+  for (int i = 0; i < n; ++i) if (a[i] > m) m = a[i];
+  if (m == -INFINITY) return -INFINITY;
+  double s = 0.0;
+  for (int i = 0; i < n; ++i) s += exp(a[i] - m);
+  return m + log(s);
+}
+
+/* ---- O13/O14 full run ------------------------------------------------------------------------
+ * Outputs caller-allocated with cap entries: dead_theta [cap][d], dead_logL, dead_logL_birth,
+ * dead_logw.  scal[0..5] = logZ, logZ_err, H, n_iter, n_dead, n_evals.
+ * Returns 0; 1 = max_iter hit (results valid); -1 Cholesky; -3 cap too small. */
+int orc_run(const orc_problem *p, int n, int k, int n_repeats, uint64_t seed, double stop_dlogz,
+            int max_iter, int64_t cap, double *dead_theta, double *dead_logL, double *dead_logL_birth,
+            double *dead_logw, double *scal, int nthreads)
+{
+  const int d = p->d;
+  double *live = (double *)malloc(sizeof(double) * (size_t)n * d);
+  double *logL = (double *)malloc(sizeof(double) * n);
+  double *birth = (double *)malloc(sizeof(double) * n);
+  double *dth = (double *)malloc(sizeof(double) * (size_t)k * d);
+  double *dl = (double *)malloc(sizeof(double) * k);
+  double *lw = (double *)malloc(sizeof(double) * k);
+  int *didx = (int *)malloc(sizeof(int) * k);
+  orc_init_live(p, n, seed, live, logL, nthreads);
+  for (int i = 0; i < n; ++i) birth[i] = -INFINITY;
+  double logX = 0.0, logZ = -INFINITY;
+  int64_t n_dead = 0, n_evals = n;
+  int t = 0, rc = 0;
+  double logZ_live = 0.0;
+  for (;;) {
+    logZ_live = logX + logsumexp(logL, n) - log((double)n);          /* O14 */
+    if (t > 0 && logZ_live - logZ < stop_dlogz) break;
+    if (t >= max_iter) { rc = 1; break; }
+    if (n_dead + k + n > cap) { rc = -3; break; }
+    /* births of the points about to die must be read before the step overwrites the slots */
+    int *surv = (int *)malloc(sizeof(int) * (n - k));
+    orc_select_lowest(logL, n, k, didx, surv);
+    free(surv);
+    for (int j = 0; j < k; ++j) dead_logL_birth[n_dead + j] = birth[didx[j]];
+    double Lstar; int64_t ne;
+    const int r = orc_replace_step(p, live, logL, n, k, NAN, n_repeats, seed, (uint32_t)t,
+                                   dth, dl, didx, &Lstar, &ne, NULL, NULL, nthreads);
+    if (r != 0) { rc = -1; break; }
+    orc_evidence_update(dl, n, k, &logX, &logZ, lw);
+    for (int j = 0; j < k; ++j) {
+      memcpy(dead_theta + (size_t)(n_dead + j) * d, dth + (size_t)j * d, sizeof(double) * d);
+      dead_logL[n_dead + j] = dl[j];
+      dead_logw[n_dead + j] = lw[j];
+      birth[didx[j]] = Lstar;
+    }
+    n_dead += k; n_evals += ne; ++t;
+  }
+  if (rc >= 0) {
+    /* append live points, ascending logL, weight X/n each */
+    int *order = (int *)malloc(sizeof(int) * n);
+    /* ascending order of all n (ties by lower slot), by repeated selection */
+    char *taken = (char *)calloc(n, 1);
+    for (int j = 0; j < n; ++j) {
+      int best = -1;
+      for (int i = 0; i < n; ++i) { if (taken[i]) continue; if (best < 0 || logL[i] < logL[best]) best = i; }
+      taken[best] = 1; order[j] = best;
+    }
+    free(taken);
+    for (int j = 0; j < n; ++j) {
+      const int i = order[j];
+      memcpy(dead_theta + (size_t)(n_dead + j) * d, live + (size_t)i * d, sizeof(double) * d);
+      dead_logL[n_dead + j] = logL[i];
+      dead_logL_birth[n_dead + j] = birth[i];
+      dead_logw[n_dead + j] = logX - log((double)n);
+    }
+    free(order);
+    const int64_t n_iter_dead = n_dead;
+    n_dead += n;
+    const double logZf = logaddexp(logZ, logZ_live);
+    /* O15: information H and replica evidence error */
+    double H = 0.0;
+    for (int64_t i = 0; i < n_dead; ++i) {
+      const double lp = dead_logL[i] + dead_logw[i] - logZf;
+      if (dead_logL[i] > -INFINITY) H += exp(lp) * (dead_logL[i] - logZf);
+    }
+    const int R = 200;
+    double sum = 0.0, sum2 = 0.0;
+    for (int rpl = 0; rpl < R; ++rpl) {
+      double lX = 0.0, lZ = -INFINITY;
+      for (int64_t j = 0; j < n_iter_dead; ++j) {
+        const double m = (double)(n - (int)(j % k));
+        uint64_t ka, kb; orc_draw53(seed, 0u, (uint32_t)j, (uint32_t)rpl, ORC_ITER_ERR, &ka, &kb);
+        const double lnt = log((double)(ka + 1) * TWO_M53) / m;
+        const double lXn = lX + lnt;
+        /* w_j = X_{j-1} - X_j */
+        const double lwj = lX + log1p(-exp(lXn - lX));
+        lZ = logaddexp(lZ, dead_logL[j] + lwj);
+        lX = lXn;
+      }
+      double ls = -INFINITY;
+      for (int j = 0; j < n; ++j) ls = logaddexp(ls, logL[j]);
+      lZ = logaddexp(lZ, lX + ls - log((double)n));
+      sum += lZ; sum2 += lZ * lZ;
+    }
+    const double mu = sum / R;
+    double var = sum2 / R - mu * mu; if (var < 0) var = 0;
+    scal[0] = logZf; scal[1] = sqrt(var * R / (R - 1)); scal[2] = H;
+  }
+  scal[3] = (double)t; scal[4] = (double)n_dead; scal[5] = (double)n_evals;
+  free(live); free(logL); free(birth); free(dth); free(dl); free(lw); free(didx);
+  return rc;
+}
+
+int orc_version(void) { return 1; }

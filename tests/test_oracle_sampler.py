@@ -1,0 +1,258 @@
+"""Pins for the sampler half of the oracle."""
+import math
+import os
+import shutil
+import subprocess
+import tempfile
+
+import numpy as np
+import pytest
+import scipy.special
+import scipy.stats
+
+from paper_2509_24949_b200 import inputs
+
+
+# ---- P10: Philox4x32-10 against cuRAND's own routine (host-compiled from the CUDA header) ---------
+_CURAND_HOST = r"""
+#include <cstdio>
+#include <cuda_runtime.h>
+#define QUALIFIERS static inline __host__ __device__
+#include <curand_philox4x32_x.h>
+int main() {
+  unsigned int s = 12345u;
+  for (int i = 0; i < 64; ++i) {
+    unsigned int v[6];
+    for (int j = 0; j < 6; ++j) { s = s * 1664525u + 1013904223u; v[j] = (i < 8 && j != (i % 6)) ? 0u : s; }
+    if (i == 8) for (int j = 0; j < 6; ++j) v[j] = 0xFFFFFFFFu;
+    uint4 c = make_uint4(v[0], v[1], v[2], v[3]); uint2 k = make_uint2(v[4], v[5]);
+    uint4 o = curand_Philox4x32_10(c, k);
+    printf("%u %u %u %u %u %u %u %u %u %u\n", v[0], v[1], v[2], v[3], v[4], v[5], o.x, o.y, o.z, o.w);
+  }
+  return 0;
+}
+"""
+
+
+@pytest.mark.skipif(shutil.which("nvcc") is None, reason="nvcc (for the cuRAND header) not found")
+def test_p10_philox_matches_curand_host(oracle):
+    with tempfile.TemporaryDirectory() as td:
+        src, exe = os.path.join(td, "p.cu"), os.path.join(td, "p")
+        open(src, "w").write(_CURAND_HOST)
+        subprocess.run(["nvcc", "-O1", "-o", exe, src], check=True, capture_output=True)
+        out = subprocess.run([exe], check=True, capture_output=True, text=True).stdout
+    rows = [list(map(int, ln.split())) for ln in out.strip().splitlines()]
+    assert len(rows) == 64
+    for r in rows:
+        assert oracle.philox(r[4:6], r[0:4]) == tuple(r[6:10])
+
+
+def test_p10_philox_is_a_bijection_sample_and_key_sensitive(oracle):
+    outs = {oracle.philox((1, 2), (i, 0, 0, 0)) for i in range(2000)}
+    assert len(outs) == 2000
+    assert oracle.philox((1, 2), (5, 6, 7, 8)) != oracle.philox((1, 3), (5, 6, 7, 8))
+    # each counter word matters
+    base = oracle.philox((9, 9), (1, 1, 1, 1))
+    for j in range(4):
+        c = [1, 1, 1, 1]; c[j] = 2
+        assert oracle.philox((9, 9), c) != base
+
+
+# ---- P11: uniforms and normals ----------------------------------------------------------------------
+def test_p11_uniform_and_normal_moments(oracle):
+    n = 40000
+    ka = np.array([oracle.draw53(3, 0, s, 1, 0) for s in range(n)], dtype=np.float64)
+    u = ka.ravel() * 2.0 ** -53
+    assert u.min() >= 0.0 and u.max() < 1.0
+    assert abs(u.mean() - 0.5) < 4 * math.sqrt(1 / 12 / u.size)
+    assert scipy.stats.kstest(u, "uniform").pvalue > 1e-3
+    # 53-bit assembly: ka = (w0 >> 5) * 2^26 + (w1 >> 6)
+    w = oracle.philox((3, 0), (0, 17, 1, 0))
+    assert oracle.draw53(3, 0, 17, 1, 0) == ((w[0] >> 5) * 2 ** 26 + (w[1] >> 6), (w[2] >> 5) * 2 ** 26 + (w[3] >> 6))
+    assert oracle.uniform_a(3, 0, 17, 1, 0) == ((w[0] >> 5) * 2 ** 26 + (w[1] >> 6)) * 2.0 ** -53
+    # seed high word is key[1]
+    assert oracle.draw53((5 << 32) | 3, 0, 17, 1, 0) != oracle.draw53(3, 0, 17, 1, 0)
+    z = np.array([oracle.normal_pair(3, 1, s, 2, 0) for s in range(n)]).ravel()
+    assert np.all(np.isfinite(z))
+    assert abs(z.mean()) < 4 / math.sqrt(z.size) and abs(z.var() - 1) < 0.03
+    assert scipy.stats.kstest(z, "norm").pvalue > 1e-3
+    zz = np.array([oracle.normal_pair(3, 1, s, 2, 0) for s in range(2000)])
+    assert abs(np.corrcoef(zz[:, 0], zz[:, 1])[0, 1]) < 0.08
+    # Box-Muller radius/angle from the documented u's
+    ka_, kb_ = oracle.draw53(3, 1, 5, 2, 0)
+    r, a = math.sqrt(-2 * math.log((ka_ + 1) * 2.0 ** -53)), 2 * math.pi * kb_ * 2.0 ** -53
+    assert oracle.normal_pair(3, 1, 5, 2, 0) == pytest.approx((r * math.cos(a), r * math.sin(a)), rel=1e-14)
+
+
+# ---- P12: bookkeeping against library routines -------------------------------------------------------
+def test_p12_select_lowest_vs_stable_argsort(oracle):
+    rng = np.random.default_rng(0)
+    for n, k in ((10, 3), (100, 50), (1000, 500), (257, 256), (64, 1)):
+        l = rng.normal(size=n)
+        l[rng.integers(0, n, n // 5)] = l[0]                 # ties
+        if n > 20:
+            l[3] = -np.inf
+        dead, surv = oracle.select_lowest(l, k)
+        order = np.argsort(l, kind="stable")
+        assert np.array_equal(dead, order[:k])
+        assert np.array_equal(surv, np.sort(order[k:]))
+
+
+def test_p12_tune_vs_numpy(oracle):
+    rng = np.random.default_rng(1)
+    scales = np.array([1.0, 0.1, 0.5, 0.5, 600.0, 1e-3, 1.5, 0.3, 0.6, 0.01, 0.014])
+    A = rng.normal(size=(11, 11))
+    x = rng.normal(size=(1000, 11)) @ A.T * scales + 1e3 * scales
+    rc, mean, cov, chol = oracle.tune(x)
+    assert rc == 0
+    assert np.allclose(mean, x.mean(0), rtol=1e-13)
+    assert np.allclose(cov, np.cov(x.T), rtol=1e-10)
+    assert np.allclose(chol, np.linalg.cholesky(np.cov(x.T)), rtol=1e-8, atol=0)
+    assert np.allclose(chol @ chol.T, cov, rtol=1e-11)
+    assert np.all(np.triu(chol, 1) == 0)
+    # degenerate population -> pivot failure reported
+    x2 = x.copy(); x2[:, 3] = x2[:, 2]
+    assert oracle.tune(x2)[0] != 0
+
+
+def test_p12_p14_evidence_update(oracle):
+    n, k = 1000, 500
+    rng = np.random.default_rng(2)
+    dl = np.sort(rng.normal(size=k) * 5 - 20)
+    logX, logZ, lw = oracle.evidence_update(dl, n, 0.0, -np.inf)
+    m = n - np.arange(k)
+    assert logX == pytest.approx(-np.sum(1.0 / m), rel=1e-13)
+    assert logZ == pytest.approx(scipy.special.logsumexp(dl + lw), rel=1e-13)
+    # weights are the shell volumes X_{j-1} - X_j: they and the remaining volume sum to exactly 1
+    assert np.sum(np.exp(lw)) + math.exp(logX) == pytest.approx(1.0, abs=1e-13)
+    Xs = np.exp(-np.concatenate([[0.0], np.cumsum(1.0 / m)]))
+    assert np.allclose(np.exp(lw), Xs[:-1] - Xs[1:], rtol=1e-11)
+    # a second batch continues from the first
+    logX2, logZ2, lw2 = oracle.evidence_update(dl + 1, n, logX, logZ)
+    assert logX2 == pytest.approx(2 * logX, rel=1e-13)
+    assert logZ2 == pytest.approx(scipy.special.logsumexp(np.concatenate([dl + lw, dl + 1 + lw2])), rel=1e-13)
+    assert oracle.lib().orc_logaddexp(-np.inf, -3.0) == -3.0
+
+
+# ---- P13: the slice sampler alone -----------------------------------------------------------------------
+def test_p13_no_constraint_gives_uniform_in_box(oracle):
+    d, n, k = 4, 1000, 500
+    w = inputs.gaussian_workload(d, sigma=1.0)
+    p = oracle.Problem(w)
+    rng = np.random.default_rng(3)
+    live = rng.uniform(-0.2, 0.2, size=(n, d))           # concentrated start: must spread to the box
+    live[::2] = rng.uniform(-1, 1, size=(n // 2, d))     # (covariance still spans the box)
+    logL = p.loglike_batch(live)
+    r = p.replace_step(live, logL, k, 40, seed=11, iteration=0, logLstar=-math.inf, want_trace=True)
+    assert r["rc"] == 0
+    new = r["live"][r["dead_idx"]]
+    assert np.all(new >= -1) and np.all(new <= 1)
+    for j in range(d):
+        assert scipy.stats.kstest((new[:, j] + 1) / 2, "uniform").pvalue > 1e-3
+    assert np.all(r["trace"][:, :, 2] >= 0)              # every step accepted something
+
+
+def test_p13_ball_constraint_gives_uniform_in_ball(oracle):
+    d, n, k, R = 4, 2000, 1000, 0.8
+    w = inputs.gaussian_workload(d, sigma=1.0)
+    p = oracle.Problem(w)
+    rng = np.random.default_rng(4)
+    x = rng.uniform(-1, 1, size=(12 * n, d))
+    x = x[np.sum(x * x, 1) < R * R][:n]
+    assert x.shape[0] == n
+    logL = p.loglike_batch(x)
+    Lstar = -0.5 * R * R
+    r = p.replace_step(x, logL, k, 30, seed=5, iteration=3, logLstar=Lstar)
+    assert r["rc"] == 0 and r["logLstar"] == Lstar
+    new = r["live"][r["dead_idx"]]
+    rad = np.sqrt(np.sum(new * new, 1))
+    assert rad.max() < R
+    assert np.all(r["logL"][r["dead_idx"]] > Lstar)
+    assert scipy.stats.kstest((rad / R) ** d, "uniform").pvalue > 1e-3
+    # new logL values are the likelihood of the new positions
+    assert np.allclose(r["logL"][r["dead_idx"]], p.loglike_batch(new), rtol=0, atol=0)
+    # survivors untouched
+    surv = np.setdiff1d(np.arange(n), r["dead_idx"])
+    assert np.array_equal(r["live"][surv], x[surv])
+    # a survivor below the supplied threshold is rejected (teacher-forced contract)
+    assert p.replace_step(x, logL, k, 1, 5, 3, logLstar=0.0)["rc"] == -2
+
+
+def test_p13_determinism_and_thread_independence(oracle):
+    w = inputs.gaussian_workload(3, sigma=0.3)
+    p = oracle.Problem(w)
+    live, logL = p.init_live(200, 9)
+    a = p.replace_step(live, logL, 100, 6, 9, 0, nthreads=1, want_trace=True)
+    b = p.replace_step(live, logL, 100, 6, 9, 0, nthreads=4, want_trace=True)
+    c = p.replace_step(live, logL, 100, 6, 9, 1, nthreads=4)
+    assert np.array_equal(a["live"], b["live"]) and np.array_equal(a["trace"], b["trace"]) and a["n_evals"] == b["n_evals"]
+    assert not np.array_equal(a["live"], c["live"])
+    # initial live points: theta_j = lo + (hi - lo) u with block j/2, lane j%2 (O11 stream layout)
+    ka, kb = oracle.draw53(9, 1, 0, 7, 0xFFFFFFFF)
+    assert live[7, 2] == -1.0 + 2.0 * (ka * 2.0 ** -53)
+    ka, kb = oracle.draw53(9, 0, 0, 7, 0xFFFFFFFF)
+    assert live[7, 1] == -1.0 + 2.0 * (kb * 2.0 ** -53)
+    # eval count = stepping-out tests + shrink tries inside the box; trace is consistent with it
+    tr = a["trace"]
+    assert a["n_evals"] <= np.sum(tr[:, :, 0] + 1 + tr[:, :, 1] + 1 + tr[:, :, 2] + 1)
+
+
+# ---- P14 / P15 / P16: full NS run on the Gaussian test likelihood --------------------------------------
+def _analytic_logz(d, sigma, half):
+    c = scipy.stats.norm.cdf(half / sigma) - scipy.stats.norm.cdf(-half / sigma)
+    return d * math.log(sigma * math.sqrt(2 * math.pi) / (2 * half) * c)
+
+
+@pytest.mark.parametrize("d,n,k,seed", [(4, 1000, 500, 1), (4, 400, 100, 2), (11, 600, 300, 3)])
+def test_p15_p16_gaussian_evidence_and_posterior(oracle, d, n, k, seed):
+    sigma = 0.05
+    w = inputs.gaussian_workload(d, sigma=sigma)
+    p = oracle.Problem(w)
+    r = p.run(n, k, 5 * d, seed)
+    assert r["rc"] == 0
+    truth = _analytic_logz(d, sigma, 1.0)
+    assert 0.02 < r["logZ_err"] < 0.6
+    assert abs(r["logZ"] - truth) < 3 * r["logZ_err"]
+    # closed-form cross-check of the error estimate: sigma^2 ~ H * sum(1/m^2)/sum(1/m) per iteration
+    m = n - np.arange(k)
+    approx = math.sqrt(r["H"] * np.sum(1.0 / m ** 2) / np.sum(1.0 / m))
+    assert 0.5 < r["logZ_err"] / approx < 2.0
+    # H of a Gaussian posterior in a wide box: H = -logZ - d/2  (KL(posterior || prior), peak logL = 0)
+    assert r["H"] == pytest.approx(-truth - d / 2, abs=0.5)
+    # P14 invariants
+    nd, ni = r["n_dead"], r["n_iter"]
+    assert nd == ni * k + n
+    assert np.sum(np.exp(r["dead_logw"])) == pytest.approx(1.0, abs=1e-10)
+    dl = r["dead_logL"]
+    assert np.all(np.diff(dl[:ni * k]) >= 0) and np.all(np.diff(dl[ni * k:]) >= 0)
+    assert np.all(r["dead_logL_birth"] < dl)
+    mm = np.concatenate([n - np.arange(k)] * ni)
+    assert r["dead_logw"][ni * k] == pytest.approx(-np.sum(1.0 / mm) - math.log(n), rel=1e-12)
+    # P16 posterior moments
+    pw = np.exp(dl + r["dead_logw"] - r["logZ"])
+    assert pw.sum() == pytest.approx(1.0, abs=1e-9)
+    ess = 1.0 / np.sum(pw ** 2)
+    mean = pw @ r["dead_theta"]
+    sd = np.sqrt(pw @ (r["dead_theta"] - mean) ** 2)
+    assert np.all(np.abs(mean) < 5 * sigma / math.sqrt(ess))
+    assert np.all(np.abs(sd / sigma - 1) < 0.15)
+
+
+def test_run_matches_stepwise_composition(oracle):
+    """orc_run is exactly init_live + repeated replace_step + evidence_update (O12-O14)."""
+    w = inputs.gaussian_workload(3, sigma=0.1)
+    p = oracle.Problem(w)
+    n, k, nr, seed = 200, 100, 9, 4
+    r = p.run(n, k, nr, seed)
+    live, logL = p.init_live(n, seed)
+    logX, logZ, t = 0.0, -np.inf, 0
+    while True:
+        lzl = logX + scipy.special.logsumexp(logL) - math.log(n)
+        if t > 0 and lzl - logZ < -3.0:
+            break
+        s = p.replace_step(live, logL, k, nr, seed, t)
+        logX, logZ, lw = oracle.evidence_update(s["dead_logL"], n, logX, logZ)
+        live, logL = s["live"], s["logL"]
+        t += 1
+    assert t == r["n_iter"]
+    assert np.logaddexp(logZ, lzl) == pytest.approx(r["logZ"], rel=1e-13)

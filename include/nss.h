@@ -1,0 +1,176 @@
+/*
+ * nss.h — C ABI of libnss.so: the B200 (sm_100a) hot path of "Parallel Nested Slice Sampling for
+ * Gravitational Wave Parameter Estimation" (arxiv 2509.24949; /root/reference/PAPER.md).
+ *
+ * One batched nested-slice-sampling replacement step whose every chain step
+ * evaluates a heterodyned / relative-binning frequency-domain GW log-likelihood (PAPER.md:33, 39,
+ * 49), plus the on-device nested-sampling bookkeeping and a full-frequency-grid likelihood.
+ * The paper prints no equations; the operations are defined by SURVEY.md §8(c) O1..O16 (restated
+ * in DESIGN.md §3), cited per call below.
+ *
+ * Conventions
+ *  - Every call returns 0 on success or a negative NSS_E* code; nothing throws or aborts.
+ *  - "device" pointers are CUDA device pointers on the device the handle was created on
+ *    (e.g. torch tensor.data_ptr()); "host" pointers are ordinary host memory.
+ *  - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *  - All floating point is IEEE fp64.  Row-major everywhere.
+ *  - One handle serves one stream at a time (not re-entrant).  Single GPU.  There is NO CPU
+ *    fallback: without a CUDA device every compute call returns NSS_ECUDA.
+ *  - Ownership: nss_create deep-copies everything it needs (the caller may free psd/data when it
+ *    returns); the handle owns its device tables and scratch; every output buffer is allocated by
+ *    the caller; the library never frees caller memory.
+ */
+#ifndef NSS_H
+#define NSS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NSS_NSLOT 11      /* canonical parameter slots, O2 */
+#define NSS_MAXDET 4
+
+/* canonical slot order (O2): 0 Mc [Msun, detector frame], 1 q = m2/m1 in (0,1], 2 chi1z, 3 chi2z,
+ * 4 dL [Mpc], 5 tc [s], 6 phic [rad], 7 iota, 8 psi, 9 ra, 10 dec.
+ * Physical domain: Mc > 0, 0 < q <= 1, |chi| < 1, dL > 0, everything finite; outside it the
+ * log-likelihood is -inf (not an error). */
+
+enum {
+  NSS_OK = 0,
+  NSS_EINVAL = -1,    /* bad sizes, lo >= hi, PSD <= 0, n_delete >= n_live, fiducial outside domain,
+                         survivor below a supplied logLstar, NULL pointer */
+  NSS_ENOMEM = -2,    /* host or device allocation failed */
+  NSS_ECUDA = -3,     /* a CUDA call failed (no device, launch error); see nss_last_cuda_error */
+  NSS_ECHOL = -4,     /* non-positive Cholesky pivot of the live-point covariance */
+  NSS_ECAP = -5,      /* nss_result arrays too small */
+  NSS_ENOTCONV = -6   /* nss_run hit max_iter; the results written are still valid */
+};
+
+enum { NSS_KIND_RB = 0, NSS_KIND_FULL = 1, NSS_KIND_GAUSS = 2 };
+
+typedef struct nss_handle nss_handle; /* opaque */
+
+typedef struct {
+  double vertex_m[3], xarm[3], yarm[3];   /* Earth-fixed frame; arms are unit vectors (O4) */
+} nss_detector;
+
+typedef struct {
+  int32_t d;                       /* sampled dimensions, 1..11                                  */
+  int32_t param_index[NSS_NSLOT];  /* sampled dim j -> canonical slot (kinds 0, 1)               */
+  double  theta_fixed[NSS_NSLOT];  /* canonical values for unsampled slots                       */
+  double  lo[NSS_NSLOT], hi[NSS_NSLOT]; /* uniform prior box per sampled dim, lo < hi (A22)      */
+  int32_t n_det;                   /* 1..4 (kinds 0, 1)                                          */
+  nss_detector det[NSS_MAXDET];
+  double  gmst;                    /* Greenwich sidereal angle [rad]                             */
+  int32_t n_freq;                  /* grid f_k = f_min + k*df, k = 0..n_freq-1                   */
+  double  f_min, df;
+  const double *psd;               /* host, [n_det][n_freq], one-sided, > 0                      */
+  const double *data;              /* host, [n_det][n_freq][2] = complex128 (re, im)             */
+  double  theta_fid[NSS_NSLOT];    /* canonical heterodyne reference, kind 0       */
+  int32_t n_bins;                  /* B, 1 <= B <= n_freq-1, kind 0                              */
+  int32_t kind;                    /* NSS_KIND_*                                                 */
+  double  gauss_mu[NSS_NSLOT], gauss_sigma[NSS_NSLOT]; /* per sampled dim, kind 2 (O16)          */
+} nss_config;
+
+/* Setup (heterodyne reference fixed in advance, excluded from quoted runtimes).
+ * Host: validates, chooses the bin edges (O8), evaluates the fiducial waveform (O3, O4), builds the
+ * per-(detector, bin) summary data A0, A1, B0, B1 and <d,d> (O9), packs the device tables and
+ * uploads them.  Synchronous. */
+int nss_create(const nss_config *cfg, nss_handle **out);
+int nss_destroy(nss_handle *h);
+
+/* Batched log-likelihood (O10 relative binning, O7 full grid or O16 Gaussian, by cfg.kind).
+ * theta_dev: device [N][d] sampled coordinates; logL_dev: device [N].  Evaluates any theta (inside
+ * the prior box or not); outside the physical domain or non-finite -> -inf.  N = 0 is a no-op.
+ * Asynchronous on the stream. */
+int nss_loglike_batch(nss_handle *h, const double *theta_dev, int64_t N, double *logL_dev,
+                      void *cuda_stream);
+
+/* Variant selector for nss_loglike_batch (profiling / tests): 0 = automatic (default),
+ * 1 = one thread per point, 2 = one warp per point. */
+int nss_set_loglike_variant(nss_handle *h, int32_t variant);
+
+/* One NS iteration (O12): select the n_delete lowest logL (ascending, ties by lower slot), tune the
+ * slice directions from the covariance of the full live set (Cholesky), run one chain per deleted
+ * point (start = uniformly chosen survivor; n_repeats x {direction, stepping-out, shrinkage} under
+ * logL > logLstar inside the prior box), overwrite the deleted slots in place.
+ * live_dev [n_live][d] and logL_dev [n_live] are updated in place.  logLstar = NaN: the threshold is
+ * the highest deleted logL; otherwise the supplied value is used and every survivor must have
+ * logL >= logLstar (NSS_EINVAL if not) — the teacher-forced form used for trajectory parity.
+ * Random numbers: Philox4x32-10, key = seed, counter = (block, step, chain, iteration) (O11).
+ * Outputs: dead_theta_dev [n_delete][d], dead_logL_dev [n_delete], dead_idx_dev [n_delete]
+ * (ascending logL); *logLstar_host, *n_evals_host (sequential-algorithm likelihood evaluations).
+ * Synchronises the stream before returning. */
+int nss_replace_step(nss_handle *h, double *live_dev, double *logL_dev, int32_t n_live,
+                     int32_t n_delete, double logLstar, int32_t n_repeats, uint64_t seed,
+                     uint32_t iteration, double *dead_theta_dev, double *dead_logL_dev,
+                     int32_t *dead_idx_dev, double *logLstar_host, int64_t *n_evals_host,
+                     void *cuda_stream);
+
+/* Test hook: if set (device pointers, may be NULL to clear), the next nss_replace_step calls also
+ * write trace_dev [n_delete][n_repeats][3] = (left expansions, right expansions, accepted shrink
+ * index or -1) and margin_dev [n_delete] = min |logL - logLstar| over the chain's bracket tests. */
+int nss_set_trace(nss_handle *h, int32_t *trace_dev, double *margin_dev);
+
+/* K4 bookkeeping kernels on their own (O12.1, O12.3, O12.2). */
+int nss_select_lowest(nss_handle *h, const double *logL_dev, int32_t n_live, int32_t n_delete,
+                      int32_t *dead_idx_dev /*[n_delete] ascending logL, ties by slot*/,
+                      int32_t *surv_idx_dev /*[n_live-n_delete] ascending slot, may be NULL*/,
+                      double *logLstar_host, void *cuda_stream);
+int nss_tune(nss_handle *h, const double *live_dev, int32_t n_live, double *mean_dev /*[d]*/,
+             double *chol_dev /*[d][d] lower, row-major*/, void *cuda_stream);
+/* logw_j = logX + ln(1 - e^{-1/m_j}), m_j = n_live - j; logX -= sum 1/m_j; logZ = logaddexp(...).
+ * state_host[2] = {logX, logZ} in/out. */
+int nss_evidence_update(nss_handle *h, const double *dead_logL_dev, int32_t n_live, int32_t n_delete,
+                        double *logw_dev /*[n_delete]*/, double *state_host, void *cuda_stream);
+/* Initial live points (O13): uniform in the box from the Philox stream, then their logL. */
+int nss_init_live(nss_handle *h, int32_t n_live, uint64_t seed, double *live_dev, double *logL_dev,
+                  void *cuda_stream);
+/* Philox test hook: out_dev [n][4] uint32 = Philox4x32-10(key = seed, counter = ctr_dev[i][4]). */
+int nss_philox(nss_handle *h, uint64_t seed, const uint32_t *ctr_dev, int64_t n, uint32_t *out_dev,
+               void *cuda_stream);
+
+typedef struct {
+  double  logZ, logZ_err, H;       /* evidence, its replica s.d. (O15), information             */
+  int32_t n_iter;
+  int64_t n_dead, n_evals;         /* rows written; sequential-algorithm likelihood evaluations  */
+  double *dead_theta;              /* host [cap][d]   caller-allocated                           */
+  double *dead_logL;               /* host [cap]                                                 */
+  double *dead_logL_birth;         /* host [cap]                                                 */
+  double *dead_logw;               /* host [cap]      log prior-volume weight                    */
+  int64_t cap;                     /* >= n_iter*n_delete + n_live                                */
+  double  gpu_ms;                  /* device time of the run (CUDA events), setup excluded       */
+} nss_result;
+
+/* Full run (O13, O14): initial live points, NS iterations until logZ_live - logZ < stop_dlogz
+ * (default -3.0) or max_iter, then the live points are appended (ascending logL, weight X/n).
+ * Everything stays on the device; results are copied to the caller's host arrays at the end. */
+int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t n_repeats, uint64_t seed,
+            double stop_dlogz, int32_t max_iter, nss_result *out, void *cuda_stream);
+
+/* Host-side strain of one detector on an arbitrary frequency list (O3, O4), the routine nss_create
+ * uses for the fiducial waveform; out [n][2].  Used by bench.py to synthesise injections. */
+int nss_waveform(const double *theta_canon /*[11]*/, const nss_detector *det, double gmst,
+                 const double *freqs, int32_t n, double *out);
+
+/* Read back the setup tables (tests): bin-edge grid indices [B+1] and summary data
+ * [n_det][B][6] = (A0re, A0im, A1re, A1im, B0, B1) as defined in O9 (unscaled). */
+int nss_get_tables(nss_handle *h, int32_t *edge_idx_host, double *summary_host, double *dd_host);
+
+/* Register-resident DFMA chain on every SM for ~`ms` milliseconds: measured fp64 FMA throughput,
+ * the roofline denominator.  *tflops_host = 2 * FMA/s / 1e12. */
+int nss_fp64_peak(double ms, double *tflops_host, void *cuda_stream);
+
+/* Kernel launches issued by this handle since creation (bench.py's gpu_launches). */
+int64_t nss_launch_count(const nss_handle *h);
+
+const char *nss_strerror(int code);
+const char *nss_last_cuda_error(void);
+int nss_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NSS_H */

@@ -1,0 +1,68 @@
+// nss_internal.cuh — handle, device-side problem description and launch helpers (CUDA path only).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "../../include/nss.h"
+#include "nss_physics.cuh"
+
+// Device-side problem description, passed to kernels by value (__grid_constant__).
+struct NssDev {
+  int32_t d, n_det, kind, n_bins, n_edges, n_freq;
+  int32_t param_index[NSS_NSLOT];
+  double theta_fixed[NSS_NSLOT];
+  double lo[NSS_NSLOT], hi[NSS_NSLOT];
+  double gauss_mu[NSS_NSLOT], gauss_isig[NSS_NSLOT];
+  double D6[NSS_MAXDET][6];   // symmetric detector tensors (O4)
+  double rc[NSS_MAXDET][3];   // vertex / c [s]
+  double gmst;
+  // heterodyne reference (kind 0)
+  double c_fid[nssp::kNB], c_const_fid, tc_fid;
+  double inv_a0[NSS_MAXDET][2];   // 1 / (complex amplitude of the fiducial waveform per detector)
+  double tau_fid[NSS_MAXDET];
+  double half_DD;                 // 1/2 sum_det <d,d>
+  // tables (device pointers owned by the handle)
+  const double *rb_rec;   // AoS  [E][rb_rs]: g0..g7, F_e, pad, then per det 6 pre-scaled bin terms of bin e-1
+  int32_t rb_rs;
+  const double *rb_soa;   // warp layout: edge part [9][m+1][32], then bin part [n_det*6][m][32]
+  int32_t rb_m;           // bins per lane = ceil(B/32)
+  const double *full_rec; // AoS [n_freq][full_rs]: g0..g7, f, f^-7/6, then per det (d_re, d_im, 4df/S), pad
+  int32_t full_rs;
+};
+
+struct nss_handle {
+  NssDev dev;
+  int device;
+  int n_sm;
+  int loglike_variant;
+  int64_t launches;
+  // host copies kept for nss_get_tables
+  std::vector<int32_t> edge_idx;
+  std::vector<double> summary;     // [n_det][B][6]
+  double DD;
+  // device allocations
+  double *d_rb_rec, *d_rb_soa, *d_full_rec;
+  size_t rb_rec_bytes, rb_soa_bytes, full_rec_bytes;
+  // sampler scratch (grown on demand)
+  int32_t scratch_n;
+  int32_t *d_surv_idx, *d_dead_idx, *d_rank, *d_flags;   // flags: [0] chol error, [1] threshold violation, [2] done
+  double *d_mean, *d_chol, *d_state;                      // state: logX, logZ, logZ_live, Lstar
+  unsigned long long *d_nevals;
+  double *d_birth;
+  int32_t *trace_dev;
+  double *margin_dev;
+};
+
+extern thread_local char g_nss_cuda_err[256];
+int nss_cuda_fail(cudaError_t e, const char *where);
+#define NSS_CUDA(x)                                              \
+  do {                                                           \
+    cudaError_t e__ = (x);                                       \
+    if (e__ != cudaSuccess) return nss_cuda_fail(e__, #x);       \
+  } while (0)
+
+// launchers implemented in nss_loglike.cu
+int nss_launch_loglike(nss_handle *h, const double *theta, int64_t N, double *logL, cudaStream_t st);
+// sampler entry points implemented in nss_sampler.cu use the device functions of nss_loglike_dev.cuh

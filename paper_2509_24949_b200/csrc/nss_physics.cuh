@@ -1,0 +1,150 @@
+// nss_physics.cuh — waveform / detector-response arithmetic of the CUDA path (host setup + kernels).
+//
+// TaylorF2 3.5PN phase + 1.5PN spin-orbit, Newtonian amplitude (BASELINE.json
+// configs) and the detector response (O4), arranged for the kernels:
+//
+//   phase in TURNS   Psi(f)/(2 pi) = sum_{j<8} c_j g_j(f) + c_const + f * tc
+//   basis            g = f^-5/3, f^-1, f^-2/3, f^-1/3, ln f, f^1/3, f^1/3 ln f, f^2/3
+//
+// so a kernel evaluates the phase at a tabulated frequency with 8 FMAs against theta-dependent
+// coefficients, plus one FMA per detector for the arrival-time term f*(tc + dt_det).
+// This file shares nothing with oracle/ (which evaluates the defining formula directly).
+#pragma once
+#include <math.h>
+#include <stdint.h>
+
+#if defined(__CUDACC__)
+#define NSS_HD __host__ __device__ __forceinline__
+#else
+#define NSS_HD inline
+#endif
+
+namespace nssp {
+
+constexpr double kGMsun = 4.925490947641267e-6;   // G Msun / c^3 [s]   (O1)
+constexpr double kMpc = 3.085677581491367e22;     // [m]
+constexpr double kC = 299792458.0;                // [m/s]
+constexpr double kEuler = 0.5772156649015329;
+constexpr double kPi = 3.14159265358979323846;
+constexpr int kNB = 8;                             // phase basis functions (above)
+constexpr int kNSlot = 11;
+
+struct Intrinsic {
+  double c[kNB];     // phase coefficients, turns
+  double c_const;    // frequency-independent phase, turns
+  double tc;         // coefficient of f, turns/Hz = seconds
+  double amp;        // Newtonian amplitude A (multiplies f^-7/6), O3
+  double cos_iota;
+};
+
+NSS_HD bool domain_ok(const double *th)
+{
+  bool ok = true;
+#pragma unroll
+  for (int j = 0; j < kNSlot; ++j) ok = ok && isfinite(th[j]);
+  ok = ok && (th[0] > 0.0) && (th[1] > 0.0) && (th[1] <= 1.0);
+  ok = ok && (fabs(th[2]) < 1.0) && (fabs(th[3]) < 1.0) && (th[4] > 0.0);
+  return ok;
+}
+
+// O3: PN coefficients regrouped by power of f.  v = u f^(1/3), u = (pi M)^(1/3).
+NSS_HD void intrinsic(const double *th, Intrinsic &I)
+{
+  const double Mc = th[0], q = th[1], chi1 = th[2], chi2 = th[3], dL = th[4];
+  const double opq = 1.0 + q;
+  const double m1 = 1.0 / opq, m2 = q * m1;
+  const double eta = q * m1 * m1;
+  const double M = Mc * pow(eta, -0.6) * kGMsun;
+  const double u = cbrt(kPi * M);
+  const double lnu = log(u);
+  const double K = 3.0 / (128.0 * eta) / (2.0 * kPi);          // turns
+  const double eta2 = eta * eta;
+  const double beta = (113.0 / 12.0 * m1 * m1 + 6.25 * eta) * chi1 + (113.0 / 12.0 * m2 * m2 + 6.25 * eta) * chi2;
+  const double phi2 = 3715.0 / 756.0 + 55.0 / 9.0 * eta;
+  const double phi3 = -16.0 * kPi + 4.0 * beta;
+  const double phi4 = 15293365.0 / 508032.0 + 27145.0 / 504.0 * eta + 3085.0 / 72.0 * eta2;
+  const double P5 = kPi * (38645.0 / 756.0 - 65.0 / 9.0 * eta);
+  const double Q6 = 11583231236531.0 / 4694215680.0 - 640.0 / 3.0 * kPi * kPi - 6848.0 / 21.0 * kEuler
+                  + eta * (-15737765635.0 / 3048192.0 + 2255.0 / 12.0 * kPi * kPi)
+                  + 76055.0 / 1728.0 * eta2 - 127825.0 / 1296.0 * eta2 * eta;
+  const double phi7 = kPi * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * eta2);
+  const double iu = 1.0 / u, iu2 = iu * iu;
+  const double ln_vlso = -0.5 * log(6.0);
+  const double ln4 = 1.3862943611198906188;
+  I.c[0] = K * iu2 * iu2 * iu;                                  // f^-5/3
+  I.c[1] = K * phi2 * iu2 * iu;                                 // f^-1
+  I.c[2] = K * phi3 * iu2;                                      // f^-2/3
+  I.c[3] = K * phi4 * iu;                                       // f^-1/3
+  I.c[4] = K * P5;                                              // ln f      (3 ln v = 3 ln u + ln f)
+  I.c[5] = K * u * (Q6 - 6848.0 / 21.0 * (ln4 + lnu));          // f^1/3
+  I.c[6] = -K * u * (6848.0 / 63.0);                            // f^1/3 ln f
+  I.c[7] = K * phi7 * u * u;                                    // f^2/3
+  I.c_const = (-th[6] - 0.25 * kPi) / (2.0 * kPi) + K * P5 * (1.0 + 3.0 * (lnu - ln_vlso));
+  I.tc = th[5];
+  I.amp = 0.45643546458763842789 /* sqrt(5/24) */ * pow(kPi, -2.0 / 3.0) * pow(Mc * kGMsun, 5.0 / 6.0) * kC / (dL * kMpc);
+  I.cos_iota = cos(th[7]);
+}
+
+// polarisation basis of O4 (independent of the detector)
+struct Sky {
+  double X[3], Y[3], n[3];
+};
+
+NSS_HD void sky_frame(double gmst, double ra, double dec, double psi, Sky &S)
+{
+  double sg, cg, sd, cd, sp, cp;
+  sincos(gmst - ra, &sg, &cg);
+  sincos(dec, &sd, &cd);
+  sincos(psi, &sp, &cp);
+  S.X[0] = -cp * sg - sp * cg * sd;
+  S.X[1] = -cp * cg + sp * sg * sd;
+  S.X[2] = sp * cd;
+  S.Y[0] = sp * sg - cp * cg * sd;
+  S.Y[1] = sp * cg + cp * sg * sd;
+  S.Y[2] = cp * cd;
+  S.n[0] = cd * cg;          // cos(ra - gmst) = cos g
+  S.n[1] = -cd * sg;         // sin(ra - gmst) = -sin g
+  S.n[2] = sd;
+}
+
+// D6 = symmetric detector tensor (xx, xy, xz, yy, yz, zz) of D = (x x^T - y y^T)/2; rc = vertex / c
+NSS_HD void antenna(const Sky &S, const double *D6, const double *rc, double &fp, double &fc, double &tau)
+{
+  const double DX0 = D6[0] * S.X[0] + D6[1] * S.X[1] + D6[2] * S.X[2];
+  const double DX1 = D6[1] * S.X[0] + D6[3] * S.X[1] + D6[4] * S.X[2];
+  const double DX2 = D6[2] * S.X[0] + D6[4] * S.X[1] + D6[5] * S.X[2];
+  const double DY0 = D6[0] * S.Y[0] + D6[1] * S.Y[1] + D6[2] * S.Y[2];
+  const double DY1 = D6[1] * S.Y[0] + D6[3] * S.Y[1] + D6[4] * S.Y[2];
+  const double DY2 = D6[2] * S.Y[0] + D6[4] * S.Y[1] + D6[5] * S.Y[2];
+  fp = (S.X[0] * DX0 + S.X[1] * DX1 + S.X[2] * DX2) - (S.Y[0] * DY0 + S.Y[1] * DY1 + S.Y[2] * DY2);
+  fc = 2.0 * (S.X[0] * DY0 + S.X[1] * DY1 + S.X[2] * DY2);
+  tau = -(rc[0] * S.n[0] + rc[1] * S.n[1] + rc[2] * S.n[2]);
+}
+
+// basis values at one frequency
+NSS_HD void basis(double f, double *g)
+{
+  const double x = cbrt(f), lf = log(f);
+  const double ix = 1.0 / x, ix2 = ix * ix;
+  g[0] = ix2 * ix2 * ix;
+  g[1] = 1.0 / f;
+  g[2] = ix2;
+  g[3] = ix;
+  g[4] = lf;
+  g[5] = x;
+  g[6] = x * lf;
+  g[7] = x * x;
+}
+
+// sin / cos of an angle given in turns
+NSS_HD void sincos_turns(double t, double *s, double *c)
+{
+  const double fr = t - rint(t);
+#if defined(__CUDA_ARCH__)
+  sincospi(2.0 * fr, s, c);
+#else
+  sincos(2.0 * kPi * fr, s, c);
+#endif
+}
+
+}  // namespace nssp

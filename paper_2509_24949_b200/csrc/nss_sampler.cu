@@ -1,0 +1,774 @@
+// nss_sampler.cu — K3 persistent slice-sampling chains, K4 on-device NS bookkeeping, and the host
+// driver behind nss_replace_step / nss_run (O11-O15).
+#include <math.h>
+#include <string.h>
+
+#include <algorithm>
+#include <vector>
+
+#include "nss_loglike_dev.cuh"
+
+namespace {
+
+constexpr double kSliceW = 2.0;       // A14
+constexpr int kMaxExpand = 32;        // A15
+constexpr int kMaxShrink = 64;        // A15
+constexpr uint32_t kIterInit = 0xFFFFFFFFu, kIterErr = 0xFFFFFFFEu, kStepStart = 0xFFFFFFFFu;
+constexpr double kTwoM53 = 1.0 / 9007199254740992.0;
+
+// ---- O11: Philox4x32-10, counter = (block, step, chain, iteration), key = seed ------------------------
+__host__ __device__ __forceinline__ void philox_round(uint32_t &c0, uint32_t &c1, uint32_t &c2, uint32_t &c3, uint32_t k0,
+                                                      uint32_t k1)
+{
+#if defined(__CUDA_ARCH__)
+  const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+  const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+#else
+  const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+  const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0, hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+#endif
+  const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+  c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+}
+
+__host__ __device__ __forceinline__ void philox4x32_10(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                       uint32_t *w)
+{
+  uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    philox_round(c0, c1, c2, c3, k0, k1);
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  w[0] = c0; w[1] = c1; w[2] = c2; w[3] = c3;
+}
+
+__host__ __device__ __forceinline__ void draw53(uint64_t seed, uint32_t block, uint32_t step, uint32_t chain, uint32_t it,
+                                                uint64_t &ka, uint64_t &kb)
+{
+  uint32_t w[4];
+  philox4x32_10(seed, block, step, chain, it, w);
+  ka = ((uint64_t)(w[0] >> 5) << 26) + (uint64_t)(w[1] >> 6);
+  kb = ((uint64_t)(w[2] >> 5) << 26) + (uint64_t)(w[3] >> 6);
+}
+
+__device__ __forceinline__ double uniform_a(uint64_t seed, uint32_t block, uint32_t step, uint32_t chain, uint32_t it)
+{
+  uint64_t ka, kb;
+  draw53(seed, block, step, chain, it, ka, kb);
+  return (double)ka * kTwoM53;
+}
+
+__global__ void k_philox(uint64_t seed, const uint32_t *__restrict__ ctr, int64_t n, uint32_t *__restrict__ out)
+{
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  uint32_t w[4];
+  philox4x32_10(seed, ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], w);
+  out[4 * i] = w[0]; out[4 * i + 1] = w[1]; out[4 * i + 2] = w[2]; out[4 * i + 3] = w[3];
+}
+
+// ---- O13: initial live points ---------------------------------------------------------------------------
+__global__ void k_init_live(const __grid_constant__ NssDev P, int n, uint64_t seed, double *__restrict__ live)
+{
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int d = P.d;
+  if (idx >= n * d) return;
+  const int i = idx / d, j = idx - i * d;
+  uint64_t ka, kb;
+  draw53(seed, (uint32_t)(j >> 1), 0u, (uint32_t)i, kIterInit, ka, kb);
+  const double u = (double)((j & 1) ? kb : ka) * kTwoM53;
+  live[idx] = P.lo[j] + (P.hi[j] - P.lo[j]) * u;
+}
+
+// ---- K4.1 (O12.1): rank of every live point in (logL, slot) order, by counting ------------------------------
+// rank_i = #{ j : logL_j < logL_i  or (logL_j == logL_i and j < i) }.  dead_idx[rank] = i for rank < k.
+constexpr int kRankThreads = 256;
+__global__ void __launch_bounds__(kRankThreads) k4_rank(const double *__restrict__ logL, int n, int k, int32_t *__restrict__ rank,
+                                                        int32_t *__restrict__ dead_idx)
+{
+  __shared__ double tile[1024];
+  const int i = blockIdx.x * kRankThreads + threadIdx.x;
+  const double Li = i < n ? logL[i] : INFINITY;
+  int cnt = 0;
+  for (int base = 0; base < n; base += 1024) {
+    const int len = min(1024, n - base);
+    __syncthreads();
+    for (int t = threadIdx.x; t < len; t += kRankThreads) tile[t] = logL[base + t];
+    __syncthreads();
+    // j < i part of the tile uses <=, the rest uses <
+    const int split = max(0, min(len, i - base));
+    for (int t = 0; t < split; ++t) cnt += tile[t] <= Li;
+    for (int t = split; t < len; ++t) cnt += tile[t] < Li;
+  }
+  if (i < n) {
+    rank[i] = cnt;
+    if (cnt < k) dead_idx[cnt] = i;
+  }
+}
+
+// ---- K4.2: survivor compaction (ascending slot), gather of the dead rows, threshold -----------------------
+constexpr int kOneCta = 1024;
+__global__ void __launch_bounds__(kOneCta) k4_finish_select(const double *__restrict__ live, const double *__restrict__ logL,
+                                                            const double *__restrict__ birth, int n, int k, int d,
+                                                            double Lstar_in, const int32_t *__restrict__ rank,
+                                                            const int32_t *__restrict__ dead_idx, int32_t *__restrict__ surv_idx,
+                                                            double *__restrict__ dead_theta, double *__restrict__ dead_logL,
+                                                            double *__restrict__ dead_birth, double *__restrict__ state,
+                                                            int32_t *__restrict__ flags)
+{
+  __shared__ int warp_tot[32];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const double Lstar = isnan(Lstar_in) ? logL[dead_idx[k - 1]] : Lstar_in;
+  const int chunk = (n + kOneCta - 1) / kOneCta;
+  const int i0 = min(n, tid * chunk), i1 = min(n, i0 + chunk);
+  int cnt = 0;
+  bool bad = false;
+  for (int i = i0; i < i1; ++i)
+    if (rank[i] >= k) { ++cnt; bad = bad || (logL[i] < Lstar); }
+  int incl = cnt;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int v = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += v;
+  }
+  if (lane == 31) warp_tot[wid] = incl;
+  __syncthreads();
+  if (wid == 0) {
+    int v = warp_tot[lane], s = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int u = __shfl_up_sync(0xffffffffu, s, o);
+      if (lane >= o) s += u;
+    }
+    warp_tot[lane] = s - v;
+  }
+  __syncthreads();
+  int pos = warp_tot[wid] + incl - cnt;
+  if (surv_idx)
+    for (int i = i0; i < i1; ++i)
+      if (rank[i] >= k) surv_idx[pos++] = i;
+  if (bad) flags[1] = 1;
+  for (int j = tid; j < k; j += kOneCta) {
+    const int slot = dead_idx[j];
+    if (dead_logL) dead_logL[j] = logL[slot];
+    if (dead_birth) dead_birth[j] = birth ? birth[slot] : -INFINITY;
+    if (dead_theta)
+      for (int a = 0; a < d; ++a) dead_theta[(size_t)j * d + a] = live[(size_t)slot * d + a];
+  }
+  if (tid == 0 && state) state[3] = Lstar;
+}
+
+// ---- K4.3 (O12.3): mean, covariance (two-pass, 1/(n-1)), lower Cholesky -------------------------------------
+__device__ __forceinline__ double block_sum(double v, double *red)
+{
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  v = nssk::warp_sum(v);
+  __syncthreads();
+  if (lane == 0) red[wid] = v;
+  __syncthreads();
+  double s = 0.0;
+  const int nw = blockDim.x >> 5;
+  for (int w = 0; w < nw; ++w) s += red[w];     // fixed order: deterministic
+  return s;
+}
+
+__global__ void __launch_bounds__(kOneCta) k4_tune(const double *__restrict__ live, int n, int d, double *__restrict__ mean_out,
+                                                   double *__restrict__ chol_out, int32_t *__restrict__ flags)
+{
+  __shared__ double red[32];
+  __shared__ double mean[NSS_NSLOT];
+  __shared__ double cov[NSS_NSLOT * NSS_NSLOT];
+  const int tid = threadIdx.x;
+  for (int j = 0; j < d; ++j) {
+    double s = 0.0;
+    for (int i = tid; i < n; i += kOneCta) s += live[(size_t)i * d + j];
+    s = block_sum(s, red);
+    if (tid == 0) mean[j] = s / n;
+  }
+  __syncthreads();
+  for (int a = 0; a < d; ++a)
+    for (int b = 0; b <= a; ++b) {
+      double s = 0.0;
+      const double ma = mean[a], mb = mean[b];
+      for (int i = tid; i < n; i += kOneCta) s = fma(live[(size_t)i * d + a] - ma, live[(size_t)i * d + b] - mb, s);
+      s = block_sum(s, red);
+      if (tid == 0) { cov[a * d + b] = s / (n - 1); cov[b * d + a] = s / (n - 1); }
+    }
+  __syncthreads();
+  if (tid == 0) {
+    double L[NSS_NSLOT * NSS_NSLOT];
+    for (int a = 0; a < d * d; ++a) L[a] = 0.0;
+    bool ok = true;
+    for (int i = 0; i < d && ok; ++i)
+      for (int j = 0; j <= i; ++j) {
+        double s = cov[i * d + j];
+        for (int m = 0; m < j; ++m) s -= L[i * d + m] * L[j * d + m];
+        if (i == j) {
+          if (!(s > 0.0)) { ok = false; break; }
+          L[i * d + i] = sqrt(s);
+        } else
+          L[i * d + j] = s / L[j * d + j];
+      }
+    if (!ok) flags[0] = 1;
+    for (int a = 0; a < d * d; ++a) chol_out[a] = L[a];
+    if (mean_out)
+      for (int a = 0; a < d; ++a) mean_out[a] = mean[a];
+  }
+}
+
+// ---- K4.4 (O12.2): log-weights of the dead points, logX shrinkage, logZ accumulation -------------------------
+__device__ __forceinline__ double block_max(double v, double *red)
+{
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  __syncthreads();
+  if (lane == 0) red[wid] = v;
+  __syncthreads();
+  double m = -INFINITY;
+  const int nw = blockDim.x >> 5;
+  for (int w = 0; w < nw; ++w) m = fmax(m, red[w]);
+  return m;
+}
+
+__device__ __forceinline__ double logaddexp_d(double a, double b)
+{
+  if (a == -INFINITY) return b;
+  if (b == -INFINITY) return a;
+  const double m = fmax(a, b);
+  return m + log(exp(a - m) + exp(b - m));
+}
+
+__global__ void __launch_bounds__(kOneCta) k4_evidence(const double *__restrict__ dead_logL, int n, int k, double *__restrict__ logw,
+                                                       double *__restrict__ state)
+{
+  __shared__ double red[32];
+  __shared__ double warp_tot[32];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const double logX0 = state[0], logZ0 = state[1];
+  const int chunk = (k + kOneCta - 1) / kOneCta;
+  const int j0 = min(k, tid * chunk), j1 = min(k, j0 + chunk);
+  double part = 0.0;
+  for (int j = j0; j < j1; ++j) part += 1.0 / (double)(n - j);
+  double incl = part;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const double v = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += v;
+  }
+  if (lane == 31) warp_tot[wid] = incl;
+  __syncthreads();
+  if (wid == 0) {
+    double v = warp_tot[lane], s = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const double u = __shfl_up_sync(0xffffffffu, s, o);
+      if (lane >= o) s += u;
+    }
+    warp_tot[lane] = s - v;
+  }
+  __syncthreads();
+  double S = warp_tot[wid] + incl - part;       // sum_{i<j0} 1/m_i
+  double mx = -INFINITY;
+  for (int j = j0; j < j1; ++j) {
+    const double im = 1.0 / (double)(n - j);
+    const double lw = (logX0 - S) + log(-expm1(-im));
+    logw[j] = lw;
+    mx = fmax(mx, dead_logL[j] + lw);
+    S += im;
+  }
+  const double total = block_sum(part, red);
+  mx = block_max(mx, red);
+  double se = 0.0;
+  if (mx > -INFINITY)
+    for (int j = j0; j < j1; ++j) se += exp(dead_logL[j] + logw[j] - mx);
+  se = block_sum(se, red);
+  if (tid == 0) {
+    state[0] = logX0 - total;
+    state[1] = mx > -INFINITY ? logaddexp_d(logZ0, mx + log(se)) : logZ0;
+  }
+}
+
+// ---- K4.5 (O14): live evidence and stop test ------------------------------------------------------------------
+__global__ void __launch_bounds__(kOneCta) k4_live_evidence(const double *__restrict__ logL, int n, double stop_dlogz, int check,
+                                                            double *__restrict__ state, int32_t *__restrict__ flags)
+{
+  __shared__ double red[32];
+  double mx = -INFINITY;
+  for (int i = threadIdx.x; i < n; i += kOneCta) mx = fmax(mx, logL[i]);
+  mx = block_max(mx, red);
+  double se = 0.0;
+  if (mx > -INFINITY)
+    for (int i = threadIdx.x; i < n; i += kOneCta) se += exp(logL[i] - mx);
+  se = block_sum(se, red);
+  if (threadIdx.x == 0) {
+    const double lzl = mx > -INFINITY ? state[0] + mx + log(se) - log((double)n) : -INFINITY;
+    state[2] = lzl;
+    if (check && (lzl - state[1] < stop_dlogz)) flags[2] = 1;
+  }
+}
+
+__global__ void k_gather_rows(const double *__restrict__ live, const double *__restrict__ logL, const double *__restrict__ birth,
+                              const int32_t *__restrict__ order, int n, int d, double *__restrict__ out_theta,
+                              double *__restrict__ out_logL, double *__restrict__ out_birth)
+{
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n) return;
+  const int slot = order[j];
+  out_logL[j] = logL[slot];
+  out_birth[j] = birth[slot];
+  for (int a = 0; a < d; ++a) out_theta[(size_t)j * d + a] = live[(size_t)slot * d + a];
+}
+
+// ---- K3: slice-sampling chains, one warp per chain (O12.4, O12.5) ------------------------------------------------
+struct ChainArgs {
+  double *live;                 // [n][d] in/out
+  double *logL;                 // [n]    in/out
+  double *birth;                // [n]    in/out, may be NULL
+  int32_t n, k, n_repeats;
+  uint64_t seed;
+  uint32_t iteration;
+  const int32_t *surv_idx, *dead_idx;
+  const double *chol;           // [d][d]
+  const double *state;          // state[3] = L*
+  const int32_t *flags;         // flags[0] != 0 (Cholesky failure) or flags[1] != 0 -> do nothing
+  unsigned long long *n_evals;
+  int32_t *trace;               // optional [k][n_repeats][3]
+  double *margin;               // optional [k]
+};
+
+constexpr int kChainThreads = 128;      // 4 chains per CTA
+
+template <int NDET, bool RESIDENT>
+__global__ void __launch_bounds__(kChainThreads) k3_slice(const __grid_constant__ NssDev P, const ChainArgs A)
+{
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  __shared__ __align__(8) uint64_t bar;
+  __shared__ double sL[NSS_NSLOT * NSS_NSLOT];
+  if (A.flags[0] | A.flags[1]) return;
+  const double *tab = P.rb_soa;
+  if (RESIDENT) {
+    if (threadIdx.x == 0) {
+      nssk::mbar_init(&bar, 1);
+      const size_t bytes = (size_t)(9 * (P.rb_m + 1) + 6 * NDET * P.rb_m) * 32 * sizeof(double);
+      nssk::stage_table(smem_raw, P.rb_soa, (uint32_t)bytes, &bar);
+    }
+  }
+  const int d = P.d;
+  for (int t = threadIdx.x; t < d * d; t += blockDim.x) sL[t] = A.chol[t];
+  __syncthreads();
+  if (RESIDENT) {
+    nssk::mbar_wait(&bar, 0);
+    tab = reinterpret_cast<const double *>(smem_raw);
+  }
+  const int lane = threadIdx.x & 31;
+  const int c = blockIdx.x * (kChainThreads / 32) + (threadIdx.x >> 5);
+  if (c >= A.k) return;
+  const double Lstar = A.state[3];
+  const uint32_t chain = (uint32_t)c, it = A.iteration;
+  const int ns = A.n - A.k;
+
+  // a4: start from a uniformly chosen survivor
+  int si = (int)floor(uniform_a(A.seed, 0u, kStepStart, chain, it) * (double)ns);
+  si = si > ns - 1 ? ns - 1 : si;
+  const int slot = A.surv_idx[si];
+  double x[NSS_NSLOT], v[NSS_NSLOT], y[NSS_NSLOT];
+#pragma unroll
+  for (int j = 0; j < NSS_NSLOT; ++j) x[j] = j < d ? A.live[(size_t)slot * d + j] : 0.0;
+  double lx = A.logL[slot];
+  long long evals = 0;
+  double margin = INFINITY;
+
+  // inside(t): box test (inclusive) first, then logL(x + t v) > L*
+  auto inside = [&](double t, double &ly) -> bool {
+    bool in = true;
+#pragma unroll
+    for (int j = 0; j < NSS_NSLOT; ++j)
+      if (j < d) {
+        y[j] = x[j] + t * v[j];
+        in = in && (y[j] >= P.lo[j]) && (y[j] <= P.hi[j]);
+      }
+    if (!in) return false;
+    ly = nssk::loglike_warp<NDET>(P, tab, y);
+    ++evals;
+    margin = fmin(margin, fabs(ly - Lstar));
+    return ly > Lstar;
+  };
+
+  for (int s = 0; s < A.n_repeats; ++s) {
+    // a5: direction n = z/|z|, v = w L n
+    double z[NSS_NSLOT + 1];
+    double nz = 0.0;
+#pragma unroll
+    for (int b = 0; b < (NSS_NSLOT + 1) / 2; ++b)
+      if (2 * b < d) {
+        uint64_t ka, kb;
+        draw53(A.seed, (uint32_t)(1 + b), (uint32_t)s, chain, it, ka, kb);
+        const double r = sqrt(-2.0 * log((double)(ka + 1) * kTwoM53));
+        double sn, cs;
+        sincospi(2.0 * ((double)kb * kTwoM53), &sn, &cs);
+        z[2 * b] = r * cs;
+        z[2 * b + 1] = r * sn;
+      }
+#pragma unroll
+    for (int j = 0; j < NSS_NSLOT; ++j)
+      if (j < d) nz += z[j] * z[j];
+    nz = sqrt(nz);
+#pragma unroll
+    for (int i = 0; i < NSS_NSLOT; ++i)
+      if (i < d) {
+        double a = 0.0;
+#pragma unroll
+        for (int j = 0; j < NSS_NSLOT; ++j)
+          if (j <= i) a += sL[i * d + j] * (z[j] / nz);
+        v[i] = kSliceW * a;
+      }
+    // a6: stepping out
+    const double u0 = uniform_a(A.seed, 0u, (uint32_t)s, chain, it);
+    double l = -u0, r = 1.0 - u0, ly = 0.0;
+    int nl = 0, nr = 0;
+    while (nl < kMaxExpand && inside(l, ly)) { l -= 1.0; ++nl; }
+    while (nr < kMaxExpand && inside(r, ly)) { r += 1.0; ++nr; }
+    // a7: shrinkage
+    int acc = -1;
+    for (int kk = 0; kk < kMaxShrink; ++kk) {
+      const double uk = uniform_a(A.seed, (uint32_t)(64 + kk), (uint32_t)s, chain, it);
+      const double t = l + (r - l) * uk;
+      if (inside(t, ly)) {
+#pragma unroll
+        for (int j = 0; j < NSS_NSLOT; ++j) x[j] = y[j];
+        lx = ly; acc = kk;
+        break;
+      }
+      if (t < 0.0) l = t; else r = t;
+    }
+    if (A.trace && lane == 0) {
+      int32_t *tr = A.trace + ((size_t)c * A.n_repeats + s) * 3;
+      tr[0] = nl; tr[1] = nr; tr[2] = acc;
+    }
+  }
+  // a10: replace the deleted slot in place
+  if (lane == 0) {
+    const int dst = A.dead_idx[c];
+    for (int j = 0; j < d; ++j) A.live[(size_t)dst * d + j] = x[j];
+    A.logL[dst] = lx;
+    if (A.birth) A.birth[dst] = Lstar;
+    if (A.margin) A.margin[c] = margin;
+    atomicAdd(A.n_evals, (unsigned long long)evals);
+  }
+}
+
+template <int NDET>
+int launch_chains(nss_handle *h, const ChainArgs &A, cudaStream_t st)
+{
+  const NssDev &P = h->dev;
+  const int grid = (A.k + kChainThreads / 32 - 1) / (kChainThreads / 32);
+  size_t bytes = 0;
+  if (P.kind == NSS_KIND_RB) bytes = (size_t)(9 * (P.rb_m + 1) + 6 * NDET * P.rb_m) * 32 * sizeof(double);
+  const bool resident = P.kind == NSS_KIND_RB && bytes + 2048 <= 200 * 1024;
+  if (resident) {
+    if (bytes > 48 * 1024)
+      NSS_CUDA(cudaFuncSetAttribute(k3_slice<NDET, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    k3_slice<NDET, true><<<grid, kChainThreads, bytes, st>>>(P, A);
+  } else {
+    k3_slice<NDET, false><<<grid, kChainThreads, 0, st>>>(P, A);
+  }
+  h->launches += 1;
+  NSS_CUDA(cudaGetLastError());
+  return NSS_OK;
+}
+
+int ensure_scratch(nss_handle *h, int n)
+{
+  if (h->scratch_n >= n && h->d_flags) return NSS_OK;
+  cudaFree(h->d_surv_idx); cudaFree(h->d_dead_idx); cudaFree(h->d_rank); cudaFree(h->d_birth);
+  h->d_surv_idx = h->d_dead_idx = h->d_rank = nullptr; h->d_birth = nullptr;
+  NSS_CUDA(cudaMalloc(&h->d_surv_idx, sizeof(int32_t) * n));
+  NSS_CUDA(cudaMalloc(&h->d_dead_idx, sizeof(int32_t) * n));
+  NSS_CUDA(cudaMalloc(&h->d_rank, sizeof(int32_t) * n));
+  NSS_CUDA(cudaMalloc(&h->d_birth, sizeof(double) * n));
+  if (!h->d_flags) {
+    NSS_CUDA(cudaMalloc(&h->d_flags, sizeof(int32_t) * 4));
+    NSS_CUDA(cudaMalloc(&h->d_mean, sizeof(double) * NSS_NSLOT));
+    NSS_CUDA(cudaMalloc(&h->d_chol, sizeof(double) * NSS_NSLOT * NSS_NSLOT));
+    NSS_CUDA(cudaMalloc(&h->d_state, sizeof(double) * 4));
+    NSS_CUDA(cudaMalloc(&h->d_nevals, sizeof(unsigned long long)));
+  }
+  h->scratch_n = n;
+  return NSS_OK;
+}
+
+// the device part of one NS iteration (no host synchronisation): K4.1, K4.2, K4.3, K3
+int enqueue_iteration(nss_handle *h, double *live, double *logL, double *birth, int n, int k, double Lstar_in, int n_repeats,
+                      uint64_t seed, uint32_t iteration, double *dead_theta, double *dead_logL, double *dead_birth,
+                      int32_t *dead_idx, cudaStream_t st)
+{
+  const int d = h->dev.d;
+  k4_rank<<<(n + kRankThreads - 1) / kRankThreads, kRankThreads, 0, st>>>(logL, n, k, h->d_rank, dead_idx);
+  k4_finish_select<<<1, kOneCta, 0, st>>>(live, logL, birth, n, k, d, Lstar_in, h->d_rank, dead_idx, h->d_surv_idx, dead_theta,
+                                          dead_logL, dead_birth, h->d_state, h->d_flags);
+  k4_tune<<<1, kOneCta, 0, st>>>(live, n, d, h->d_mean, h->d_chol, h->d_flags);
+  h->launches += 3;
+  NSS_CUDA(cudaGetLastError());
+  ChainArgs A;
+  A.live = live; A.logL = logL; A.birth = birth; A.n = n; A.k = k; A.n_repeats = n_repeats; A.seed = seed;
+  A.iteration = iteration; A.surv_idx = h->d_surv_idx; A.dead_idx = dead_idx; A.chol = h->d_chol; A.state = h->d_state;
+  A.flags = h->d_flags; A.n_evals = h->d_nevals; A.trace = h->trace_dev; A.margin = h->margin_dev;
+  switch (h->dev.n_det) {
+    case 0: case 1: return launch_chains<1>(h, A, st);
+    case 2: return launch_chains<2>(h, A, st);
+    case 3: return launch_chains<3>(h, A, st);
+    default: return launch_chains<4>(h, A, st);
+  }
+}
+
+}  // namespace
+
+extern "C" int nss_set_trace(nss_handle *h, int32_t *trace_dev, double *margin_dev)
+{
+  if (!h) return NSS_EINVAL;
+  h->trace_dev = trace_dev;
+  h->margin_dev = margin_dev;
+  return NSS_OK;
+}
+
+extern "C" int nss_philox(nss_handle *h, uint64_t seed, const uint32_t *ctr_dev, int64_t n, uint32_t *out_dev, void *cuda_stream)
+{
+  if (!h || n < 0 || (n > 0 && (!ctr_dev || !out_dev))) return NSS_EINVAL;
+  if (n == 0) return NSS_OK;
+  NSS_CUDA(cudaSetDevice(h->device));
+  k_philox<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(seed, ctr_dev, n, out_dev);
+  h->launches += 1;
+  NSS_CUDA(cudaGetLastError());
+  return NSS_OK;
+}
+
+extern "C" int nss_init_live(nss_handle *h, int32_t n_live, uint64_t seed, double *live_dev, double *logL_dev, void *cuda_stream)
+{
+  if (!h || n_live < 1 || !live_dev || !logL_dev) return NSS_EINVAL;
+  NSS_CUDA(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int tot = n_live * h->dev.d;
+  k_init_live<<<(tot + 255) / 256, 256, 0, st>>>(h->dev, n_live, seed, live_dev);
+  h->launches += 1;
+  NSS_CUDA(cudaGetLastError());
+  return nss_launch_loglike(h, live_dev, n_live, logL_dev, st);
+}
+
+extern "C" int nss_select_lowest(nss_handle *h, const double *logL_dev, int32_t n_live, int32_t n_delete, int32_t *dead_idx_dev,
+                                 int32_t *surv_idx_dev, double *logLstar_host, void *cuda_stream)
+{
+  if (!h || !logL_dev || !dead_idx_dev || n_live < 2 || n_delete < 1 || n_delete >= n_live) return NSS_EINVAL;
+  NSS_CUDA(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = ensure_scratch(h, n_live);
+  if (rc) return rc;
+  NSS_CUDA(cudaMemsetAsync(h->d_flags, 0, sizeof(int32_t) * 4, st));
+  k4_rank<<<(n_live + kRankThreads - 1) / kRankThreads, kRankThreads, 0, st>>>(logL_dev, n_live, n_delete, h->d_rank, dead_idx_dev);
+  k4_finish_select<<<1, kOneCta, 0, st>>>(nullptr, logL_dev, nullptr, n_live, n_delete, h->dev.d, NAN, h->d_rank, dead_idx_dev,
+                                          surv_idx_dev, nullptr, nullptr, nullptr, h->d_state, h->d_flags);
+  h->launches += 2;
+  NSS_CUDA(cudaGetLastError());
+  double state[4];
+  NSS_CUDA(cudaMemcpyAsync(state, h->d_state, sizeof(state), cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaStreamSynchronize(st));
+  if (logLstar_host) *logLstar_host = state[3];
+  return NSS_OK;
+}
+
+extern "C" int nss_tune(nss_handle *h, const double *live_dev, int32_t n_live, double *mean_dev, double *chol_dev, void *cuda_stream)
+{
+  if (!h || !live_dev || !chol_dev || n_live < 2) return NSS_EINVAL;
+  NSS_CUDA(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = ensure_scratch(h, n_live);
+  if (rc) return rc;
+  NSS_CUDA(cudaMemsetAsync(h->d_flags, 0, sizeof(int32_t) * 4, st));
+  k4_tune<<<1, kOneCta, 0, st>>>(live_dev, n_live, h->dev.d, mean_dev, chol_dev, h->d_flags);
+  h->launches += 1;
+  NSS_CUDA(cudaGetLastError());
+  int32_t flags[4];
+  NSS_CUDA(cudaMemcpyAsync(flags, h->d_flags, sizeof(flags), cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaStreamSynchronize(st));
+  return flags[0] ? NSS_ECHOL : NSS_OK;
+}
+
+extern "C" int nss_evidence_update(nss_handle *h, const double *dead_logL_dev, int32_t n_live, int32_t n_delete, double *logw_dev,
+                                   double *state_host, void *cuda_stream)
+{
+  if (!h || !dead_logL_dev || !logw_dev || !state_host || n_delete < 1 || n_delete >= n_live) return NSS_EINVAL;
+  NSS_CUDA(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = ensure_scratch(h, n_live);
+  if (rc) return rc;
+  double state[4] = {state_host[0], state_host[1], 0.0, 0.0};
+  NSS_CUDA(cudaMemcpyAsync(h->d_state, state, sizeof(state), cudaMemcpyHostToDevice, st));
+  k4_evidence<<<1, kOneCta, 0, st>>>(dead_logL_dev, n_live, n_delete, logw_dev, h->d_state);
+  h->launches += 1;
+  NSS_CUDA(cudaGetLastError());
+  NSS_CUDA(cudaMemcpyAsync(state, h->d_state, sizeof(state), cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaStreamSynchronize(st));
+  state_host[0] = state[0];
+  state_host[1] = state[1];
+  return NSS_OK;
+}
+
+extern "C" int nss_replace_step(nss_handle *h, double *live_dev, double *logL_dev, int32_t n_live, int32_t n_delete, double logLstar,
+                                int32_t n_repeats, uint64_t seed, uint32_t iteration, double *dead_theta_dev, double *dead_logL_dev,
+                                int32_t *dead_idx_dev, double *logLstar_host, int64_t *n_evals_host, void *cuda_stream)
+{
+  if (!h || !live_dev || !logL_dev || !dead_theta_dev || !dead_logL_dev || !dead_idx_dev) return NSS_EINVAL;
+  if (n_live < 2 || n_delete < 1 || n_delete >= n_live || n_repeats < 0) return NSS_EINVAL;
+  NSS_CUDA(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = ensure_scratch(h, n_live);
+  if (rc) return rc;
+  NSS_CUDA(cudaMemsetAsync(h->d_flags, 0, sizeof(int32_t) * 4, st));
+  NSS_CUDA(cudaMemsetAsync(h->d_nevals, 0, sizeof(unsigned long long), st));
+  rc = enqueue_iteration(h, live_dev, logL_dev, nullptr, n_live, n_delete, logLstar, n_repeats, seed, iteration, dead_theta_dev,
+                         dead_logL_dev, nullptr, dead_idx_dev, st);
+  if (rc) return rc;
+  int32_t flags[4];
+  double state[4];
+  unsigned long long ne = 0;
+  NSS_CUDA(cudaMemcpyAsync(flags, h->d_flags, sizeof(flags), cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaMemcpyAsync(state, h->d_state, sizeof(state), cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaMemcpyAsync(&ne, h->d_nevals, sizeof(ne), cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaStreamSynchronize(st));
+  if (logLstar_host) *logLstar_host = state[3];
+  if (n_evals_host) *n_evals_host = (int64_t)ne;
+  if (flags[1]) return NSS_EINVAL;
+  if (flags[0]) return NSS_ECHOL;
+  return NSS_OK;
+}
+
+extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t n_repeats, uint64_t seed, double stop_dlogz,
+                       int32_t max_iter, nss_result *out, void *cuda_stream)
+{
+  if (!h || !out || !out->dead_theta || !out->dead_logL || !out->dead_logL_birth || !out->dead_logw) return NSS_EINVAL;
+  if (n_live < 2 || n_delete < 1 || n_delete >= n_live || n_repeats < 0 || max_iter < 0) return NSS_EINVAL;
+  if (out->cap < n_live) return NSS_ECAP;
+  NSS_CUDA(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int n = n_live, k = n_delete, d = h->dev.d;
+  int rc = ensure_scratch(h, n);
+  if (rc) return rc;
+  const int64_t cap = out->cap;
+  double *live = nullptr, *logL = nullptr, *dth = nullptr, *dl = nullptr, *db = nullptr, *dw = nullptr;
+  int32_t *h_flags = nullptr;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  auto cleanup = [&]() {
+    cudaFree(live); cudaFree(logL); cudaFree(dth); cudaFree(dl); cudaFree(db); cudaFree(dw);
+    if (h_flags) cudaFreeHost(h_flags);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+  };
+#define RUN_CUDA(x)                                                           \
+  do {                                                                        \
+    cudaError_t e__ = (x);                                                    \
+    if (e__ != cudaSuccess) { cleanup(); return nss_cuda_fail(e__, #x); }     \
+  } while (0)
+  RUN_CUDA(cudaMalloc(&live, sizeof(double) * (size_t)n * d));
+  RUN_CUDA(cudaMalloc(&logL, sizeof(double) * n));
+  RUN_CUDA(cudaMalloc(&dth, sizeof(double) * (size_t)cap * d));
+  RUN_CUDA(cudaMalloc(&dl, sizeof(double) * cap));
+  RUN_CUDA(cudaMalloc(&db, sizeof(double) * cap));
+  RUN_CUDA(cudaMalloc(&dw, sizeof(double) * cap));
+  RUN_CUDA(cudaMallocHost(&h_flags, sizeof(int32_t) * 4));
+  RUN_CUDA(cudaEventCreate(&e0));
+  RUN_CUDA(cudaEventCreate(&e1));
+
+  RUN_CUDA(cudaEventRecord(e0, st));
+  const double state0[4] = {0.0, -INFINITY, 0.0, 0.0};
+  RUN_CUDA(cudaMemcpyAsync(h->d_state, state0, sizeof(state0), cudaMemcpyHostToDevice, st));
+  RUN_CUDA(cudaMemsetAsync(h->d_flags, 0, sizeof(int32_t) * 4, st));
+  RUN_CUDA(cudaMemsetAsync(h->d_nevals, 0, sizeof(unsigned long long), st));
+  rc = nss_init_live(h, n, seed, live, logL, st);
+  if (rc) { cleanup(); return rc; }
+  {
+    std::vector<double> ninf(n, -INFINITY);
+    RUN_CUDA(cudaMemcpyAsync(h->d_birth, ninf.data(), sizeof(double) * n, cudaMemcpyHostToDevice, st));
+    RUN_CUDA(cudaStreamSynchronize(st));
+  }
+  int t = 0;
+  int64_t n_dead = 0;
+  int result = NSS_OK;
+  for (;;) {
+    k4_live_evidence<<<1, kOneCta, 0, st>>>(logL, n, stop_dlogz, t > 0, h->d_state, h->d_flags);
+    h->launches += 1;
+    RUN_CUDA(cudaMemcpyAsync(h_flags, h->d_flags, sizeof(int32_t) * 4, cudaMemcpyDeviceToHost, st));
+    RUN_CUDA(cudaStreamSynchronize(st));
+    if (h_flags[0]) { result = NSS_ECHOL; break; }
+    if (h_flags[2]) break;
+    if (t >= max_iter) { result = NSS_ENOTCONV; break; }
+    if (n_dead + k + n > cap) { result = NSS_ECAP; break; }
+    rc = enqueue_iteration(h, live, logL, h->d_birth, n, k, NAN, n_repeats, seed, (uint32_t)t, dth + (size_t)n_dead * d, dl + n_dead,
+                           db + n_dead, h->d_dead_idx, st);
+    if (rc) { cleanup(); return rc; }
+    k4_evidence<<<1, kOneCta, 0, st>>>(dl + n_dead, n, k, dw + n_dead, h->d_state);
+    h->launches += 1;
+    n_dead += k;
+    ++t;
+  }
+  if (result == NSS_OK || result == NSS_ENOTCONV) {
+    // O14: append the live points in ascending logL
+    k4_rank<<<(n + kRankThreads - 1) / kRankThreads, kRankThreads, 0, st>>>(logL, n, n, h->d_rank, h->d_dead_idx);
+    k_gather_rows<<<(n + 255) / 256, 256, 0, st>>>(live, logL, h->d_birth, h->d_dead_idx, n, d, dth + (size_t)n_dead * d, dl + n_dead,
+                                                   db + n_dead);
+    h->launches += 2;
+    const int64_t n_it_dead = n_dead;
+    n_dead += n;
+    double state[4];
+    unsigned long long ne = 0;
+    RUN_CUDA(cudaMemcpyAsync(state, h->d_state, sizeof(state), cudaMemcpyDeviceToHost, st));
+    RUN_CUDA(cudaMemcpyAsync(&ne, h->d_nevals, sizeof(ne), cudaMemcpyDeviceToHost, st));
+    RUN_CUDA(cudaMemcpyAsync(out->dead_theta, dth, sizeof(double) * (size_t)n_dead * d, cudaMemcpyDeviceToHost, st));
+    RUN_CUDA(cudaMemcpyAsync(out->dead_logL, dl, sizeof(double) * n_dead, cudaMemcpyDeviceToHost, st));
+    RUN_CUDA(cudaMemcpyAsync(out->dead_logL_birth, db, sizeof(double) * n_dead, cudaMemcpyDeviceToHost, st));
+    RUN_CUDA(cudaMemcpyAsync(out->dead_logw, dw, sizeof(double) * n_it_dead, cudaMemcpyDeviceToHost, st));
+    RUN_CUDA(cudaEventRecord(e1, st));
+    RUN_CUDA(cudaStreamSynchronize(st));
+    float ms = 0.f;
+    RUN_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    out->gpu_ms = ms;
+    const double logX = state[0], logZ = state[1], logZ_live = state[2];
+    for (int j = 0; j < n; ++j) out->dead_logw[n_it_dead + j] = logX - log((double)n);
+    auto lae = [](double a, double b) {
+      if (a == -INFINITY) return b;
+      if (b == -INFINITY) return a;
+      const double m = a > b ? a : b;
+      return m + log(exp(a - m) + exp(b - m));
+    };
+    const double logZf = lae(logZ, logZ_live);
+    // O15: information and replica evidence error (host post-processing)
+    double H = 0.0;
+    for (int64_t i = 0; i < n_dead; ++i)
+      if (out->dead_logL[i] > -INFINITY) H += exp(out->dead_logL[i] + out->dead_logw[i] - logZf) * (out->dead_logL[i] - logZf);
+    const int R = 200;
+    double ls = -INFINITY;
+    for (int j = 0; j < n; ++j) ls = lae(ls, out->dead_logL[n_it_dead + j]);
+    double sum = 0.0, sum2 = 0.0;
+    for (int rpl = 0; rpl < R; ++rpl) {
+      double lX = 0.0, lZ = -INFINITY;
+      for (int64_t j = 0; j < n_it_dead; ++j) {
+        const double m = (double)(n - (int)(j % k));
+        uint64_t ka, kb;
+        draw53(seed, 0u, (uint32_t)j, (uint32_t)rpl, kIterErr, ka, kb);
+        const double lXn = lX + log((double)(ka + 1) * kTwoM53) / m;
+        lZ = lae(lZ, out->dead_logL[j] + lX + log1p(-exp(lXn - lX)));
+        lX = lXn;
+      }
+      lZ = lae(lZ, lX + ls - log((double)n));
+      sum += lZ; sum2 += lZ * lZ;
+    }
+    const double mu = sum / R;
+    double var = sum2 / R - mu * mu;
+    var = var < 0 ? 0 : var;
+    out->logZ = logZf; out->logZ_err = sqrt(var * R / (R - 1)); out->H = H;
+    out->n_iter = t; out->n_dead = n_dead; out->n_evals = (int64_t)ne + n;
+  }
+#undef RUN_CUDA
+  cleanup();
+  return result;
+}

@@ -1,0 +1,348 @@
+// nss_setup.cu — L0 host setup (untimed) and handle lifetime.
+//
+// nss_create: validate -> bin edges (O8) -> fiducial waveform on the full grid (O3, O4) ->
+// summary data A0/A1/B0/B1 per (detector, bin) and <d,d> (O9) -> pack device tables -> upload.
+#include <math.h>
+#include <string.h>
+
+#include <complex>
+#include <new>
+#include <vector>
+
+#include "nss_internal.cuh"
+
+thread_local char g_nss_cuda_err[256] = "";
+
+int nss_cuda_fail(cudaError_t e, const char *where)
+{
+  snprintf(g_nss_cuda_err, sizeof(g_nss_cuda_err), "%s: %s", where, cudaGetErrorString(e));
+  cudaGetLastError();
+  return NSS_ECUDA;
+}
+
+extern "C" const char *nss_last_cuda_error(void) { return g_nss_cuda_err; }
+
+extern "C" const char *nss_strerror(int code)
+{
+  switch (code) {
+    case NSS_OK: return "ok";
+    case NSS_EINVAL: return "invalid argument";
+    case NSS_ENOMEM: return "out of memory";
+    case NSS_ECUDA: return "CUDA error (see nss_last_cuda_error)";
+    case NSS_ECHOL: return "non-positive Cholesky pivot of the live-point covariance";
+    case NSS_ECAP: return "result arrays too small";
+    case NSS_ENOTCONV: return "max_iter reached before the stop rule (results valid)";
+    default: return "unknown error";
+  }
+}
+
+extern "C" int nss_version(void) { return 1; }
+
+using cplx = std::complex<double>;
+
+namespace {
+
+void detector_tensor(const nss_detector &det, double *D6, double *rc)
+{
+  const double *x = det.xarm, *y = det.yarm;
+  D6[0] = 0.5 * (x[0] * x[0] - y[0] * y[0]);
+  D6[1] = 0.5 * (x[0] * x[1] - y[0] * y[1]);
+  D6[2] = 0.5 * (x[0] * x[2] - y[0] * y[2]);
+  D6[3] = 0.5 * (x[1] * x[1] - y[1] * y[1]);
+  D6[4] = 0.5 * (x[1] * x[2] - y[1] * y[2]);
+  D6[5] = 0.5 * (x[2] * x[2] - y[2] * y[2]);
+  for (int c = 0; c < 3; ++c) rc[c] = det.vertex_m[c] / nssp::kC;
+}
+
+// complex amplitude (without f^-7/6) and arrival-time offset of one detector
+void det_amplitude(const nssp::Intrinsic &I, const double *th, double gmst, const double *D6, const double *rc,
+                   cplx &amp, double &tau)
+{
+  nssp::Sky S;
+  nssp::sky_frame(gmst, th[9], th[10], th[8], S);
+  double fp, fc;
+  nssp::antenna(S, D6, rc, fp, fc, tau);
+  const double ci = I.cos_iota;
+  amp = I.amp * cplx(fp * 0.5 * (1.0 + ci * ci), -fc * ci);
+}
+
+void host_waveform(const double *th, const double *D6, const double *rc, double gmst, const double *f, int n,
+                   cplx *out)
+{
+  nssp::Intrinsic I;
+  nssp::intrinsic(th, I);
+  cplx amp;
+  double tau;
+  det_amplitude(I, th, gmst, D6, rc, amp, tau);
+  for (int k = 0; k < n; ++k) {
+    double g[nssp::kNB];
+    nssp::basis(f[k], g);
+    double ph = I.c_const;
+    for (int j = 0; j < nssp::kNB; ++j) ph += I.c[j] * g[j];
+    ph += f[k] * (I.tc + tau);
+    double s, c;
+    nssp::sincos_turns(ph, &s, &c);
+    const double x = cbrt(f[k]);
+    const double f76 = 1.0 / (f[k] * sqrt(x));          // f^-7/6 = 1 / (f * f^(1/6))
+    out[k] = amp * f76 * cplx(c, -s);
+  }
+}
+
+// O8: equal increments of a power-law dephasing measure, snapped to the grid, strictly increasing
+std::vector<int32_t> choose_edges(int n, double f_min, double df, int B)
+{
+  const double f_max = f_min + (n - 1) * df;
+  static const double gam[5] = {-5.0 / 3.0, -2.0 / 3.0, 1.0, 5.0 / 3.0, 7.0 / 3.0};
+  std::vector<double> del(n);
+  for (int k = 0; k < n; ++k) {
+    const double f = f_min + k * df;
+    double s = 0.0;
+    for (double g : gam) s += (g > 0 ? 1.0 : -1.0) * pow(f / (g > 0 ? f_max : f_min), g);
+    del[k] = s;
+  }
+  std::vector<int32_t> ie(B + 1);
+  int cur = 0;                       // del is monotone: a forward scan finds the nearest grid point
+  for (int e = 0; e <= B; ++e) {
+    const double target = del[0] + ((double)e / (double)B) * (del[n - 1] - del[0]);
+    while (cur + 1 < n && fabs(del[cur + 1] - target) < fabs(del[cur] - target)) ++cur;
+    ie[e] = cur;
+  }
+  ie[0] = 0;
+  ie[B] = n - 1;
+  for (int e = 1; e <= B; ++e) ie[e] = ie[e] < ie[e - 1] + 1 ? ie[e - 1] + 1 : ie[e];
+  ie[B] = n - 1;
+  for (int e = B - 1; e >= 0; --e) ie[e] = ie[e] > ie[e + 1] - 1 ? ie[e + 1] - 1 : ie[e];
+  return ie;
+}
+
+template <class T>
+int upload(const std::vector<T> &v, T **dptr, size_t *bytes)
+{
+  *bytes = v.size() * sizeof(T);
+  if (v.empty()) { *dptr = nullptr; return NSS_OK; }
+  cudaError_t e = cudaMalloc((void **)dptr, *bytes);
+  if (e != cudaSuccess) { nss_cuda_fail(e, "cudaMalloc(table)"); return e == cudaErrorMemoryAllocation ? NSS_ENOMEM : NSS_ECUDA; }
+  NSS_CUDA(cudaMemcpy(*dptr, v.data(), *bytes, cudaMemcpyHostToDevice));
+  return NSS_OK;
+}
+
+}  // namespace
+
+extern "C" int nss_waveform(const double *theta_canon, const nss_detector *det, double gmst, const double *freqs,
+                            int32_t n, double *out)
+{
+  if (!theta_canon || !det || !freqs || !out || n < 0) return NSS_EINVAL;
+  if (!nssp::domain_ok(theta_canon)) return NSS_EINVAL;
+  double D6[6], rc[3];
+  detector_tensor(*det, D6, rc);
+  std::vector<cplx> h(n);
+  host_waveform(theta_canon, D6, rc, gmst, freqs, n, h.data());
+  for (int k = 0; k < n; ++k) { out[2 * k] = h[k].real(); out[2 * k + 1] = h[k].imag(); }
+  return NSS_OK;
+}
+
+extern "C" int nss_destroy(nss_handle *h)
+{
+  if (!h) return NSS_OK;
+  cudaSetDevice(h->device);
+  cudaFree(h->d_rb_rec); cudaFree(h->d_rb_soa); cudaFree(h->d_full_rec);
+  cudaFree(h->d_surv_idx); cudaFree(h->d_dead_idx); cudaFree(h->d_rank); cudaFree(h->d_flags);
+  cudaFree(h->d_mean); cudaFree(h->d_chol); cudaFree(h->d_state); cudaFree(h->d_nevals); cudaFree(h->d_birth);
+  delete h;
+  return NSS_OK;
+}
+
+extern "C" int nss_create(const nss_config *cfg, nss_handle **out)
+{
+  if (!cfg || !out) return NSS_EINVAL;
+  *out = nullptr;
+  if (cfg->d < 1 || cfg->d > NSS_NSLOT) return NSS_EINVAL;
+  if (cfg->kind < 0 || cfg->kind > 2) return NSS_EINVAL;
+  for (int j = 0; j < cfg->d; ++j)
+    if (!(cfg->lo[j] < cfg->hi[j]) || !isfinite(cfg->lo[j]) || !isfinite(cfg->hi[j])) return NSS_EINVAL;
+  const int kind = cfg->kind;
+  if (kind == NSS_KIND_GAUSS) {
+    for (int j = 0; j < cfg->d; ++j)
+      if (!(cfg->gauss_sigma[j] > 0.0) || !isfinite(cfg->gauss_mu[j])) return NSS_EINVAL;
+  } else {
+    if (cfg->n_det < 1 || cfg->n_det > NSS_MAXDET || cfg->n_freq < 2 || !cfg->psd || !cfg->data) return NSS_EINVAL;
+    if (!(cfg->df > 0.0) || !(cfg->f_min > 0.0)) return NSS_EINVAL;
+    bool seen[NSS_NSLOT] = {false};
+    for (int j = 0; j < cfg->d; ++j) {
+      const int s = cfg->param_index[j];
+      if (s < 0 || s >= NSS_NSLOT || seen[s]) return NSS_EINVAL;
+      seen[s] = true;
+    }
+    const size_t nn = (size_t)cfg->n_det * cfg->n_freq;
+    for (size_t k = 0; k < nn; ++k)
+      if (!(cfg->psd[k] > 0.0) || !isfinite(cfg->psd[k])) return NSS_EINVAL;
+    if (kind == NSS_KIND_RB) {
+      if (cfg->n_bins < 1 || cfg->n_bins > cfg->n_freq - 1) return NSS_EINVAL;
+      if (!nssp::domain_ok(cfg->theta_fid)) return NSS_EINVAL;
+    }
+  }
+
+  int dev_id = 0;
+  NSS_CUDA(cudaGetDevice(&dev_id));
+  cudaDeviceProp prop;
+  NSS_CUDA(cudaGetDeviceProperties(&prop, dev_id));
+
+  nss_handle *h = new (std::nothrow) nss_handle();
+  if (!h) return NSS_ENOMEM;
+  h->device = dev_id;
+  h->n_sm = prop.multiProcessorCount;
+  NssDev &P = h->dev;
+  memset(&P, 0, sizeof(P));
+  P.d = cfg->d; P.kind = kind; P.n_det = kind == NSS_KIND_GAUSS ? 0 : cfg->n_det;
+  P.n_freq = kind == NSS_KIND_GAUSS ? 0 : cfg->n_freq;
+  P.gmst = cfg->gmst;
+  for (int j = 0; j < NSS_NSLOT; ++j) {
+    P.param_index[j] = j < cfg->d ? (kind == NSS_KIND_GAUSS ? j : cfg->param_index[j]) : 0;
+    P.theta_fixed[j] = cfg->theta_fixed[j];
+    P.lo[j] = j < cfg->d ? cfg->lo[j] : 0.0;
+    P.hi[j] = j < cfg->d ? cfg->hi[j] : 0.0;
+    P.gauss_mu[j] = j < cfg->d ? cfg->gauss_mu[j] : 0.0;
+    P.gauss_isig[j] = (j < cfg->d && kind == NSS_KIND_GAUSS) ? 1.0 / cfg->gauss_sigma[j] : 0.0;
+  }
+  if (kind == NSS_KIND_GAUSS) { *out = h; return NSS_OK; }
+
+  const int n = cfg->n_freq, nd = cfg->n_det;
+  const double df = cfg->df;
+  for (int a = 0; a < nd; ++a) detector_tensor(cfg->det[a], P.D6[a], P.rc[a]);
+  std::vector<double> f(n);
+  for (int k = 0; k < n; ++k) f[k] = cfg->f_min + k * df;
+  const cplx *data = reinterpret_cast<const cplx *>(cfg->data);
+
+  double DD = 0.0;
+  for (int a = 0; a < nd; ++a)
+    for (int k = 0; k < n; ++k) DD += 4.0 * df * std::norm(data[(size_t)a * n + k]) / cfg->psd[(size_t)a * n + k];
+  h->DD = DD;
+  P.half_DD = 0.5 * DD;
+
+  int rc_up = NSS_OK;
+  if (kind == NSS_KIND_FULL) {
+    // full-grid records: g0..g7, f, f^-7/6, then per detector (d_re, d_im, 4 df / S)
+    const int rs = (10 + 3 * nd + 1) & ~1;
+    std::vector<double> rec((size_t)n * rs, 0.0);
+    for (int k = 0; k < n; ++k) {
+      double *r = &rec[(size_t)k * rs];
+      nssp::basis(f[k], r);
+      r[8] = f[k];
+      r[9] = 1.0 / (f[k] * sqrt(cbrt(f[k])));
+      for (int a = 0; a < nd; ++a) {
+        r[10 + 3 * a] = data[(size_t)a * n + k].real();
+        r[11 + 3 * a] = data[(size_t)a * n + k].imag();
+        r[12 + 3 * a] = 4.0 * df / cfg->psd[(size_t)a * n + k];
+      }
+    }
+    P.full_rs = rs;
+    rc_up = upload(rec, &h->d_full_rec, &h->full_rec_bytes);
+    P.full_rec = h->d_full_rec;
+  } else {
+    const int B = cfg->n_bins, E = B + 1;
+    P.n_bins = B; P.n_edges = E;
+    h->edge_idx = choose_edges(n, cfg->f_min, df, B);
+    // fiducial
+    nssp::Intrinsic I0;
+    nssp::intrinsic(cfg->theta_fid, I0);
+    for (int j = 0; j < nssp::kNB; ++j) P.c_fid[j] = I0.c[j];
+    P.c_const_fid = I0.c_const; P.tc_fid = I0.tc;
+    h->summary.assign((size_t)nd * B * 6, 0.0);
+    std::vector<cplx> h0(n);
+    for (int a = 0; a < nd; ++a) {
+      cplx amp0; double tau0;
+      det_amplitude(I0, cfg->theta_fid, cfg->gmst, P.D6[a], P.rc[a], amp0, tau0);
+      if (!(std::abs(amp0) > 0.0)) { nss_destroy(h); return NSS_EINVAL; }   // fiducial invisible in this detector
+      const cplx inv = 1.0 / amp0;
+      P.inv_a0[a][0] = inv.real(); P.inv_a0[a][1] = inv.imag();
+      P.tau_fid[a] = tau0;
+      host_waveform(cfg->theta_fid, P.D6[a], P.rc[a], cfg->gmst, f.data(), n, h0.data());
+      for (int b = 0; b < B; ++b) {
+        const int k0 = h->edge_idx[b];
+        const int k1 = b == B - 1 ? h->edge_idx[B] + 1 : h->edge_idx[b + 1];     // last bin owns its right edge (A8)
+        const double fbar = 0.5 * (f[h->edge_idx[b]] + f[h->edge_idx[b + 1]]);
+        cplx a0 = 0, a1 = 0; double b0 = 0, b1 = 0;
+        for (int k = k0; k < k1; ++k) {
+          const double w = 4.0 * df / cfg->psd[(size_t)a * n + k];
+          const cplx dh = data[(size_t)a * n + k] * std::conj(h0[k]) * w;
+          const double hh = std::norm(h0[k]) * w;
+          a0 += dh; a1 += dh * (f[k] - fbar);
+          b0 += hh; b1 += hh * (f[k] - fbar);
+        }
+        double *s = &h->summary[((size_t)a * B + b) * 6];
+        s[0] = a0.real(); s[1] = a0.imag(); s[2] = a1.real(); s[3] = a1.imag(); s[4] = b0; s[5] = b1;
+      }
+    }
+    // pre-scaled bin terms: with s = r_b + r_{b+1}, t = r_{b+1} - r_b  (r0 = s/2, r1 = t/dF):
+    //   <d,h> - <h,h>/2 = q0 s_re + q1 s_im + q2 t_re + q3 t_im + q4 |s|^2 + q5 Re(s conj t)
+    auto scaled = [&](int a, int b, double *q) {
+      const double *s = &h->summary[((size_t)a * B + b) * 6];
+      const double idF = 1.0 / (f[h->edge_idx[b + 1]] - f[h->edge_idx[b]]);
+      q[0] = 0.5 * s[0]; q[1] = 0.5 * s[1];
+      q[2] = s[2] * idF; q[3] = s[3] * idF;
+      q[4] = -0.125 * s[4];
+      q[5] = -0.5 * s[5] * idF;
+    };
+    // (1) AoS records for the thread-per-point kernel
+    const int rs = 10 + 6 * nd;
+    std::vector<double> rec((size_t)E * rs, 0.0);
+    for (int e = 0; e < E; ++e) {
+      double *r = &rec[(size_t)e * rs];
+      nssp::basis(f[h->edge_idx[e]], r);
+      r[8] = f[h->edge_idx[e]];
+      if (e > 0)
+        for (int a = 0; a < nd; ++a) scaled(a, e - 1, r + 10 + 6 * a);
+    }
+    P.rb_rs = rs;
+    rc_up = upload(rec, &h->d_rb_rec, &h->rb_rec_bytes);
+    P.rb_rec = h->d_rb_rec;
+    // (2) warp layout: lane l owns bins [l*m, l*m+m) and edges [l*m, l*m+m]
+    const int m = (B + 31) / 32;
+    P.rb_m = m;
+    std::vector<double> soa((size_t)(9 * (m + 1) + 6 * nd * m) * 32, 0.0);
+    double *te = soa.data(), *tb = soa.data() + (size_t)9 * (m + 1) * 32;
+    for (int l = 0; l < 32; ++l) {
+      for (int j = 0; j <= m; ++j) {
+        int e = l * m + j;
+        if (e > B) e = B;
+        double g[nssp::kNB];
+        nssp::basis(f[h->edge_idx[e]], g);
+        for (int c = 0; c < 8; ++c) te[((size_t)c * (m + 1) + j) * 32 + l] = g[c];
+        te[((size_t)8 * (m + 1) + j) * 32 + l] = f[h->edge_idx[e]];
+      }
+      for (int j = 0; j < m; ++j) {
+        const int b = l * m + j;
+        if (b >= B) continue;
+        for (int a = 0; a < nd; ++a) {
+          double q[6];
+          scaled(a, b, q);
+          for (int c = 0; c < 6; ++c) tb[((size_t)(a * 6 + c) * m + j) * 32 + l] = q[c];
+        }
+      }
+    }
+    if (rc_up == NSS_OK) rc_up = upload(soa, &h->d_rb_soa, &h->rb_soa_bytes);
+    P.rb_soa = h->d_rb_soa;
+  }
+  if (rc_up != NSS_OK) { nss_destroy(h); return rc_up; }
+  *out = h;
+  return NSS_OK;
+}
+
+extern "C" int nss_get_tables(nss_handle *h, int32_t *edge_idx_host, double *summary_host, double *dd_host)
+{
+  if (!h) return NSS_EINVAL;
+  if (dd_host) *dd_host = h->DD;
+  if (h->dev.kind != NSS_KIND_RB) return (edge_idx_host || summary_host) ? NSS_EINVAL : NSS_OK;
+  if (edge_idx_host) memcpy(edge_idx_host, h->edge_idx.data(), h->edge_idx.size() * sizeof(int32_t));
+  if (summary_host) memcpy(summary_host, h->summary.data(), h->summary.size() * sizeof(double));
+  return NSS_OK;
+}
+
+extern "C" int nss_set_loglike_variant(nss_handle *h, int32_t variant)
+{
+  if (!h || variant < 0 || variant > 2) return NSS_EINVAL;
+  h->loglike_variant = variant;
+  return NSS_OK;
+}
+
+extern "C" int64_t nss_launch_count(const nss_handle *h) { return h ? h->launches : 0; }

@@ -1,0 +1,243 @@
+"""GPU parity: Philox, K4 bookkeeping kernels, K3 slice-sampling chains and nss_run vs the oracle."""
+import math
+
+import numpy as np
+import pytest
+import scipy.stats
+
+from paper_2509_24949_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def nssmod():
+    from paper_2509_24949_b200 import build, nss
+    build.build()
+    return nss
+
+
+@pytest.fixture(scope="module")
+def ggauss(nssmod):
+    return nssmod.Nss(inputs.gaussian_workload(4, sigma=0.05))
+
+
+def test_philox_bit_exact(ggauss, oracle):
+    rng = np.random.default_rng(0)
+    n = 100000
+    ctr = rng.integers(0, 2 ** 32, size=(n, 4), dtype=np.uint64).astype(np.uint32)
+    ctr[0] = 0
+    ctr[1] = 0xFFFFFFFF
+    seed = (0xDEADBEEF << 32) | 0x12345678
+    got = ggauss.nss_philox(seed, ctr)
+    for i in list(range(64)) + list(rng.integers(0, n, 400)):
+        assert tuple(int(x) for x in got[i]) == oracle.philox((seed & 0xFFFFFFFF, seed >> 32), [int(c) for c in ctr[i]])
+    # all rows distinct (bijection)
+    assert len({tuple(r) for r in got[:20000].tolist()}) == 20000
+
+
+@pytest.mark.parametrize("n,k", [(100, 50), (1000, 500), (5000, 2500), (1025, 1), (300, 299), (2, 1), (33000, 16500)])
+def test_select_lowest_bit_exact(ggauss, oracle, n, k):
+    rng = np.random.default_rng(n)
+    l = rng.normal(size=n) * 10
+    l[rng.integers(0, n, n // 4)] = l[0]           # ties -> slot order
+    if n > 10:
+        l[5] = -np.inf
+        l[n - 1] = -np.inf
+    dead, surv, lstar = ggauss.nss_select_lowest(l, k)
+    if n <= 5000:
+        odead, osurv = oracle.select_lowest(l, k)
+    else:
+        order = np.argsort(l, kind="stable")           # the library routine that pins the oracle (P12)
+        odead, osurv = order[:k], np.sort(order[k:])
+    assert np.array_equal(dead.cpu().numpy(), odead)
+    assert np.array_equal(surv.cpu().numpy(), osurv)
+    assert lstar == l[odead[-1]]
+
+
+def test_tune_matches_oracle(nssmod, oracle):
+    rng = np.random.default_rng(1)
+    for d, n in ((11, 1000), (11, 5000), (4, 100), (1, 50), (7, 33)):
+        w = inputs.gaussian_workload(d)
+        g = nssmod.Nss(w)
+        scales = np.array([1.0, 0.1, 0.5, 0.5, 600.0, 1e-3, 1.5, 0.3, 0.6, 0.01, 0.014])[:d]
+        A = rng.normal(size=(d, d))
+        x = rng.normal(size=(n, d)) @ A.T * scales + 1e3 * scales
+        rc, mean, chol = g.nss_tune(x)
+        orc, omean, ocov, ochol = oracle.tune(x)
+        assert rc == 0 and orc == 0
+        assert np.allclose(mean.cpu().numpy(), omean, rtol=1e-13)
+        assert np.allclose(chol.cpu().numpy(), ochol, rtol=1e-8, atol=1e-300)
+        if d > 2:
+            x[:, 2] = x[:, 1]
+            assert g.nss_tune(x)[0] == nssmod.NSS_ECHOL
+        g.close()
+
+
+@pytest.mark.parametrize("n,k", [(1000, 500), (5000, 2500), (100, 1), (3000, 2999)])
+def test_evidence_update_matches_oracle(ggauss, oracle, n, k):
+    rng = np.random.default_rng(2)
+    dl = np.sort(rng.normal(size=k) * 5 - 1.2e4)
+    if k > 10:
+        dl[0] = -np.inf
+    logX, logZ = -0.7, -1.2e4
+    gx, gz, lw = ggauss.nss_evidence_update(dl, n, logX, logZ)
+    ox, oz, olw = oracle.evidence_update(dl, n, logX, logZ)
+    assert gx == pytest.approx(ox, rel=1e-13)
+    assert gz == pytest.approx(oz, rel=1e-13, abs=1e-9)
+    assert np.allclose(lw.cpu().numpy(), olw, rtol=0, atol=1e-9)
+    gx2, gz2, _ = ggauss.nss_evidence_update(dl, n, 0.0, -np.inf)
+    ox2, oz2, _ = oracle.evidence_update(dl, n, 0.0, -np.inf)
+    assert gz2 == pytest.approx(oz2, rel=1e-13)
+
+
+def test_init_live_matches_oracle(nssmod, oracle, wl1):
+    g, p = nssmod.Nss(wl1), oracle.Problem(wl1)
+    live, logL = g.nss_init_live(300, 77)
+    olive, ologL = p.init_live(300, 77)
+    assert np.array_equal(live.cpu().numpy(), olive)                 # same Philox words, same affine map
+    assert np.allclose(logL.cpu().numpy(), ologL, rtol=1e-9, atol=1e-6)
+    g.close()
+
+
+def _trajectory_parity(g, p, live, logL, k, n_repeats, seed, it, logLstar=math.nan, max_excluded=0.03, w=None):
+    r = g.nss_replace_step(live, logL, k, n_repeats, seed, it, logLstar=logLstar, want_trace=True)
+    o = p.replace_step(live, logL, k, n_repeats, seed, it, logLstar=logLstar, want_trace=True)
+    assert o["rc"] == 0
+    assert np.array_equal(r["dead_idx"].cpu().numpy(), o["dead_idx"])
+    assert np.array_equal(r["dead_theta"].cpu().numpy(), o["dead_theta"])
+    assert np.array_equal(r["dead_logL"].cpu().numpy(), o["dead_logL"])
+    assert r["logLstar"] == o["logLstar"]
+    gtr, otr = r["trace"].cpu().numpy(), o["trace"]
+    margin = np.minimum(r["margin"].cpu().numpy(), o["margin"])
+    safe = margin > 1e-6                          # A20: chains whose bracket tests all clear L* by > 1e-6
+    assert safe.mean() >= 1 - max_excluded, f"{(~safe).sum()} of {k} chains excluded"
+    assert np.array_equal(gtr[safe], otr[safe])                       # identical decisions
+    didx = o["dead_idx"]
+    gl, ol = r["live"].cpu().numpy(), o["live"]
+    width = (w.hi - w.lo) if w is not None else 1.0
+    assert np.all(np.abs(gl[didx][safe] - ol[didx][safe]) <= 1e-9 * width)
+    glog, olog = r["logL"].cpu().numpy(), o["logL"]
+    assert np.all(np.abs(glog[didx][safe] - olog[didx][safe]) <= 1e-6 + 1e-9 * np.abs(olog[didx][safe]))
+    surv = np.setdiff1d(np.arange(live.shape[0]), didx)
+    assert np.array_equal(gl[surv], np.asarray(live)[surv]) and np.array_equal(glog[surv], np.asarray(logL)[surv])
+    if safe.all():
+        assert r["n_evals"] == o["n_evals"]
+    assert np.all(glog[didx] > o["logLstar"])
+    return r, o, safe
+
+
+def test_replace_step_trajectories_gaussian(nssmod, oracle):
+    for d, n, k in ((4, 1000, 500), (11, 400, 399), (3, 64, 1)):
+        w = inputs.gaussian_workload(d, sigma=0.05)
+        g, p = nssmod.Nss(w), oracle.Problem(w)
+        live, logL = p.init_live(n, 3)
+        _trajectory_parity(g, p, live, logL, k, 3 * d, seed=3, it=0, w=w)
+        # a later iteration, compressed population
+        live2 = live * 0.1
+        logL2 = p.loglike_batch(live2)
+        _trajectory_parity(g, p, live2, logL2, k, 3 * d, seed=3, it=7, w=w)
+        g.close()
+
+
+def test_replace_step_trajectories_config1(nssmod, oracle, wl1):
+    g, p = nssmod.Nss(wl1), oracle.Problem(wl1)
+    live, logL = p.init_live(100, 1)
+    state = (live, logL)
+    for it in range(3):                                   # follow the oracle's own state (teacher forcing)
+        r, o, safe = _trajectory_parity(g, p, state[0], state[1], 50, 12, seed=1, it=it, w=wl1, max_excluded=0.06)
+        state = (o["live"], o["logL"])
+    g.close()
+
+
+def test_replace_step_trajectories_config2_and_teacher_forced_threshold(nssmod, oracle, wl2):
+    g, p = nssmod.Nss(wl2), oracle.Problem(wl2)
+    live, logL = p.init_live(1000, 2)
+    r, o, safe = _trajectory_parity(g, p, live, logL, 500, 6, seed=2, it=0, w=wl2)
+    # teacher-forced threshold below the internal one: same deletions, looser constraint
+    forced = o["logLstar"] - 5.0
+    _trajectory_parity(g, p, live, logL, 500, 3, seed=2, it=1, logLstar=forced, w=wl2)
+    # a survivor below the supplied threshold is rejected on both sides
+    bad = float(np.max(logL))
+    assert p.replace_step(live, logL, 500, 1, 2, 0, logLstar=bad)["rc"] == -2
+    assert g.nss_replace_step(live, logL, 500, 1, 2, 0, logLstar=bad, ok=(nssmod.NSS_EINVAL,))["rc"] == nssmod.NSS_EINVAL
+    g.close()
+
+
+def test_replace_step_full_grid_kind(nssmod, oracle):
+    w = inputs.make_data(inputs.config4(), oracle.waveform)
+    g, p = nssmod.Nss(w), oracle.Problem(w)
+    live, logL = p.init_live(64, 5)
+    _trajectory_parity(g, p, live, logL, 32, 2, seed=5, it=0, w=w, max_excluded=0.1)
+    g.close()
+
+
+def test_replace_step_degenerate_population_reports_cholesky(nssmod, oracle):
+    w = inputs.gaussian_workload(3)
+    g = nssmod.Nss(w)
+    live = np.random.default_rng(0).uniform(-1, 1, size=(50, 3))
+    live[:, 2] = live[:, 1]
+    logL = oracle.Problem(w).loglike_batch(live)
+    r = g.nss_replace_step(live, logL, 25, 2, 1, 0, ok=(nssmod.NSS_ECHOL,))
+    assert r["rc"] == nssmod.NSS_ECHOL
+    assert np.array_equal(r["live"].cpu().numpy(), live)             # nothing was replaced
+    g.close()
+
+
+def _analytic_logz(d, sigma, half):
+    c = scipy.stats.norm.cdf(half / sigma) - scipy.stats.norm.cdf(-half / sigma)
+    return d * math.log(sigma * math.sqrt(2 * math.pi) / (2 * half) * c)
+
+
+@pytest.mark.parametrize("d,n,k,seed", [(4, 1000, 500, 1), (11, 600, 300, 3)])
+def test_run_gaussian_matches_oracle_and_analytic(nssmod, oracle, d, n, k, seed):
+    w = inputs.gaussian_workload(d, sigma=0.05)
+    g, p = nssmod.Nss(w), oracle.Problem(w)
+    r = g.nss_run(n, k, 5 * d, seed)
+    o = p.run(n, k, 5 * d, seed)
+    truth = _analytic_logz(d, 0.05, 1.0)
+    assert r["rc"] == 0
+    assert abs(r["logZ"] - truth) < 3 * r["logZ_err"]
+    assert abs(r["logZ"] - o["logZ"]) < 3 * math.hypot(r["logZ_err"], o["logZ_err"])
+    assert abs(r["n_iter"] - o["n_iter"]) <= 1
+    assert r["logZ_err"] == pytest.approx(o["logZ_err"], rel=0.3)
+    assert r["H"] == pytest.approx(o["H"], abs=0.5)
+    nd, ni = r["n_dead"], r["n_iter"]
+    assert nd == ni * k + n
+    assert np.sum(np.exp(r["dead_logw"])) == pytest.approx(1.0, abs=1e-10)
+    dl = r["dead_logL"]
+    assert np.all(np.diff(dl[:ni * k].reshape(ni, k), axis=1) >= 0) and np.all(np.diff(dl[ni * k:]) >= 0)
+    assert np.all(r["dead_logL_birth"] < dl)
+    pw = np.exp(dl + r["dead_logw"] - r["logZ"])
+    ess = 1.0 / np.sum(pw ** 2)
+    mean = pw @ r["dead_theta"]
+    sd = np.sqrt(pw @ (r["dead_theta"] - mean) ** 2)
+    assert np.all(np.abs(mean) < 5 * 0.05 / math.sqrt(ess)) and np.all(np.abs(sd / 0.05 - 1) < 0.15)
+    g.close()
+
+
+def test_run_config1_matches_oracle(nssmod, oracle, wl1):
+    """End-to-end: logZ within 3 sigma_NS, posterior means within 0.1 sigma of the posterior width,
+    over the seed ensemble of config 1 (trajectories are identical until a near-threshold test flips)."""
+    g, p = nssmod.Nss(wl1), oracle.Problem(wl1)
+    dz, exact = [], 0
+    for seed in (1, 2, 3, 4):
+        r = g.nss_run(100, 50, 12, seed)
+        o = p.run(100, 50, 12, seed)
+        assert r["rc"] == 0 and o["rc"] == 0
+        sig = math.hypot(r["logZ_err"], o["logZ_err"])
+        assert abs(r["logZ"] - o["logZ"]) < 3 * sig
+        dz.append(r["logZ"] - o["logZ"])
+        if r["n_dead"] == o["n_dead"] and np.allclose(r["dead_logL"], o["dead_logL"], rtol=1e-9, atol=1e-6):
+            exact += 1
+            assert np.allclose(r["dead_logw"], o["dead_logw"], rtol=0, atol=1e-9)
+            assert r["logZ"] == pytest.approx(o["logZ"], abs=1e-6)
+            assert r["n_evals"] == o["n_evals"]
+        pw_g = np.exp(r["dead_logL"] + r["dead_logw"] - r["logZ"])
+        pw_o = np.exp(o["dead_logL"] + o["dead_logw"] - o["logZ"])
+        mg, mo = pw_g @ r["dead_theta"], pw_o @ o["dead_theta"]
+        so = np.sqrt(pw_o @ (o["dead_theta"] - mo) ** 2)
+        if exact:
+            assert np.all(np.abs(mg - mo) < 0.1 * so)
+    assert exact >= 2, "at least half the seeds should replay bit-for-bit identical decision sequences"
+    g.close()

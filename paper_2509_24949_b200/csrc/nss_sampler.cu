@@ -78,7 +78,7 @@ __global__ void k_init_live(const __grid_constant__ NssDev P, int n, uint64_t se
   uint64_t ka, kb;
   draw53(seed, (uint32_t)(j >> 1), 0u, (uint32_t)i, kIterInit, ka, kb);
   const double u = (double)((j & 1) ? kb : ka) * kTwoM53;
-  live[idx] = P.lo[j] + (P.hi[j] - P.lo[j]) * u;
+  live[idx] = __dadd_rn(P.lo[j], __dmul_rn(P.hi[j] - P.lo[j], u));   // unfused: same bits as the oracle
 }
 
 // ---- K4.1 (O12.1): rank of every live point in (logL, slot) order, by counting ------------------------------
@@ -386,7 +386,7 @@ __global__ void __launch_bounds__(kChainThreads) k3_slice(const __grid_constant_
 #pragma unroll
     for (int j = 0; j < NSS_NSLOT; ++j)
       if (j < d) {
-        y[j] = x[j] + t * v[j];
+        y[j] = __dadd_rn(x[j], __dmul_rn(t, v[j]));
         in = in && (y[j] >= P.lo[j]) && (y[j] <= P.hi[j]);
       }
     if (!in) return false;
@@ -434,7 +434,7 @@ __global__ void __launch_bounds__(kChainThreads) k3_slice(const __grid_constant_
     int acc = -1;
     for (int kk = 0; kk < kMaxShrink; ++kk) {
       const double uk = uniform_a(A.seed, (uint32_t)(64 + kk), (uint32_t)s, chain, it);
-      const double t = l + (r - l) * uk;
+      const double t = __dadd_rn(l, __dmul_rn(r - l, uk));
       if (inside(t, ly)) {
 #pragma unroll
         for (int j = 0; j < NSS_NSLOT; ++j) x[j] = y[j];

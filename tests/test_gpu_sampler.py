@@ -69,8 +69,8 @@ def test_tune_matches_oracle(nssmod, oracle):
         assert np.allclose(mean.cpu().numpy(), omean, rtol=1e-13)
         assert np.allclose(chol.cpu().numpy(), ochol, rtol=1e-8, atol=1e-300)
         if d > 2:
-            x[:, 2] = x[:, 1]
-            assert g.nss_tune(x)[0] == nssmod.NSS_ECHOL
+            x[:, 2] = 7.0                   # zero variance: the pivot is exactly 0 on both sides
+            assert g.nss_tune(x)[0] == nssmod.NSS_ECHOL and oracle.tune(x)[0] != 0
         g.close()
 
 
@@ -176,7 +176,7 @@ def test_replace_step_degenerate_population_reports_cholesky(nssmod, oracle):
     w = inputs.gaussian_workload(3)
     g = nssmod.Nss(w)
     live = np.random.default_rng(0).uniform(-1, 1, size=(50, 3))
-    live[:, 2] = live[:, 1]
+    live[:, 2] = 0.25
     logL = oracle.Problem(w).loglike_batch(live)
     r = g.nss_replace_step(live, logL, 25, 2, 1, 0, ok=(nssmod.NSS_ECHOL,))
     assert r["rc"] == nssmod.NSS_ECHOL

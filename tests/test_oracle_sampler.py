@@ -111,7 +111,7 @@ def test_p12_tune_vs_numpy(oracle):
     assert np.allclose(chol @ chol.T, cov, rtol=1e-11)
     assert np.all(np.triu(chol, 1) == 0)
     # degenerate population -> pivot failure reported
-    x2 = x.copy(); x2[:, 3] = x2[:, 2]
+    x2 = x.copy(); x2[:, 3] = 7.0        # zero variance -> pivot exactly 0
     assert oracle.tune(x2)[0] != 0
 
 

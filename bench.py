@@ -1,0 +1,356 @@
+#!/usr/bin/env python
+"""bench.py — the measurement contract.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+A "step" is ONE COMPLETE NESTED-SLICE-SAMPLING ITERATION of BASELINE.json configs[1] (11 parameters,
+H1+L1+V1, relative binning with 128 bins per detector, n_live = 1000, n_delete = 500, 55 slice
+repeats): delete-select, evidence bookkeeping, covariance + Cholesky, 500 slice chains whose every
+bracket test is one heterodyned log-likelihood evaluation, in-place replacement, live-evidence stop
+test — one `nss_iterate` call of the C ABI.  Steps are consecutive
+iterations of one seeded run (a fresh run is started, untimed, whenever the stop rule fires).
+
+metric  = heterodyned logL evaluations per second (sequential-algorithm count / device time)
+value   = device-resident steps (CUDA events around each step on the launching stream)
+e2e     = the same through `nss_iterate_host` with pinned HOST buffers (H2D + D2H inside the call)
+roofline= the dominant kernel (K3 slice chains): fp64 flop of the likelihood evaluations it made /
+          its own CUDA-event duration, against the DFMA peak measured in the same process
+extras  = K1 batch-likelihood microbenchmark (config 5, N = 1e6), a full `nss_run` to convergence,
+          the oracle timed on the host cores (cpu_baseline).
+
+`--impl reference` times the ORACLE (oracle/, plain C on the host cores) on a bounded sample of the same
+workload; it is the only other place this file executes oracle/ code.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "heterodyned logL evals/s (NSS iteration, config 2)"
+UNIT = "evals/s"
+SEED = 1
+
+
+# ---- algorithmic work of one relative-binning likelihood evaluation -------------------------
+def rb_work(B: int, n_det: int):
+    """(fp64-pipe instructions, flop) one evaluation needs: per point, per edge, per (edge, detector),
+    per (bin, detector).  FMA = 1 instruction = 2 flop; add/mul = 1 flop."""
+    E = B + 1
+    per_point_i, per_point_f = 600, 900
+    edge_i, edge_f = 8, 16                       # 8 FMA: phase difference against the tabulated basis
+    ed_i, ed_f = 27, 45                          # arrival-time FMA, range reduction, sincospi, complex scale
+    bd_i, bd_f = 15, 23                          # sums/differences of the edge ratios, six pre-scaled terms
+    instr = per_point_i + E * edge_i + E * n_det * ed_i + B * n_det * bd_i
+    flop = per_point_f + E * edge_f + E * n_det * ed_f + B * n_det * bd_f
+    return instr, flop
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled in a thread while the GPU is under load."""
+
+    def __init__(self, index=0, period=0.02):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._t = None
+        self.period = period
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
+                 "hw_power_brake": 0x80, "sync_boost": 0x10, "applications_clocks_setting": 0x2}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h) if hasattr(nv, "nvmlDeviceGetCurrentClocksEventReasons") \
+                    else nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def __enter__(self):
+        if self.nv:
+            self._t = threading.Thread(target=self._run, daemon=True)
+            self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._t:
+            self._t.join()
+
+    def summary(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+def oracle_steps(w_oracle, steps, warmup, n_repeats, seed):
+    """Times the oracle, as it stands, on the host cores: consecutive NS iterations of config 2 with
+    `n_repeats` slice repeats per chain.  Returns (evals, seconds, cores)."""
+    from oracle import nss_oracle as orc
+    p = orc.Problem(w_oracle)
+    cores = orc.n_cores()
+    live, logL = p.init_live(w_oracle.n_live, seed, nthreads=cores)
+    evals, secs = 0, 0.0
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        o = p.replace_step(live, logL, w_oracle.n_delete, n_repeats, seed, it, nthreads=cores)
+        orc.evidence_update(o["dead_logL"], w_oracle.n_live, 0.0, -math.inf)
+        dt = time.perf_counter() - t0
+        assert o["rc"] == 0
+        live, logL = o["live"], o["logL"]
+        if it >= warmup:
+            evals += o["n_evals"]
+            secs += dt
+    return evals, secs, cores
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, on a bounded sample of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from oracle import nss_oracle as orc
+    from paper_2509_24949_b200 import inputs
+    orc.build()
+    w = inputs.make_data(inputs.config2(), orc.waveform)
+    n_rep = 5
+    evals, secs, cores = oracle_steps(w, args.steps, args.warmup, n_rep, SEED)
+    v = evals / secs
+    sample = (f"{args.steps} consecutive NS iterations of config 2 (n_live 1000, n_delete 500) with {n_rep} slice repeats "
+              f"per chain instead of 55 (evals/s is per evaluation), OpenMP over chains on {cores} cores")
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": config_dict(w),
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def config_dict(w):
+    return {"workload": "BASELINE.json configs[1]: 11-param aligned-spin BBH, H1+L1+V1, TaylorF2 3.5PN + 1.5PN SO, "
+                        "aLIGO-fit PSD, 20-1024 Hz df 0.25 (4017 bins), SNR-20 injection + seeded coloured noise, "
+                        "relative binning B=128/detector, n_live 1000, n_delete 500, 55 slice repeats",
+            "n_live": int(w.n_live), "n_delete": int(w.n_delete), "n_repeats": int(w.n_repeats), "n_bins": int(w.n_bins),
+            "n_det": int(w.n_det), "d": int(w.d), "seed": SEED,
+            "l2": "flushed (256 MiB write) between steps, outside the per-step event pairs; working set < 1 MB, ALU-bound"}
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    from paper_2509_24949_b200 import build, inputs, nss
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        build.build()
+    if dist:
+        dist.barrier()
+
+    # inputs: injection synthesised by the CUDA library's own host waveform (never the oracle's)
+    w = inputs.make_data(inputs.config2(), nss.nss_waveform)
+    g = nss.Nss(w)
+    n, k, nrep, d = w.n_live, w.n_delete, w.n_repeats, w.d
+    seed = SEED + 1000 * rank                      # replicas only: independent seeds per GPU
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def fresh(sd):
+        live, logL = g.nss_init_live(n, sd)
+        return live, logL, nss.nss_iter_state(logX=0.0, logZ=-math.inf), 0
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    peak_tf = nss.nss_fp64_peak(300.0)
+
+    with ClockSampler(local) as clocks:
+        # ---- device-resident steps -----------------------------------------------------------------------
+        live, logL, st, it = fresh(seed)
+        bufs = g.iter_buffers(k)
+        runs = 0
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        evals, k3_ms, launches0 = 0, 0.0, 0
+        barrier()
+        wall0 = None
+        for s in range(args.warmup + args.steps):
+            if s == args.warmup:
+                barrier()
+                wall0 = time.perf_counter()
+                launches0 = g.launches
+            if st.converged:
+                runs += 1
+                live, logL, st, it = fresh(seed + 7919 * runs)
+            flush.fill_(s & 0xFF)
+            if s >= args.warmup:
+                ev[s - args.warmup][0].record(stream)
+            g.nss_iterate(live, logL, k, nrep, seed + 7919 * runs, it, st, bufs)
+            if s >= args.warmup:
+                ev[s - args.warmup][1].record(stream)
+                evals += st.n_evals
+                k3_ms += g.nss_last_chain_ms()
+            it += 1
+        barrier()
+        wall = time.perf_counter() - wall0
+        launches = g.launches - launches0
+        ms = sum(a.elapsed_time(b) for a, b in ev)
+
+        # ---- end to end: pinned host buffers through nss_iterate_host ----------------------------------------
+        live_d, logL_d, st_h, it_h = fresh(seed + 1)
+        live_h = torch.empty((n, d), dtype=torch.float64, pin_memory=True)
+        logL_h = torch.empty(n, dtype=torch.float64, pin_memory=True)
+        live_h.copy_(live_d); logL_h.copy_(logL_d)
+        hb = g.iter_buffers(k, host=True)
+        e2e_steps = args.steps
+        evals_h, t_h = 0, 0.0
+        barrier()
+        for s in range(args.warmup + e2e_steps):
+            if st_h.converged:
+                live_d, logL_d, st_h, it_h = fresh(seed + 1 + 104729 * (s + 1))
+                live_h.copy_(live_d); logL_h.copy_(logL_d)
+                torch.cuda.synchronize()
+            flush.fill_(s & 0xFF)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            g.nss_iterate(live_h, logL_h, k, nrep, seed + 1, it_h, st_h, hb, host=True)   # synchronous
+            dt = time.perf_counter() - t0
+            if s >= args.warmup:
+                evals_h += st_h.n_evals
+                t_h += dt
+            it_h += 1
+        barrier()
+        h2d = n * d * 8 + n * 8
+        d2h = n * d * 8 + n * 8 + k * d * 8 + k * 8 + k * 8 + k * 4
+
+        # ---- K1 microbenchmark (config 5): N = 1e6 prior draws, B = 128 x 3 detectors --------------------------
+        N1 = 1_000_000
+        X = torch.as_tensor(inputs.draw_prior(w, N1, 5), device="cuda")
+        out = torch.empty(N1, dtype=torch.float64, device="cuda")
+        g.set_loglike_variant(1)
+        for _ in range(3):
+            g.nss_loglike_batch(X, out)
+        k1 = []
+        for _ in range(5):
+            flush.fill_(1)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            g.nss_loglike_batch(X, out)
+            b.record(stream)
+            b.synchronize()
+            k1.append(a.elapsed_time(b))
+        g.set_loglike_variant(0)
+        k1_ms = sorted(k1)[len(k1) // 2]
+
+        # ---- full run to convergence ------------------------------------------------------------------------
+        g.nss_run(n, k, nrep, seed)                         # warm
+        t0 = time.perf_counter()
+        r = g.nss_run(n, k, nrep, seed)
+        run_wall = time.perf_counter() - t0
+
+    # max over ranks of the timed quantities; sum of the work
+    if dist:
+        t = torch.tensor([ms, t_h, k3_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        c = torch.tensor([evals, evals_h, launches], dtype=torch.float64, device="cuda")
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+        ms, t_h, k3_ms = (float(x) for x in t)
+        evals, evals_h, launches = (int(x) for x in c)
+    if rank != 0:
+        if dist:
+            dist.destroy_process_group()
+        return 0
+
+    instr, flop = rb_work(w.n_bins, w.n_det)
+    value = evals / (ms * 1e-3)
+    k3_tf = (evals / world) * flop / (k3_ms * 1e-3) / 1e12
+    k1_rate = N1 / (k1_ms * 1e-3)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": config_dict(w),
+        "e2e": {"value": evals_h / t_h, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": 1e3 * t_h / e2e_steps, "timing": "host wall clock around the synchronous nss_iterate_host call"},
+        "gpu_launches": launches,
+        "evals_per_step": evals / args.steps / world,
+        "wall_ms_timed_region": 1e3 * wall,
+        "roofline": {"bound": "alu", "kernel": "k3_slice (persistent slice-sampling chains, likelihood inlined)",
+                     "achieved": k3_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": k3_tf / peak_tf,
+                     "peak_source": "fp64 DFMA chain measured in this process (nss_fp64_peak); nominal 148 SM x 64 lanes x 2 x "
+                                    "1.965 GHz = 37.2; MEASURED_PEAKS.json has no fp64 figure",
+                     "flop_per_eval": flop, "fp64_instr_per_eval": instr,
+                     "pipe_frac": (evals / world) * instr / (k3_ms * 1e-3) / (peak_tf * 1e12 / 2),
+                     "kernel_ms_per_step": k3_ms / args.steps, "kernel_share_of_step": k3_ms / ms, "traffic": None},
+        "loglike_batch": {"workload": "config 5: N=1e6 prior draws, B=128 x 3 detectors, k1_rb_thread", "ms": k1_ms,
+                          "evals_per_s": k1_rate, "tflops": k1_rate * flop / 1e12, "frac": k1_rate * flop / 1e12 / peak_tf,
+                          "pipe_frac": k1_rate * instr / (peak_tf * 1e12 / 2)},
+        "nss_run": {"wall_s": run_wall, "gpu_ms": r["gpu_ms"], "n_iter": r["n_iter"], "n_evals": r["n_evals"],
+                    "logZ": r["logZ"], "logZ_err": r["logZ_err"], "H": r["H"], "rc": r["rc"]},
+        "clocks": clocks.summary(),
+    }
+    # ---- CPU baseline: the oracle as it stands, on this box's host cores, bounded sample -----------------------
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle import nss_oracle as orc
+        orc.build()
+        wo = inputs.make_data(inputs.config2(), orc.waveform)
+        n_it = 2
+        ev_o, s_o, cores = oracle_steps(wo, n_it, 0, w.n_repeats, SEED)
+        line["cpu_baseline"] = {"value": ev_o / s_o, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"NS iterations 0..{n_it - 1} of the same config-2 run (n_live 1000, n_delete 500, "
+                                          f"55 repeats): {ev_o} evaluations in {s_o:.1f} s, OpenMP over chains"}
+    print(json.dumps(line))
+    g.close()
+    if dist:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

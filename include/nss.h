@@ -109,6 +109,40 @@ int nss_replace_step(nss_handle *h, double *live_dev, double *logL_dev, int32_t 
                      int32_t *dead_idx_dev, double *logLstar_host, int64_t *n_evals_host,
                      void *cuda_stream);
 
+/* One COMPLETE NS iteration = every row of the hot path with one host
+ * synchronisation: nss_replace_step's work (delete select, tuning, chains, replace; threshold
+ * selected internally), then the evidence bookkeeping of the deleted batch (O12.2) and the live
+ * evidence / stop test (O14).  This is the loop body of nss_run and the "step" bench.py times.
+ * state: logX, logZ in/out (start a run with 0, -inf); the rest out. */
+typedef struct {
+  double  logX, logZ;              /* in/out: log prior volume, log evidence of the dead points  */
+  double  logZ_live;               /* out: logX + logsumexp(logL_live) - ln n after the step     */
+  double  logLstar;                /* out: threshold of this iteration                           */
+  int64_t n_evals;                 /* out: sequential-algorithm likelihood evaluations           */
+  int32_t converged;               /* out: logZ_live - logZ < stop_dlogz                         */
+  int32_t pad_;
+} nss_iter_state;
+
+int nss_iterate(nss_handle *h, double *live_dev, double *logL_dev, int32_t n_live, int32_t n_delete,
+                int32_t n_repeats, uint64_t seed, uint32_t iteration, double stop_dlogz,
+                double *dead_theta_dev /*[n_delete][d]*/, double *dead_logL_dev /*[n_delete]*/,
+                double *dead_logw_dev /*[n_delete]*/, int32_t *dead_idx_dev /*[n_delete]*/,
+                nss_iter_state *state_host, void *cuda_stream);
+
+/* The same iteration with HOST buffers (pinned memory recommended): live/logL are copied to the
+ * device, the iteration runs, and live, logL and the dead rows are copied back, all on the stream,
+ * inside the call.  bench.py's end-to-end (`e2e`) leg. */
+int nss_iterate_host(nss_handle *h, double *live_host, double *logL_host, int32_t n_live,
+                     int32_t n_delete, int32_t n_repeats, uint64_t seed, uint32_t iteration,
+                     double stop_dlogz, double *dead_theta_host, double *dead_logL_host,
+                     double *dead_logw_host, int32_t *dead_idx_host, nss_iter_state *state_host,
+                     void *cuda_stream);
+
+/* Host-buffer form of nss_loglike_batch: theta_host [N][d] -> logL_host [N]; H2D copy, kernel and
+ * D2H copy on the stream, synchronised before returning. */
+int nss_loglike_batch_host(nss_handle *h, const double *theta_host, int64_t N, double *logL_host,
+                           void *cuda_stream);
+
 /* Test hook: if set (device pointers, may be NULL to clear), the next nss_replace_step calls also
  * write trace_dev [n_delete][n_repeats][3] = (left expansions, right expansions, accepted shrink
  * index or -1) and margin_dev [n_delete] = min |logL - logLstar| over the chain's bracket tests. */
@@ -162,6 +196,11 @@ int nss_get_tables(nss_handle *h, int32_t *edge_idx_host, double *summary_host, 
 /* Register-resident DFMA chain on every SM for ~`ms` milliseconds: measured fp64 FMA throughput,
  * the roofline denominator.  *tflops_host = 2 * FMA/s / 1e12. */
 int nss_fp64_peak(double ms, double *tflops_host, void *cuda_stream);
+
+/* Device time [ms] of the most recent K3 (slice-sampling chains) launch, from CUDA events the library
+ * records around it on the caller's stream (bench.py's roofline for the dominant kernel).
+ * NSS_EINVAL before the first iteration. */
+int nss_last_chain_ms(nss_handle *h, double *ms_host);
 
 /* Kernel launches issued by this handle since creation (bench.py's gpu_launches). */
 int64_t nss_launch_count(const nss_handle *h);

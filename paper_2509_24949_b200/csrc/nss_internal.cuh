@@ -53,6 +53,12 @@ struct nss_handle {
   double *d_birth;
   int32_t *trace_dev;
   double *margin_dev;
+  // device staging for the host-buffer entry points (grown on demand)
+  unsigned char *d_stage;
+  size_t stage_bytes;
+  // CUDA events recorded around the most recent K3 (slice chains) launch: nss_last_chain_ms
+  cudaEvent_t ev_k3[2];
+  int ev_k3_valid;
 };
 
 extern thread_local char g_nss_cuda_err[256];

@@ -467,6 +467,11 @@ int launch_chains(nss_handle *h, const ChainArgs &A, cudaStream_t st)
   size_t bytes = 0;
   if (P.kind == NSS_KIND_RB) bytes = (size_t)(9 * (P.rb_m + 1) + 6 * NDET * P.rb_m) * 32 * sizeof(double);
   const bool resident = P.kind == NSS_KIND_RB && bytes + 2048 <= 200 * 1024;
+  if (!h->ev_k3[0]) {
+    NSS_CUDA(cudaEventCreate(&h->ev_k3[0]));
+    NSS_CUDA(cudaEventCreate(&h->ev_k3[1]));
+  }
+  NSS_CUDA(cudaEventRecord(h->ev_k3[0], st));
   if (resident) {
     if (bytes > 48 * 1024)
       NSS_CUDA(cudaFuncSetAttribute(k3_slice<NDET, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
@@ -474,6 +479,8 @@ int launch_chains(nss_handle *h, const ChainArgs &A, cudaStream_t st)
   } else {
     k3_slice<NDET, false><<<grid, kChainThreads, 0, st>>>(P, A);
   }
+  NSS_CUDA(cudaEventRecord(h->ev_k3[1], st));
+  h->ev_k3_valid = 1;
   h->launches += 1;
   NSS_CUDA(cudaGetLastError());
   return NSS_OK;
@@ -524,6 +531,16 @@ int enqueue_iteration(nss_handle *h, double *live, double *logL, double *birth, 
 }
 
 }  // namespace
+
+extern "C" int nss_last_chain_ms(nss_handle *h, double *ms_host)
+{
+  if (!h || !ms_host || !h->ev_k3_valid) return NSS_EINVAL;
+  NSS_CUDA(cudaEventSynchronize(h->ev_k3[1]));
+  float ms = 0.f;
+  NSS_CUDA(cudaEventElapsedTime(&ms, h->ev_k3[0], h->ev_k3[1]));
+  *ms_host = ms;
+  return NSS_OK;
+}
 
 extern "C" int nss_set_trace(nss_handle *h, int32_t *trace_dev, double *margin_dev)
 {
@@ -640,6 +657,109 @@ extern "C" int nss_replace_step(nss_handle *h, double *live_dev, double *logL_de
   if (n_evals_host) *n_evals_host = (int64_t)ne;
   if (flags[1]) return NSS_EINVAL;
   if (flags[0]) return NSS_ECHOL;
+  return NSS_OK;
+}
+
+namespace {
+int ensure_stage(nss_handle *h, size_t bytes)
+{
+  if (h->stage_bytes >= bytes && h->d_stage) return NSS_OK;
+  cudaFree(h->d_stage);
+  h->d_stage = nullptr; h->stage_bytes = 0;
+  cudaError_t e = cudaMalloc((void **)&h->d_stage, bytes);
+  if (e != cudaSuccess) { nss_cuda_fail(e, "cudaMalloc(stage)"); return e == cudaErrorMemoryAllocation ? NSS_ENOMEM : NSS_ECUDA; }
+  h->stage_bytes = bytes;
+  return NSS_OK;
+}
+size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
+}  // namespace
+
+extern "C" int nss_iterate(nss_handle *h, double *live_dev, double *logL_dev, int32_t n_live, int32_t n_delete, int32_t n_repeats,
+                           uint64_t seed, uint32_t iteration, double stop_dlogz, double *dead_theta_dev, double *dead_logL_dev,
+                           double *dead_logw_dev, int32_t *dead_idx_dev, nss_iter_state *state_host, void *cuda_stream)
+{
+  if (!h || !live_dev || !logL_dev || !dead_theta_dev || !dead_logL_dev || !dead_logw_dev || !dead_idx_dev || !state_host)
+    return NSS_EINVAL;
+  if (n_live < 2 || n_delete < 1 || n_delete >= n_live || n_repeats < 0) return NSS_EINVAL;
+  NSS_CUDA(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = ensure_scratch(h, n_live);
+  if (rc) return rc;
+  double state[4] = {state_host->logX, state_host->logZ, 0.0, 0.0};
+  NSS_CUDA(cudaMemcpyAsync(h->d_state, state, sizeof(state), cudaMemcpyHostToDevice, st));
+  NSS_CUDA(cudaMemsetAsync(h->d_flags, 0, sizeof(int32_t) * 4, st));
+  NSS_CUDA(cudaMemsetAsync(h->d_nevals, 0, sizeof(unsigned long long), st));
+  rc = enqueue_iteration(h, live_dev, logL_dev, nullptr, n_live, n_delete, NAN, n_repeats, seed, iteration, dead_theta_dev,
+                         dead_logL_dev, nullptr, dead_idx_dev, st);
+  if (rc) return rc;
+  k4_evidence<<<1, kOneCta, 0, st>>>(dead_logL_dev, n_live, n_delete, dead_logw_dev, h->d_state);
+  k4_live_evidence<<<1, kOneCta, 0, st>>>(logL_dev, n_live, stop_dlogz, 1, h->d_state, h->d_flags);
+  h->launches += 2;
+  NSS_CUDA(cudaGetLastError());
+  int32_t flags[4];
+  unsigned long long ne = 0;
+  NSS_CUDA(cudaMemcpyAsync(flags, h->d_flags, sizeof(flags), cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaMemcpyAsync(state, h->d_state, sizeof(state), cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaMemcpyAsync(&ne, h->d_nevals, sizeof(ne), cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaStreamSynchronize(st));
+  if (flags[0]) return NSS_ECHOL;
+  state_host->logX = state[0]; state_host->logZ = state[1]; state_host->logZ_live = state[2]; state_host->logLstar = state[3];
+  state_host->n_evals = (int64_t)ne;
+  state_host->converged = flags[2];
+  return NSS_OK;
+}
+
+extern "C" int nss_iterate_host(nss_handle *h, double *live_host, double *logL_host, int32_t n_live, int32_t n_delete,
+                                int32_t n_repeats, uint64_t seed, uint32_t iteration, double stop_dlogz, double *dead_theta_host,
+                                double *dead_logL_host, double *dead_logw_host, int32_t *dead_idx_host, nss_iter_state *state_host,
+                                void *cuda_stream)
+{
+  if (!h || !live_host || !logL_host || !dead_theta_host || !dead_logL_host || !dead_logw_host || !dead_idx_host || !state_host)
+    return NSS_EINVAL;
+  if (n_live < 2 || n_delete < 1 || n_delete >= n_live || n_repeats < 0) return NSS_EINVAL;
+  NSS_CUDA(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t d = (size_t)h->dev.d, n = (size_t)n_live, k = (size_t)n_delete;
+  const size_t o_live = 0, o_logL = o_live + align256(n * d * 8), o_dth = o_logL + align256(n * 8),
+               o_dl = o_dth + align256(k * d * 8), o_dw = o_dl + align256(k * 8), o_di = o_dw + align256(k * 8),
+               total = o_di + align256(k * 4);
+  int rc = ensure_stage(h, total);
+  if (rc) return rc;
+  unsigned char *b = h->d_stage;
+  double *live = (double *)(b + o_live), *logL = (double *)(b + o_logL), *dth = (double *)(b + o_dth), *dl = (double *)(b + o_dl),
+         *dw = (double *)(b + o_dw);
+  int32_t *di = (int32_t *)(b + o_di);
+  NSS_CUDA(cudaMemcpyAsync(live, live_host, n * d * 8, cudaMemcpyHostToDevice, st));
+  NSS_CUDA(cudaMemcpyAsync(logL, logL_host, n * 8, cudaMemcpyHostToDevice, st));
+  // the device copies are queued behind the iteration; nss_iterate's synchronisation is followed by one more below
+  rc = nss_iterate(h, live, logL, n_live, n_delete, n_repeats, seed, iteration, stop_dlogz, dth, dl, dw, di, state_host, st);
+  if (rc) return rc;
+  NSS_CUDA(cudaMemcpyAsync(live_host, live, n * d * 8, cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaMemcpyAsync(logL_host, logL, n * 8, cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaMemcpyAsync(dead_theta_host, dth, k * d * 8, cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaMemcpyAsync(dead_logL_host, dl, k * 8, cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaMemcpyAsync(dead_logw_host, dw, k * 8, cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaMemcpyAsync(dead_idx_host, di, k * 4, cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaStreamSynchronize(st));
+  return NSS_OK;
+}
+
+extern "C" int nss_loglike_batch_host(nss_handle *h, const double *theta_host, int64_t N, double *logL_host, void *cuda_stream)
+{
+  if (!h || N < 0) return NSS_EINVAL;
+  if (N == 0) return NSS_OK;
+  if (!theta_host || !logL_host) return NSS_EINVAL;
+  NSS_CUDA(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t d = (size_t)h->dev.d, o_out = align256((size_t)N * d * 8);
+  int rc = ensure_stage(h, o_out + align256((size_t)N * 8));
+  if (rc) return rc;
+  double *th = (double *)h->d_stage, *out = (double *)(h->d_stage + o_out);
+  NSS_CUDA(cudaMemcpyAsync(th, theta_host, (size_t)N * d * 8, cudaMemcpyHostToDevice, st));
+  rc = nss_launch_loglike(h, th, N, out, st);
+  if (rc) return rc;
+  NSS_CUDA(cudaMemcpyAsync(logL_host, out, (size_t)N * 8, cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaStreamSynchronize(st));
   return NSS_OK;
 }
 

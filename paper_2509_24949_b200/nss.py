@@ -51,9 +51,16 @@ class nss_result(C.Structure):
         ("dead_logw", C.POINTER(C.c_double)), ("cap", C.c_int64), ("gpu_ms", C.c_double)]
 
 
-EXPORTS = ("nss_create", "nss_destroy", "nss_loglike_batch", "nss_set_loglike_variant", "nss_replace_step",
+class nss_iter_state(C.Structure):
+    _fields_ = [("logX", C.c_double), ("logZ", C.c_double), ("logZ_live", C.c_double), ("logLstar", C.c_double),
+                ("n_evals", C.c_int64), ("converged", C.c_int32), ("pad_", C.c_int32)]
+
+
+EXPORTS = ("nss_create", "nss_destroy", "nss_loglike_batch", "nss_loglike_batch_host", "nss_set_loglike_variant",
+           "nss_replace_step", "nss_iterate", "nss_iterate_host",
            "nss_set_trace", "nss_select_lowest", "nss_tune", "nss_evidence_update", "nss_init_live",
            "nss_philox", "nss_run", "nss_waveform", "nss_get_tables", "nss_fp64_peak", "nss_launch_count",
+           "nss_last_chain_ms",
            "nss_strerror", "nss_last_cuda_error", "nss_version")
 
 _lib = None
@@ -76,6 +83,10 @@ def lib():
         L.nss_replace_step.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, C.c_double, C.c_int32, C.c_uint64,
                                        C.c_uint32, vp, vp, vp, c_dp, C.POINTER(C.c_int64), vp]
         L.nss_set_trace.argtypes = [vp, vp, vp]
+        L.nss_iterate.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, C.c_uint64, C.c_uint32, C.c_double,
+                                  vp, vp, vp, vp, C.POINTER(nss_iter_state), vp]
+        L.nss_iterate_host.argtypes = L.nss_iterate.argtypes
+        L.nss_loglike_batch_host.argtypes = [vp, vp, C.c_int64, vp, vp]
         L.nss_select_lowest.argtypes = [vp, vp, C.c_int32, C.c_int32, vp, vp, c_dp, vp]
         L.nss_tune.argtypes = [vp, vp, C.c_int32, vp, vp, vp]
         L.nss_evidence_update.argtypes = [vp, vp, C.c_int32, C.c_int32, vp, c_dp, vp]
@@ -87,6 +98,7 @@ def lib():
         L.nss_get_tables.argtypes = [vp, vp, c_dp, c_dp]
         L.nss_fp64_peak.argtypes = [C.c_double, c_dp, vp]
         L.nss_launch_count.argtypes = [vp]
+        L.nss_last_chain_ms.argtypes = [vp, c_dp]
         L.nss_launch_count.restype = C.c_int64
         L.nss_strerror.argtypes = [C.c_int]
         L.nss_strerror.restype = C.c_char_p
@@ -189,6 +201,11 @@ class Nss:
     def launches(self) -> int:
         return int(lib().nss_launch_count(self._h))
 
+    def nss_last_chain_ms(self) -> float:
+        ms = C.c_double()
+        _check(lib().nss_last_chain_ms(self._h, C.byref(ms)), "nss_last_chain_ms")
+        return ms.value
+
     def set_loglike_variant(self, variant: int):
         _check(lib().nss_set_loglike_variant(self._h, int(variant)), "nss_set_loglike_variant")
 
@@ -202,12 +219,30 @@ class Nss:
         _check(lib().nss_loglike_batch(self._h, th.data_ptr(), n, out.data_ptr(), _stream()), "nss_loglike_batch")
         return out
 
-    def nss_loglike_batch_host(self, theta_pinned, out_pinned, theta_dev, out_dev):
-        """End-to-end form used by bench.py: H2D copy, kernel, D2H copy on the current stream."""
-        theta_dev.copy_(theta_pinned, non_blocking=True)
-        _check(lib().nss_loglike_batch(self._h, theta_dev.data_ptr(), theta_dev.shape[0], out_dev.data_ptr(), _stream()),
-               "nss_loglike_batch")
-        out_pinned.copy_(out_dev, non_blocking=True)
+    def nss_loglike_batch_host(self, theta_host, out_host):
+        """Host-buffer form (torch CPU tensors, pinned recommended): H2D copy, kernel, D2H copy inside the call."""
+        n = theta_host.shape[0]
+        _check(lib().nss_loglike_batch_host(self._h, theta_host.data_ptr(), n, out_host.data_ptr(), _stream()),
+               "nss_loglike_batch_host")
+        return out_host
+
+    def iter_buffers(self, n_delete, host=False):
+        """Caller-allocated outputs of nss_iterate / nss_iterate_host (dead_theta, dead_logL, dead_logw, dead_idx)."""
+        torch = self.torch
+        kw = dict(device="cpu", pin_memory=True) if host else dict(device="cuda")
+        k = int(n_delete)
+        return (torch.empty((k, self.d), dtype=torch.float64, **kw), torch.empty(k, dtype=torch.float64, **kw),
+                torch.empty(k, dtype=torch.float64, **kw), torch.empty(k, dtype=torch.int32, **kw))
+
+    def nss_iterate(self, live, logL, n_delete, n_repeats, seed, iteration, state, bufs, stop_dlogz=-3.0, host=False):
+        """One complete NS iteration IN PLACE on (live, logL): device tensors, or (host=True) CPU tensors.
+        `state` is an nss_iter_state carried between calls; `bufs` from iter_buffers()."""
+        fn = lib().nss_iterate_host if host else lib().nss_iterate
+        dth, dl, dw, di = bufs
+        _check(fn(self._h, live.data_ptr(), logL.data_ptr(), live.shape[0], int(n_delete), int(n_repeats), int(seed),
+                  int(iteration), float(stop_dlogz), dth.data_ptr(), dl.data_ptr(), dw.data_ptr(), di.data_ptr(),
+                  C.byref(state), _stream()), "nss_iterate_host" if host else "nss_iterate")
+        return state
 
     def nss_init_live(self, n_live, seed):
         torch = self.torch

@@ -3,6 +3,7 @@ import math
 
 import numpy as np
 import pytest
+import scipy.special
 import scipy.stats
 
 from paper_2509_24949_b200 import inputs
@@ -240,4 +241,46 @@ def test_run_config1_matches_oracle(nssmod, oracle, wl1):
         if exact:
             assert np.all(np.abs(mg - mo) < 0.1 * so)
     assert exact >= 2, "at least half the seeds should replay bit-for-bit identical decision sequences"
+    g.close()
+
+
+def test_iterate_device_and_host_forms_match_oracle(nssmod, oracle, wl1):
+    """nss_iterate = replace step + evidence bookkeeping + live evidence (all §8(a) rows); the host-buffer
+    form returns the same bits as the device form."""
+    import torch
+    g, p = nssmod.Nss(wl1), oracle.Problem(wl1)
+    n, k, nrep = 100, 50, 12
+    live, logL = p.init_live(n, 4)
+    st = nssmod.nss_iter_state(logX=0.0, logZ=-math.inf)
+    sth = nssmod.nss_iter_state(logX=0.0, logZ=-math.inf)
+    dl, dL = torch.as_tensor(live, device="cuda").clone(), torch.as_tensor(logL, device="cuda").clone()
+    hl, hL = torch.as_tensor(live).clone().pin_memory(), torch.as_tensor(logL).clone().pin_memory()
+    bufs, hbufs = g.iter_buffers(k), g.iter_buffers(k, host=True)
+    ol, oL, ox, oz = live, logL, 0.0, -math.inf
+    for it in range(3):
+        g.nss_iterate(dl, dL, k, nrep, 4, it, st, bufs)
+        g.nss_iterate(hl, hL, k, nrep, 4, it, sth, hbufs, host=True)
+        assert torch.equal(dl.cpu(), hl) and torch.equal(dL.cpu(), hL)
+        for a, b in zip(bufs, hbufs):
+            assert torch.equal(a.cpu(), b)
+        assert (st.logX, st.logZ, st.logZ_live, st.logLstar, st.n_evals) == \
+               (sth.logX, sth.logZ, sth.logZ_live, sth.logLstar, sth.n_evals)
+        # oracle, teacher-forced from the GPU's own pre-step state
+        o = p.replace_step(ol, oL, k, nrep, 4, it, want_trace=True)
+        ox, oz, olw = oracle.evidence_update(o["dead_logL"], n, ox, oz)
+        assert np.array_equal(bufs[3].cpu().numpy(), o["dead_idx"])
+        assert np.array_equal(bufs[1].cpu().numpy(), o["dead_logL"])
+        assert np.allclose(bufs[2].cpu().numpy(), olw, rtol=0, atol=1e-9)
+        assert st.logLstar == o["logLstar"]
+        assert st.logX == pytest.approx(ox, abs=1e-12) and st.logZ == pytest.approx(oz, abs=1e-9)
+        gl = dL.cpu().numpy()
+        lzl = st.logX + scipy.special.logsumexp(gl) - math.log(n)
+        assert st.logZ_live == pytest.approx(lzl, abs=1e-9)
+        assert st.converged == int(st.logZ_live - st.logZ < -3.0)
+        ol, oL = dl.cpu().numpy(), gl                    # follow the GPU state
+    # host-buffer likelihood form
+    X = torch.as_tensor(inputs.draw_prior(wl1, 777, 3)).pin_memory()
+    out = torch.empty(777, dtype=torch.float64).pin_memory()
+    g.nss_loglike_batch_host(X, out)
+    assert torch.equal(out, g.nss_loglike_batch(X.cuda()).cpu())
     g.close()

@@ -92,6 +92,12 @@ int nss_loglike_batch(nss_handle *h, const double *theta_dev, int64_t N, double 
  * 1 = one thread per point, 2 = one warp per point. */
 int nss_set_loglike_variant(nss_handle *h, int32_t variant);
 
+/* Warps that run one slice chain (K3): 0 = automatic (the widest of 1, 2, 4, 8 that keeps all n_delete
+ * chains resident on the GPU), else 1, 2, 4 or 8.  A group of G warps evaluates, in one round, the next G
+ * bracket tests of the sequential algorithm speculatively; the decisions, positions and evaluation count
+ * are those of the sequential algorithm for every G (tests/test_gpu_sampler.py). */
+int nss_set_chain_warps(nss_handle *h, int32_t warps);
+
 /* One NS iteration (O12): select the n_delete lowest logL (ascending, ties by lower slot), tune the
  * slice directions from the covariance of the full live set (Cholesky), run one chain per deleted
  * point (start = uniformly chosen survivor; n_repeats x {direction, stepping-out, shrinkage} under

@@ -11,7 +11,8 @@
 // Device-side problem description, passed to kernels by value (__grid_constant__).
 struct NssDev {
   int32_t d, n_det, kind, n_bins, n_edges, n_freq;
-  int32_t param_index[NSS_NSLOT];
+  int32_t param_index[NSS_NSLOT];   // sampled dim j -> canonical slot
+  int32_t slot_src[NSS_NSLOT];      // canonical slot t -> sampled dim, or -1 (fixed)
   double theta_fixed[NSS_NSLOT];
   double lo[NSS_NSLOT], hi[NSS_NSLOT];
   double gauss_mu[NSS_NSLOT], gauss_isig[NSS_NSLOT];
@@ -26,7 +27,7 @@ struct NssDev {
   // tables (device pointers owned by the handle)
   const double *rb_rec;   // AoS  [E][rb_rs]: g0..g7, F_e, pad, then per det 6 pre-scaled bin terms of bin e-1
   int32_t rb_rs;
-  const double *rb_soa;   // warp layout: edge part [9][m+1][32], then bin part [n_det*6][m][32]
+  const double *rb_soa;   // warp layout, edge-round major: [9][32], then m x ([9][32] edge, [n_det*6][32] bin terms)
   int32_t rb_m;           // bins per lane = ceil(B/32)
   const double *full_rec; // AoS [n_freq][full_rs]: g0..g7, f, f^-7/6, then per det (d_re, d_im, 4df/S), pad
   int32_t full_rs;
@@ -37,6 +38,7 @@ struct nss_handle {
   int device;
   int n_sm;
   int loglike_variant;
+  int chain_warps;          // warps per slice chain: 0 = automatic, else 1, 2, 4 or 8
   int64_t launches;
   // host copies kept for nss_get_tables
   std::vector<int32_t> edge_idx;

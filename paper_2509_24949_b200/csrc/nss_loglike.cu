@@ -32,10 +32,8 @@ __global__ void __launch_bounds__(kThreads) k1_rb_thread(const __grid_constant__
   }
   const int d = P.d;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
-    double x[NSS_NSLOT], th[NSS_NSLOT];
-#pragma unroll
-    for (int j = 0; j < NSS_NSLOT; ++j) x[j] = j < d ? theta[i * d + j] : 0.0;
-    nssk::canon_from_sampled(P, x, th);
+    double th[NSS_NSLOT];
+    nssk::canon_from_mem(P, theta + i * d, th);
     double l = -INFINITY;
     if (nssp::domain_ok(th)) {
       nssk::RbPoint<NDET> R;
@@ -67,10 +65,7 @@ __global__ void __launch_bounds__(kThreads) k1_rb_warp(const __grid_constant__ N
   const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int64_t nwarp = ((int64_t)gridDim.x * blockDim.x) >> 5;
   for (int64_t i = warp0; i < N; i += nwarp) {
-    double x[NSS_NSLOT];
-#pragma unroll
-    for (int j = 0; j < NSS_NSLOT; ++j) x[j] = j < d ? theta[i * d + j] : 0.0;
-    const double l = nssk::loglike_warp<NDET>(P, tab, x);
+    const double l = nssk::loglike_warp<NDET, NSS_KIND_RB>(P, tab, theta + i * d);
     if (lane == 0) out[i] = l;
   }
 }
@@ -83,10 +78,7 @@ __global__ void __launch_bounds__(kThreads) k2_full_warp(const __grid_constant__
   const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int64_t nwarp = ((int64_t)gridDim.x * blockDim.x) >> 5;
   for (int64_t i = warp0; i < N; i += nwarp) {
-    double x[NSS_NSLOT];
-#pragma unroll
-    for (int j = 0; j < NSS_NSLOT; ++j) x[j] = j < d ? theta[i * d + j] : 0.0;
-    const double l = nssk::loglike_warp<NDET>(P, nullptr, x);
+    const double l = nssk::loglike_warp<NDET, NSS_KIND_FULL>(P, nullptr, theta + i * d);
     if (lane == 0) out[i] = l;
   }
 }
@@ -96,10 +88,7 @@ __global__ void __launch_bounds__(kThreads) k_gauss(const __grid_constant__ NssD
 {
   const int d = P.d;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
-    double x[NSS_NSLOT];
-#pragma unroll
-    for (int j = 0; j < NSS_NSLOT; ++j) x[j] = j < d ? theta[i * d + j] : 0.0;
-    out[i] = nssk::gauss_loglike(P, x);
+    out[i] = nssk::gauss_loglike(P, theta + i * d);
   }
 }
 

@@ -1,7 +1,9 @@
 // nss_loglike_dev.cuh — device functions of the likelihood kernels (K1 relative binning, K2 full grid).
 //
-// Shared by the batch kernels (nss_loglike.cu) and the persistent slice-sampling kernel
-// (nss_sampler.cu), where one warp evaluates one point co-operatively.
+// Shared by the batch kernels (nss_loglike.cu) and the slice-sampling kernel (nss_sampler.cu), where one
+// warp evaluates one point co-operatively: the canonical parameter vector sits in a per-warp shared-memory
+// scratch, the transcendental part of the per-point setup is spread over lanes (same instruction, different
+// argument) and broadcast by shuffles, and lanes own contiguous slices of the bins.
 #pragma once
 #include "nss_internal.cuh"
 
@@ -49,20 +51,25 @@ __device__ __forceinline__ void stage_table(void *dst_smem, const void *src, uin
   }
 }
 
-// ---- per-point quantities -------------------------------------------------------------------------
-__device__ __forceinline__ void canon_from_sampled(const NssDev &P, const double *theta, double *th)
+__device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+
+__device__ __forceinline__ double warp_sum(double v)
 {
 #pragma unroll
-  for (int j = 0; j < NSS_NSLOT; ++j) th[j] = P.theta_fixed[j];
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;       // butterfly: every lane ends with the same bits
+}
+
+// ---- per-point quantities -------------------------------------------------------------------------
+// canonical vector from sampled coordinates held in memory (global or shared): slot t takes
+// theta[slot_src[t]] if sampled, else the fixed value.  All indices are uniform.
+__device__ __forceinline__ void canon_from_mem(const NssDev &P, const double *__restrict__ theta, double *th)
+{
 #pragma unroll
-  for (int j = 0; j < NSS_NSLOT; ++j)
-    if (j < P.d) {
-      const int s = P.param_index[j];
-      const double v = theta[j];
-#pragma unroll
-      for (int t = 0; t < NSS_NSLOT; ++t)
-        if (t == s) th[t] = v;
-    }
+  for (int t = 0; t < NSS_NSLOT; ++t) {
+    const int s = P.slot_src[t];
+    th[t] = s >= 0 ? theta[s] : P.theta_fixed[t];
+  }
 }
 
 // heterodyned point: phase difference to the fiducial (turns) and complex amplitude ratio per detector
@@ -75,15 +82,11 @@ struct RbPoint {
 };
 
 template <int NDET>
-__device__ __forceinline__ void rb_point(const NssDev &P, const double *th, RbPoint<NDET> &R)
+__device__ __forceinline__ void rb_finish_point(const NssDev &P, const nssp::Intrinsic &I, const nssp::Sky &S, RbPoint<NDET> &R)
 {
-  nssp::Intrinsic I;
-  nssp::intrinsic(th, I);
 #pragma unroll
   for (int j = 0; j < kNB; ++j) R.dc[j] = I.c[j] - P.c_fid[j];
   R.dconst = I.c_const - P.c_const_fid;
-  nssp::Sky S;
-  nssp::sky_frame(P.gmst, th[9], th[10], th[8], S);
   const double ci = I.cos_iota;
   const double pp = 0.5 * (1.0 + ci * ci) * I.amp, pc = -ci * I.amp;
 #pragma unroll
@@ -95,6 +98,56 @@ __device__ __forceinline__ void rb_point(const NssDev &P, const double *th, RbPo
     R.ai[a] = hr * P.inv_a0[a][1] + hi * P.inv_a0[a][0];
     R.ft[a] = (I.tc - P.tc_fid) + (tau - P.tau_fid[a]);
   }
+}
+
+// one thread does everything (batch kernel, one thread per point)
+template <int NDET>
+__device__ __forceinline__ void rb_point(const NssDev &P, const double *th, RbPoint<NDET> &R)
+{
+  nssp::Intrinsic I;
+  nssp::intrinsic(th, I);
+  nssp::Sky S;
+  nssp::sky_frame(P.gmst, th[9], th[10], th[8], S);
+  rb_finish_point<NDET>(P, I, S, R);
+}
+
+// One warp, same th[] in every lane.  The transcendental calls are spread over lanes and broadcast:
+//   sincos: lane 0 gmst - ra, 1 dec, 2 psi, 3 iota          (one call instead of four)
+//   log   : lane 0 pi G Mc / c^3, lane 1 eta                 (u = (pi M)^(1/3) via ln u = ln(.)/3 - ln(eta)/5)
+//   exp   : lane 0 u, lane 1 1/u, lane 2 (G Mc/c^3)^(5/6)
+// Every lane ends with identical bits (all inputs of the replicated arithmetic come from one lane).
+__device__ __forceinline__ void point_setup_warp(const NssDev &P, const double *th, nssp::Intrinsic &I, nssp::Sky &S)
+{
+  const int lane = threadIdx.x & 31;
+  const double q = th[1];
+  const double m1 = 1.0 / (1.0 + q), m2 = q * m1;
+  const double eta = q * m1 * m1;
+  // stage 1: four angles
+  const double ang = lane == 0 ? P.gmst - th[9] : lane == 1 ? th[10] : lane == 2 ? th[8] : th[7];
+  double sn, cs;
+  sincos(ang, &sn, &cs);
+  const double sg = shfl_d(sn, 0), cg = shfl_d(cs, 0), sd = shfl_d(sn, 1), cd = shfl_d(cs, 1), sp = shfl_d(sn, 2),
+               cp = shfl_d(cs, 2), ci = shfl_d(cs, 3);
+  nssp::sky_from_sincos(sg, cg, sd, cd, sp, cp, S);
+  // stage 2: two logarithms
+  const double mcs = th[0] * nssp::kGMsun;                       // G Mc / c^3 [s]
+  const double lg = log(lane == 0 ? nssp::kPi * mcs : eta);
+  const double ln_pimc = shfl_d(lg, 0), ln_eta = shfl_d(lg, 1);
+  const double lnu = ln_pimc * (1.0 / 3.0) - 0.2 * ln_eta;       // ln (pi M)^(1/3), M = Mc eta^(-3/5)
+  // stage 3: three exponentials
+  const double ln_mcs = ln_pimc - 1.1447298858494001741;         // ln(pi)
+  const double ex = exp(lane == 0 ? lnu : lane == 1 ? -lnu : (5.0 / 6.0) * ln_mcs);
+  const double u = shfl_d(ex, 0), iu = shfl_d(ex, 1), mc56 = shfl_d(ex, 2);
+  nssp::intrinsic_from(th, eta, m1, m2, u, iu, lnu, mc56, ci, I);
+}
+
+template <int NDET>
+__device__ __forceinline__ void rb_point_warp(const NssDev &P, const double *th, RbPoint<NDET> &R)
+{
+  nssp::Intrinsic I;
+  nssp::Sky S;
+  point_setup_warp(P, th, I, S);
+  rb_finish_point<NDET>(P, I, S, R);
 }
 
 // bin contribution from the waveform ratio at the bin's two edges (pre-scaled terms q[0..5], see nss_setup.cu)
@@ -146,40 +199,48 @@ __device__ __forceinline__ double rb_loglike_thread(const NssDev &P, const doubl
   return tot - P.half_DD;
 }
 
-__device__ __forceinline__ double warp_sum(double v)
-{
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-  return v;       // butterfly: every lane ends with the same bits
-}
+// ---- K1, one warp per point: lane l owns bins [l*m, l*m+m) and edges [l*m, l*m+m].
+// `tab` = warp layout (shared or global), edge-round major so every offset inside a round is an immediate:
+//   round 0 : [9][32]                      g0..g7, F of edge l*m
+//   round j : [9][32] then [NDET*6][32]    edge l*m+j, then the six pre-scaled terms of bin l*m+j-1, j = 1..m
+template <int NDET>
+__device__ __forceinline__ int rb_warp_table_doubles(int m) { return (9 + m * (9 + 6 * NDET)) * 32; }
 
-// ---- K1, one warp per point: lane l owns bins [l*m, l*m+m); `tab` = warp layout (shared or global)
 template <int NDET>
 __device__ __forceinline__ double rb_loglike_warp(const NssDev &P, const double *__restrict__ tab,
                                                   const RbPoint<NDET> &R)
 {
   const int lane = threadIdx.x & 31, m = P.rb_m;
-  const double *te = tab + lane;
-  const double *tb = tab + (size_t)9 * (m + 1) * 32 + lane;
+  const double *t = tab + lane;
   double pr[NDET], pi[NDET], acc[NDET];
-#pragma unroll
-  for (int a = 0; a < NDET; ++a) { pr[a] = 0.0; pi[a] = 0.0; acc[a] = 0.0; }
-  for (int j = 0; j <= m; ++j) {
+  {
     double ph = R.dconst;
 #pragma unroll
-    for (int c = 0; c < kNB; ++c) ph = fma(R.dc[c], te[((size_t)c * (m + 1) + j) * 32], ph);
-    const double F = te[((size_t)8 * (m + 1) + j) * 32];
+    for (int c = 0; c < kNB; ++c) ph = fma(R.dc[c], t[c * 32], ph);
+    const double F = t[8 * 32];
+#pragma unroll
+    for (int a = 0; a < NDET; ++a) {
+      double s, c;
+      nssp::sincos_turns(fma(F, R.ft[a], ph), &s, &c);
+      pr[a] = fma(R.ar[a], c, R.ai[a] * s);
+      pi[a] = fma(R.ai[a], c, -R.ar[a] * s);
+      acc[a] = 0.0;
+    }
+  }
+  t += 9 * 32;
+  for (int j = 1; j <= m; ++j, t += (9 + 6 * NDET) * 32) {
+    double ph = R.dconst;
+#pragma unroll
+    for (int c = 0; c < kNB; ++c) ph = fma(R.dc[c], t[c * 32], ph);
+    const double F = t[8 * 32];
 #pragma unroll
     for (int a = 0; a < NDET; ++a) {
       double s, c;
       nssp::sincos_turns(fma(F, R.ft[a], ph), &s, &c);
       const double rr = fma(R.ar[a], c, R.ai[a] * s);
       const double ri = fma(R.ai[a], c, -R.ar[a] * s);
-      if (j > 0) {
-        const double *q = tb + ((size_t)(a * 6) * m + (j - 1)) * 32;
-        const size_t st = (size_t)m * 32;
-        acc[a] += bin_term(q[0], q[st], q[2 * st], q[3 * st], q[4 * st], q[5 * st], pr[a], pi[a], rr, ri);
-      }
+      const double *q = t + (9 + 6 * a) * 32;
+      acc[a] += bin_term(q[0], q[32], q[64], q[96], q[128], q[160], pr[a], pi[a], rr, ri);
       pr[a] = rr; pi[a] = ri;
     }
   }
@@ -194,9 +255,8 @@ template <int NDET>
 __device__ __forceinline__ double full_loglike_warp(const NssDev &P, const double *th)
 {
   nssp::Intrinsic I;
-  nssp::intrinsic(th, I);
   nssp::Sky S;
-  nssp::sky_frame(P.gmst, th[9], th[10], th[8], S);
+  point_setup_warp(P, th, I, S);
   const double ci = I.cos_iota;
   const double pp = 0.5 * (1.0 + ci * ci) * I.amp, pc = -ci * I.amp;
   double hr[NDET], hi[NDET], ft[NDET], acc[NDET];
@@ -232,33 +292,35 @@ __device__ __forceinline__ double full_loglike_warp(const NssDev &P, const doubl
   return -0.5 * warp_sum(tot);
 }
 
-// O16 Gaussian test likelihood on sampled coordinates
-__device__ __forceinline__ double gauss_loglike(const NssDev &P, const double *theta)
+// O16 Gaussian test likelihood on sampled coordinates (memory operand; uniform indices)
+__device__ __forceinline__ double gauss_loglike(const NssDev &P, const double *__restrict__ theta)
 {
   double s = 0.0;
   bool ok = true;
 #pragma unroll
   for (int j = 0; j < NSS_NSLOT; ++j)
     if (j < P.d) {
-      ok = ok && isfinite(theta[j]);
-      const double z = (theta[j] - P.gauss_mu[j]) * P.gauss_isig[j];
+      const double x = theta[j];
+      ok = ok && isfinite(x);
+      const double z = (x - P.gauss_mu[j]) * P.gauss_isig[j];
       s = fma(z, z, s);
     }
   return ok ? -0.5 * s : -INFINITY;
 }
 
-// One warp evaluates logL of sampled coordinates theta (identical in all lanes); every lane returns
-// the same bits.  `tab` = warp-layout RB table (shared or global), ignored for other kinds.
-template <int NDET>
-__device__ __forceinline__ double loglike_warp(const NssDev &P, const double *__restrict__ tab, const double *theta)
+// One warp evaluates logL of the sampled coordinates `theta` (memory the whole warp can read: global or the
+// warp's shared scratch); every lane returns the same bits.  `tab` = warp-layout RB table (shared or
+// global), ignored for other kinds.
+template <int NDET, int KIND>
+__device__ __forceinline__ double loglike_warp(const NssDev &P, const double *__restrict__ tab, const double *__restrict__ theta)
 {
-  if (P.kind == NSS_KIND_GAUSS) return gauss_loglike(P, theta);
+  if (KIND == NSS_KIND_GAUSS) return gauss_loglike(P, theta);
   double th[NSS_NSLOT];
-  canon_from_sampled(P, theta, th);
+  canon_from_mem(P, theta, th);
   if (!nssp::domain_ok(th)) return -INFINITY;
-  if (P.kind == NSS_KIND_RB) {
+  if (KIND == NSS_KIND_RB) {
     RbPoint<NDET> R;
-    rb_point<NDET>(P, th, R);
+    rb_point_warp<NDET>(P, th, R);
     return rb_loglike_warp<NDET>(P, tab, R);
   }
   return full_loglike_warp<NDET>(P, th);

@@ -48,15 +48,11 @@ NSS_HD bool domain_ok(const double *th)
 }
 
 // O3: PN coefficients regrouped by power of f.  v = u f^(1/3), u = (pi M)^(1/3).
-NSS_HD void intrinsic(const double *th, Intrinsic &I)
+// Inputs: eta, m1 = m_1/M, m2 = m_2/M, u, iu = 1/u, lnu = ln u, mc56 = (G Mc/c^3)^(5/6), ci = cos(iota).
+NSS_HD void intrinsic_from(const double *th, double eta, double m1, double m2, double u, double iu, double lnu, double mc56,
+                           double ci, Intrinsic &I)
 {
-  const double Mc = th[0], q = th[1], chi1 = th[2], chi2 = th[3], dL = th[4];
-  const double opq = 1.0 + q;
-  const double m1 = 1.0 / opq, m2 = q * m1;
-  const double eta = q * m1 * m1;
-  const double M = Mc * pow(eta, -0.6) * kGMsun;
-  const double u = cbrt(kPi * M);
-  const double lnu = log(u);
+  const double chi1 = th[2], chi2 = th[3], dL = th[4];
   const double K = 3.0 / (128.0 * eta) / (2.0 * kPi);          // turns
   const double eta2 = eta * eta;
   const double beta = (113.0 / 12.0 * m1 * m1 + 6.25 * eta) * chi1 + (113.0 / 12.0 * m2 * m2 + 6.25 * eta) * chi2;
@@ -68,8 +64,8 @@ NSS_HD void intrinsic(const double *th, Intrinsic &I)
                   + eta * (-15737765635.0 / 3048192.0 + 2255.0 / 12.0 * kPi * kPi)
                   + 76055.0 / 1728.0 * eta2 - 127825.0 / 1296.0 * eta2 * eta;
   const double phi7 = kPi * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * eta2);
-  const double iu = 1.0 / u, iu2 = iu * iu;
-  const double ln_vlso = -0.5 * log(6.0);
+  const double iu2 = iu * iu;
+  const double ln_vlso = -0.89587973461402748;                  // -ln(6)/2
   const double ln4 = 1.3862943611198906188;
   I.c[0] = K * iu2 * iu2 * iu;                                  // f^-5/3
   I.c[1] = K * phi2 * iu2 * iu;                                 // f^-1
@@ -81,8 +77,19 @@ NSS_HD void intrinsic(const double *th, Intrinsic &I)
   I.c[7] = K * phi7 * u * u;                                    // f^2/3
   I.c_const = (-th[6] - 0.25 * kPi) / (2.0 * kPi) + K * P5 * (1.0 + 3.0 * (lnu - ln_vlso));
   I.tc = th[5];
-  I.amp = 0.45643546458763842789 /* sqrt(5/24) */ * pow(kPi, -2.0 / 3.0) * pow(Mc * kGMsun, 5.0 / 6.0) * kC / (dL * kMpc);
-  I.cos_iota = cos(th[7]);
+  I.amp = 0.45643546458763842789 /* sqrt(5/24) */ * 0.46619407703541166 /* pi^(-2/3) */ * mc56 * kC / (dL * kMpc);
+  I.cos_iota = ci;
+}
+
+// everything in one thread (host setup, one-thread-per-point kernel)
+NSS_HD void intrinsic(const double *th, Intrinsic &I)
+{
+  const double Mc = th[0], q = th[1];
+  const double m1 = 1.0 / (1.0 + q), m2 = q * m1;
+  const double eta = q * m1 * m1;
+  const double M = Mc * pow(eta, -0.6) * kGMsun;
+  const double u = cbrt(kPi * M);
+  intrinsic_from(th, eta, m1, m2, u, 1.0 / u, log(u), pow(Mc * kGMsun, 5.0 / 6.0), cos(th[7]), I);
 }
 
 // polarisation basis of O4 (independent of the detector)
@@ -90,12 +97,8 @@ struct Sky {
   double X[3], Y[3], n[3];
 };
 
-NSS_HD void sky_frame(double gmst, double ra, double dec, double psi, Sky &S)
+NSS_HD void sky_from_sincos(double sg, double cg, double sd, double cd, double sp, double cp, Sky &S)
 {
-  double sg, cg, sd, cd, sp, cp;
-  sincos(gmst - ra, &sg, &cg);
-  sincos(dec, &sd, &cd);
-  sincos(psi, &sp, &cp);
   S.X[0] = -cp * sg - sp * cg * sd;
   S.X[1] = -cp * cg + sp * sg * sd;
   S.X[2] = sp * cd;
@@ -105,6 +108,15 @@ NSS_HD void sky_frame(double gmst, double ra, double dec, double psi, Sky &S)
   S.n[0] = cd * cg;          // cos(ra - gmst) = cos g
   S.n[1] = -cd * sg;         // sin(ra - gmst) = -sin g
   S.n[2] = sd;
+}
+
+NSS_HD void sky_frame(double gmst, double ra, double dec, double psi, Sky &S)
+{
+  double sg, cg, sd, cd, sp, cp;
+  sincos(gmst - ra, &sg, &cg);
+  sincos(dec, &sd, &cd);
+  sincos(psi, &sp, &cp);
+  sky_from_sincos(sg, cg, sd, cd, sp, cp, S);
 }
 
 // D6 = symmetric detector tensor (xx, xy, xz, yy, yz, zz) of D = (x x^T - y y^T)/2; rc = vertex / c
@@ -139,10 +151,10 @@ NSS_HD void basis(double f, double *g)
 // sin / cos of an angle given in turns
 NSS_HD void sincos_turns(double t, double *s, double *c)
 {
-  const double fr = t - rint(t);
 #if defined(__CUDA_ARCH__)
-  sincospi(2.0 * fr, s, c);
+  sincospi(2.0 * t, s, c);                 // 2t is exact and sincospi reduces its argument exactly
 #else
+  const double fr = t - rint(t);
   sincos(2.0 * kPi * fr, s, c);
 #endif
 }

@@ -321,7 +321,19 @@ __global__ void k_gather_rows(const double *__restrict__ live, const double *__r
   for (int a = 0; a < d; ++a) out_theta[(size_t)j * d + a] = live[(size_t)slot * d + a];
 }
 
-// ---- K3: slice-sampling chains, one warp per chain (O12.4, O12.5) ------------------------------------------------
+// ---- K3: slice-sampling chains (O12.4, O12.5) -------------------------------------------------------------------
+// A chain is run by a GROUP of G warps (G = 1, 2, 4 or 8, chosen so the chains fill the GPU).  Every bracket
+// test is one likelihood evaluation by ONE warp; the G warps of a group evaluate, in the same round, the next
+// G tests of the sequential algorithm under the assumption that each of them fails — which is what they do
+// most of the time:
+//     [left end l, if the left side is still stepping out] [right end r, likewise]
+//     [shrinkage proposals t_kk, t_kk+1, ... from the bracket those two tests would leave]
+// The proposals that follow a rejection depend only on the rejected proposals (bracket <- t on the side of
+// sign(t)) and on counter-based Philox draws, never on logL, so they are known in advance.  After the round
+// every warp replays the sequential decisions on the shared results and discards whatever the sequential
+// algorithm would not have evaluated (shrinkage proposals speculated across an expansion; proposals after
+// the accepted one).  Decisions, positions and the evaluation count are those of the sequential oracle.
+// The chain position x and direction v are spread over lanes (lane j holds x_j, v_j).
 struct ChainArgs {
   double *live;                 // [n][d] in/out
   double *logL;                 // [n]    in/out
@@ -336,23 +348,35 @@ struct ChainArgs {
   unsigned long long *n_evals;
   int32_t *trace;               // optional [k][n_repeats][3]
   double *margin;               // optional [k]
+  int32_t G;                    // warps per chain
 };
 
-constexpr int kChainThreads = 128;      // 4 chains per CTA
+constexpr int kChainThreads = 256;      // 8 warps per CTA = 8/G chain groups
+constexpr int kChainWarps = kChainThreads / 32;
+constexpr int kDirChunk = 16;           // slice directions are drawn 16 steps at a time by the whole group
 
-template <int NDET, bool RESIDENT>
-__global__ void __launch_bounds__(kChainThreads) k3_slice(const __grid_constant__ NssDev P, const ChainArgs A)
+__device__ __forceinline__ void group_sync(int id, int nthreads)
+{
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+template <int NDET, int KIND, bool RESIDENT>
+__global__ void __launch_bounds__(kChainThreads, 2) k3_slice(const __grid_constant__ NssDev P, const ChainArgs A)
 {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ __align__(8) uint64_t bar;
   __shared__ double sL[NSS_NSLOT * NSS_NSLOT];
+  __shared__ double sZ[kChainWarps][kDirChunk][NSS_NSLOT + 1];     // normals of the current chunk, per group
+  __shared__ double sV[kChainWarps][kDirChunk][NSS_NSLOT];         // directions v = w L z/|z|
+  __shared__ double sY[kChainWarps][NSS_NSLOT + 1];                // per warp: sampled coordinates of its candidate
+  __shared__ double sRes[kChainWarps][2][kChainWarps];             // per group, double-buffered: logL of slot w
+  __shared__ int32_t sFlag[kChainWarps][2][kChainWarps];           // 1 = in the box (evaluated), 0 = outside the box
   if (A.flags[0] | A.flags[1]) return;
   const double *tab = P.rb_soa;
   if (RESIDENT) {
     if (threadIdx.x == 0) {
       nssk::mbar_init(&bar, 1);
-      const size_t bytes = (size_t)(9 * (P.rb_m + 1) + 6 * NDET * P.rb_m) * 32 * sizeof(double);
-      nssk::stage_table(smem_raw, P.rb_soa, (uint32_t)bytes, &bar);
+      nssk::stage_table(smem_raw, P.rb_soa, (uint32_t)(nssk::rb_warp_table_doubles<NDET>(P.rb_m) * sizeof(double)), &bar);
     }
   }
   const int d = P.d;
@@ -362,124 +386,198 @@ __global__ void __launch_bounds__(kChainThreads) k3_slice(const __grid_constant_
     nssk::mbar_wait(&bar, 0);
     tab = reinterpret_cast<const double *>(smem_raw);
   }
-  const int lane = threadIdx.x & 31;
-  const int c = blockIdx.x * (kChainThreads / 32) + (threadIdx.x >> 5);
-  if (c >= A.k) return;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int G = A.G, GL = G * 32;
+  const int gi = warp / G, w = warp - gi * G;            // group in the CTA, warp in the group
+  const int gl = w * 32 + lane;                          // lane in the group
+  const int bar_id = 1 + gi;
+  const int groups_per_cta = kChainWarps / G;
   const double Lstar = A.state[3];
-  const uint32_t chain = (uint32_t)c, it = A.iteration;
+  const uint32_t it = A.iteration;
   const int ns = A.n - A.k;
+  const bool own = lane < d;
+  const double lo_j = own ? P.lo[lane] : 0.0, hi_j = own ? P.hi[lane] : 0.0;
+  int par = 0;
+  const int nb = (d + 1) >> 1;
 
-  // a4: start from a uniformly chosen survivor
-  int si = (int)floor(uniform_a(A.seed, 0u, kStepStart, chain, it) * (double)ns);
-  si = si > ns - 1 ? ns - 1 : si;
-  const int slot = A.surv_idx[si];
-  double x[NSS_NSLOT], v[NSS_NSLOT], y[NSS_NSLOT];
-#pragma unroll
-  for (int j = 0; j < NSS_NSLOT; ++j) x[j] = j < d ? A.live[(size_t)slot * d + j] : 0.0;
-  double lx = A.logL[slot];
-  long long evals = 0;
-  double margin = INFINITY;
+  for (int c = blockIdx.x * groups_per_cta + gi; c < A.k; c += gridDim.x * groups_per_cta) {
+    const uint32_t chain = (uint32_t)c;
+    // a4: start from a uniformly chosen survivor
+    int si = (int)floor(uniform_a(A.seed, 0u, kStepStart, chain, it) * (double)ns);
+    si = si > ns - 1 ? ns - 1 : si;
+    const int slot = A.surv_idx[si];
+    double xj = own ? A.live[(size_t)slot * d + lane] : 0.0;
+    double lx = A.logL[slot];
+    long long evals = 0;
+    double margin = INFINITY;
 
-  // inside(t): box test (inclusive) first, then logL(x + t v) > L*
-  auto inside = [&](double t, double &ly) -> bool {
-    bool in = true;
-#pragma unroll
-    for (int j = 0; j < NSS_NSLOT; ++j)
-      if (j < d) {
-        y[j] = __dadd_rn(x[j], __dmul_rn(t, v[j]));
-        in = in && (y[j] >= P.lo[j]) && (y[j] <= P.hi[j]);
-      }
-    if (!in) return false;
-    ly = nssk::loglike_warp<NDET>(P, tab, y);
-    ++evals;
-    margin = fmin(margin, fabs(ly - Lstar));
-    return ly > Lstar;
-  };
-
-  for (int s = 0; s < A.n_repeats; ++s) {
-    // a5: direction n = z/|z|, v = w L n
-    double z[NSS_NSLOT + 1];
-    double nz = 0.0;
-#pragma unroll
-    for (int b = 0; b < (NSS_NSLOT + 1) / 2; ++b)
-      if (2 * b < d) {
+    for (int s0 = 0; s0 < A.n_repeats; s0 += kDirChunk) {
+      const int clen = min(kDirChunk, A.n_repeats - s0);
+      // a5: directions of steps s0 .. s0+clen-1.  Normals z (Box-Muller, one Philox block per pair) ...
+      group_sync(bar_id, GL);                            // the previous chunk's directions are no longer read
+      for (int idx = gl; idx < clen * nb; idx += GL) {
+        const int ss = idx / nb, b = idx - ss * nb;
         uint64_t ka, kb;
-        draw53(A.seed, (uint32_t)(1 + b), (uint32_t)s, chain, it, ka, kb);
+        draw53(A.seed, (uint32_t)(1 + b), (uint32_t)(s0 + ss), chain, it, ka, kb);
         const double r = sqrt(-2.0 * log((double)(ka + 1) * kTwoM53));
         double sn, cs;
         sincospi(2.0 * ((double)kb * kTwoM53), &sn, &cs);
-        z[2 * b] = r * cs;
-        z[2 * b + 1] = r * sn;
+        sZ[gi][ss][2 * b] = r * cs;
+        sZ[gi][ss][2 * b + 1] = r * sn;
       }
-#pragma unroll
-    for (int j = 0; j < NSS_NSLOT; ++j)
-      if (j < d) nz += z[j] * z[j];
-    nz = sqrt(nz);
-#pragma unroll
-    for (int i = 0; i < NSS_NSLOT; ++i)
-      if (i < d) {
+      group_sync(bar_id, GL);
+      // ... then n = z/|z|, v = w L n, one (step, row) pair per lane
+      for (int idx = gl; idx < clen * d; idx += GL) {
+        const int ss = idx / d, i = idx - ss * d;
+        const double *z = sZ[gi][ss];
+        double nz = 0.0;
+        for (int j = 0; j < d; ++j) nz += z[j] * z[j];
+        nz = sqrt(nz);
         double a = 0.0;
-#pragma unroll
-        for (int j = 0; j < NSS_NSLOT; ++j)
-          if (j <= i) a += sL[i * d + j] * (z[j] / nz);
-        v[i] = kSliceW * a;
+        for (int j = 0; j <= i; ++j) a += sL[i * d + j] * (z[j] / nz);
+        sV[gi][ss][i] = kSliceW * a;
       }
-    // a6: stepping out
-    const double u0 = uniform_a(A.seed, 0u, (uint32_t)s, chain, it);
-    double l = -u0, r = 1.0 - u0, ly = 0.0;
-    int nl = 0, nr = 0;
-    while (nl < kMaxExpand && inside(l, ly)) { l -= 1.0; ++nl; }
-    while (nr < kMaxExpand && inside(r, ly)) { r += 1.0; ++nr; }
-    // a7: shrinkage
-    int acc = -1;
-    for (int kk = 0; kk < kMaxShrink; ++kk) {
-      const double uk = uniform_a(A.seed, (uint32_t)(64 + kk), (uint32_t)s, chain, it);
-      const double t = __dadd_rn(l, __dmul_rn(r - l, uk));
-      if (inside(t, ly)) {
-#pragma unroll
-        for (int j = 0; j < NSS_NSLOT; ++j) x[j] = y[j];
-        lx = ly; acc = kk;
-        break;
+      group_sync(bar_id, GL);
+
+      for (int s = s0; s < s0 + clen; ++s) {
+        const double vj = own ? sV[gi][s - s0][lane] : 0.0;
+        // uniforms of this step: lane 0 -> bracket offset (block 0), lane 1+kk -> kk-th shrinkage proposal (block 64+kk)
+        const double ulane = uniform_a(A.seed, lane == 0 ? 0u : (uint32_t)(63 + lane), (uint32_t)s, chain, it);
+        const double u0 = nssk::shfl_d(ulane, 0);
+        double l = -u0, r = 1.0 - u0;
+        int nl = 0, nr = 0, kk = 0, acc = -1;
+        bool ldone = false, rdone = false, done = false;
+        while (!done) {
+          // ---- candidate of this warp ------------------------------------------------------------------------
+          const int nside = (ldone ? 0 : 1) + (rdone ? 0 : 1);
+          int nshr = G - nside;
+          nshr = nshr < kMaxShrink - kk ? nshr : kMaxShrink - kk;
+          double t = 0.0;
+          bool active = w < nside + nshr;
+          if (w < nside) {
+            t = (w == 0 && !ldone) ? l : r;
+          } else if (active) {
+            double ls = l, rs = r;
+            for (int i = 0; i <= w - nside; ++i) {
+              const int q = kk + i;
+              const double uk = q < 31 ? nssk::shfl_d(ulane, q + 1) : uniform_a(A.seed, (uint32_t)(64 + q), (uint32_t)s, chain, it);
+              t = __dadd_rn(ls, __dmul_rn(rs - ls, uk));
+              if (t < 0.0) ls = t; else rs = t;
+            }
+          }
+          // ---- evaluate: box test (inclusive) first, then logL(x + t v) ---------------------------------------
+          double ly = -INFINITY;
+          int inbox = 0;
+          if (active) {
+            const double yj = __dadd_rn(xj, __dmul_rn(t, vj));
+            inbox = __all_sync(0xffffffffu, !own || (yj >= lo_j && yj <= hi_j));
+            if (inbox) {
+              if (own) sY[warp][lane] = yj;
+              __syncwarp();
+              ly = nssk::loglike_warp<NDET, KIND>(P, tab, sY[warp]);
+              __syncwarp();
+            }
+          }
+          if (lane == 0) { sRes[gi][par][w] = ly; sFlag[gi][par][w] = inbox; }
+          group_sync(bar_id, GL);
+          const double *res = sRes[gi][par];
+          const int32_t *flg = sFlag[gi][par];
+          par ^= 1;
+          // ---- replay the sequential decisions ---------------------------------------------------------------
+          bool expanded = false;
+          int slot_i = 0;
+          if (!ldone) {
+            const double v = res[slot_i]; const int f = flg[slot_i]; ++slot_i;
+            if (f) { ++evals; margin = fmin(margin, fabs(v - Lstar)); }
+            if (f && v > Lstar) { l -= 1.0; ++nl; expanded = true; ldone = nl >= kMaxExpand; } else ldone = true;
+          }
+          if (!rdone) {
+            const double v = res[slot_i]; const int f = flg[slot_i]; ++slot_i;
+            if (f) { ++evals; margin = fmin(margin, fabs(v - Lstar)); }
+            if (f && v > Lstar) { r += 1.0; ++nr; expanded = true; rdone = nr >= kMaxExpand; } else rdone = true;
+          }
+          if (ldone && rdone && !expanded) {
+            for (int i = 0; i < nshr; ++i) {
+              const int q = kk + i;
+              const double uk = q < 31 ? nssk::shfl_d(ulane, q + 1) : uniform_a(A.seed, (uint32_t)(64 + q), (uint32_t)s, chain, it);
+              const double ti = __dadd_rn(l, __dmul_rn(r - l, uk));
+              const double v = res[slot_i + i]; const int f = flg[slot_i + i];
+              if (f) { ++evals; margin = fmin(margin, fabs(v - Lstar)); }
+              if (f && v > Lstar) {
+                xj = __dadd_rn(xj, __dmul_rn(ti, vj));
+                lx = v; acc = q; done = true;
+                break;
+              }
+              if (ti < 0.0) l = ti; else r = ti;
+            }
+            if (!done) { kk += nshr; done = kk >= kMaxShrink; }
+          }
+        }
+        if (A.trace && gl == 0) {
+          int32_t *tr = A.trace + ((size_t)c * A.n_repeats + s) * 3;
+          tr[0] = nl; tr[1] = nr; tr[2] = acc;
+        }
       }
-      if (t < 0.0) l = t; else r = t;
     }
-    if (A.trace && lane == 0) {
-      int32_t *tr = A.trace + ((size_t)c * A.n_repeats + s) * 3;
-      tr[0] = nl; tr[1] = nr; tr[2] = acc;
+    // a10: replace the deleted slot in place
+    if (w == 0) {
+      const int dst = A.dead_idx[c];
+      if (own) A.live[(size_t)dst * d + lane] = xj;
+      if (lane == 0) {
+        A.logL[dst] = lx;
+        if (A.birth) A.birth[dst] = Lstar;
+        if (A.margin) A.margin[c] = margin;
+        atomicAdd(A.n_evals, (unsigned long long)evals);
+      }
     }
-  }
-  // a10: replace the deleted slot in place
-  if (lane == 0) {
-    const int dst = A.dead_idx[c];
-    for (int j = 0; j < d; ++j) A.live[(size_t)dst * d + j] = x[j];
-    A.logL[dst] = lx;
-    if (A.birth) A.birth[dst] = Lstar;
-    if (A.margin) A.margin[c] = margin;
-    atomicAdd(A.n_evals, (unsigned long long)evals);
   }
 }
 
+template <int NDET, int KIND, bool RESIDENT>
+int launch_chains_k(nss_handle *h, ChainArgs &A, size_t smem, cudaStream_t st)
+{
+  auto kern = k3_slice<NDET, KIND, RESIDENT>;
+  if (smem > 48 * 1024) NSS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int occ = 0;
+  NSS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kChainThreads, smem));
+  if (occ < 1) occ = 1;
+  const int cap_warps = h->n_sm * occ * kChainWarps;
+  int G = h->chain_warps;
+  if (G != 1 && G != 2 && G != 4 && G != 8) {            // automatic: the widest group that keeps every chain resident
+    G = 8;
+    while (G > 1 && (long long)A.k * G > cap_warps) G >>= 1;
+  }
+  A.G = G;
+  const int gpc = kChainWarps / G;
+  int grid = (A.k + gpc - 1) / gpc;
+  if (grid > h->n_sm * occ) grid = h->n_sm * occ;
+  NSS_CUDA(cudaEventRecord(h->ev_k3[0], st));
+  kern<<<grid, kChainThreads, smem, st>>>(h->dev, A);
+  NSS_CUDA(cudaEventRecord(h->ev_k3[1], st));
+  return NSS_OK;
+}
+
 template <int NDET>
-int launch_chains(nss_handle *h, const ChainArgs &A, cudaStream_t st)
+int launch_chains(nss_handle *h, ChainArgs &A, cudaStream_t st)
 {
   const NssDev &P = h->dev;
-  const int grid = (A.k + kChainThreads / 32 - 1) / (kChainThreads / 32);
-  size_t bytes = 0;
-  if (P.kind == NSS_KIND_RB) bytes = (size_t)(9 * (P.rb_m + 1) + 6 * NDET * P.rb_m) * 32 * sizeof(double);
-  const bool resident = P.kind == NSS_KIND_RB && bytes + 2048 <= 200 * 1024;
   if (!h->ev_k3[0]) {
     NSS_CUDA(cudaEventCreate(&h->ev_k3[0]));
     NSS_CUDA(cudaEventCreate(&h->ev_k3[1]));
   }
-  NSS_CUDA(cudaEventRecord(h->ev_k3[0], st));
-  if (resident) {
-    if (bytes > 48 * 1024)
-      NSS_CUDA(cudaFuncSetAttribute(k3_slice<NDET, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
-    k3_slice<NDET, true><<<grid, kChainThreads, bytes, st>>>(P, A);
+  int rc;
+  if (P.kind == NSS_KIND_RB) {
+    const size_t bytes = (size_t)(9 + P.rb_m * (9 + 6 * NDET)) * 32 * sizeof(double);
+    if (bytes + 40 * 1024 <= 110 * 1024)                 // table + static arrays, two CTAs per SM
+      rc = launch_chains_k<NDET, NSS_KIND_RB, true>(h, A, bytes, st);
+    else
+      rc = launch_chains_k<NDET, NSS_KIND_RB, false>(h, A, 0, st);
+  } else if (P.kind == NSS_KIND_FULL) {
+    rc = launch_chains_k<NDET, NSS_KIND_FULL, false>(h, A, 0, st);
   } else {
-    k3_slice<NDET, false><<<grid, kChainThreads, 0, st>>>(P, A);
+    rc = launch_chains_k<1, NSS_KIND_GAUSS, false>(h, A, 0, st);
   }
-  NSS_CUDA(cudaEventRecord(h->ev_k3[1], st));
+  if (rc) return rc;
   h->ev_k3_valid = 1;
   h->launches += 1;
   NSS_CUDA(cudaGetLastError());
@@ -522,6 +620,7 @@ int enqueue_iteration(nss_handle *h, double *live, double *logL, double *birth, 
   A.live = live; A.logL = logL; A.birth = birth; A.n = n; A.k = k; A.n_repeats = n_repeats; A.seed = seed;
   A.iteration = iteration; A.surv_idx = h->d_surv_idx; A.dead_idx = dead_idx; A.chol = h->d_chol; A.state = h->d_state;
   A.flags = h->d_flags; A.n_evals = h->d_nevals; A.trace = h->trace_dev; A.margin = h->margin_dev;
+  A.G = 1;
   switch (h->dev.n_det) {
     case 0: case 1: return launch_chains<1>(h, A, st);
     case 2: return launch_chains<2>(h, A, st);
@@ -539,6 +638,13 @@ extern "C" int nss_last_chain_ms(nss_handle *h, double *ms_host)
   float ms = 0.f;
   NSS_CUDA(cudaEventElapsedTime(&ms, h->ev_k3[0], h->ev_k3[1]));
   *ms_host = ms;
+  return NSS_OK;
+}
+
+extern "C" int nss_set_chain_warps(nss_handle *h, int32_t warps)
+{
+  if (!h || !(warps == 0 || warps == 1 || warps == 2 || warps == 4 || warps == 8)) return NSS_EINVAL;
+  h->chain_warps = warps;
   return NSS_OK;
 }
 

@@ -198,8 +198,10 @@ extern "C" int nss_create(const nss_config *cfg, nss_handle **out)
   P.d = cfg->d; P.kind = kind; P.n_det = kind == NSS_KIND_GAUSS ? 0 : cfg->n_det;
   P.n_freq = kind == NSS_KIND_GAUSS ? 0 : cfg->n_freq;
   P.gmst = cfg->gmst;
+  for (int j = 0; j < NSS_NSLOT; ++j) P.slot_src[j] = -1;
   for (int j = 0; j < NSS_NSLOT; ++j) {
     P.param_index[j] = j < cfg->d ? (kind == NSS_KIND_GAUSS ? j : cfg->param_index[j]) : 0;
+    if (j < cfg->d) P.slot_src[P.param_index[j]] = j;
     P.theta_fixed[j] = cfg->theta_fixed[j];
     P.lo[j] = j < cfg->d ? cfg->lo[j] : 0.0;
     P.hi[j] = j < cfg->d ? cfg->hi[j] : 0.0;
@@ -298,27 +300,27 @@ extern "C" int nss_create(const nss_config *cfg, nss_handle **out)
     P.rb_rs = rs;
     rc_up = upload(rec, &h->d_rb_rec, &h->rb_rec_bytes);
     P.rb_rec = h->d_rb_rec;
-    // (2) warp layout: lane l owns bins [l*m, l*m+m) and edges [l*m, l*m+m]
+    // (2) warp layout, edge-round major: lane l owns bins [l*m, l*m+m) and edges [l*m, l*m+m]
+    //     round 0: [9][32] (g0..g7, F of edge l*m); round j = 1..m: [9][32] of edge l*m+j, then [nd*6][32] of bin l*m+j-1
     const int m = (B + 31) / 32;
     P.rb_m = m;
-    std::vector<double> soa((size_t)(9 * (m + 1) + 6 * nd * m) * 32, 0.0);
-    double *te = soa.data(), *tb = soa.data() + (size_t)9 * (m + 1) * 32;
+    const size_t round_sz = (size_t)(9 + 6 * nd) * 32;
+    std::vector<double> soa((size_t)9 * 32 + (size_t)m * round_sz, 0.0);
     for (int l = 0; l < 32; ++l) {
       for (int j = 0; j <= m; ++j) {
+        double *te = j == 0 ? soa.data() : soa.data() + 9 * 32 + (size_t)(j - 1) * round_sz;
         int e = l * m + j;
         if (e > B) e = B;
         double g[nssp::kNB];
         nssp::basis(f[h->edge_idx[e]], g);
-        for (int c = 0; c < 8; ++c) te[((size_t)c * (m + 1) + j) * 32 + l] = g[c];
-        te[((size_t)8 * (m + 1) + j) * 32 + l] = f[h->edge_idx[e]];
-      }
-      for (int j = 0; j < m; ++j) {
-        const int b = l * m + j;
-        if (b >= B) continue;
+        for (int c = 0; c < 8; ++c) te[c * 32 + l] = g[c];
+        te[8 * 32 + l] = f[h->edge_idx[e]];
+        const int b = l * m + j - 1;
+        if (j == 0 || b >= B) continue;
         for (int a = 0; a < nd; ++a) {
           double q[6];
           scaled(a, b, q);
-          for (int c = 0; c < 6; ++c) tb[((size_t)(a * 6 + c) * m + j) * 32 + l] = q[c];
+          for (int c = 0; c < 6; ++c) te[(9 + a * 6 + c) * 32 + l] = q[c];
         }
       }
     }

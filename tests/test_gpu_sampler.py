@@ -284,3 +284,37 @@ def test_iterate_device_and_host_forms_match_oracle(nssmod, oracle, wl1):
     g.nss_loglike_batch_host(X, out)
     assert torch.equal(out, g.nss_loglike_batch(X.cuda()).cpu())
     g.close()
+
+
+@pytest.mark.parametrize("cfg", ["gauss", "config1", "config2"])
+def test_chain_group_width_does_not_change_the_trajectory(nssmod, oracle, wl1, wl2, cfg):
+    """K3 runs a chain on G = 1, 2, 4 or 8 warps that evaluate the next G bracket tests speculatively; the
+    decisions, positions, logL and the sequential-algorithm evaluation count must be the same bits for
+    every G (G = 1 is the plain sequential algorithm)."""
+    if cfg == "gauss":
+        w, n, k, nrep = inputs.gaussian_workload(6, sigma=0.05), 300, 150, 20
+    elif cfg == "config1":
+        w, n, k, nrep = wl1, 100, 50, 12
+    else:
+        w, n, k, nrep = wl2, 400, 200, 18            # 18 repeats: crosses the 16-step direction chunk
+    g, p = nssmod.Nss(w), oracle.Problem(w)
+    live, logL = p.init_live(n, 11)
+    if cfg != "gauss":                                # a compressed population: brackets expand and shrink a lot
+        for it in range(4):
+            o = p.replace_step(live, logL, k, 3, 11, it)
+            live, logL = o["live"], o["logL"]
+    ref = None
+    for G in (1, 2, 4, 8, 0):
+        g.set_chain_warps(G)
+        r = g.nss_replace_step(live, logL, k, nrep, 11, 9, want_trace=True)
+        cur = (r["live"].cpu().numpy(), r["logL"].cpu().numpy(), r["trace"].cpu().numpy(), r["margin"].cpu().numpy(),
+               r["n_evals"])
+        if ref is None:
+            ref = cur
+            assert ref[2][:, :, 0].max() > 0 or ref[2][:, :, 1].max() > 0      # some brackets did step out
+            assert ref[2][:, :, 2].max() >= 4                                    # and some shrank several times
+        else:
+            for a, b in zip(ref[:4], cur[:4]):
+                assert np.array_equal(a, b), f"G={G} changed the result"
+            assert ref[4] == cur[4]
+    g.close()

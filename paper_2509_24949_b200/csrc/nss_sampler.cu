@@ -449,7 +449,8 @@ __global__ void __launch_bounds__(kChainThreads, 2) k3_slice(const __grid_consta
         bool ldone = false, rdone = false, done = false;
         while (!done) {
           // ---- candidate of this warp ------------------------------------------------------------------------
-          const int nside = (ldone ? 0 : 1) + (rdone ? 0 : 1);
+          int nside = (ldone ? 0 : 1) + (rdone ? 0 : 1);
+          nside = nside < G ? nside : G;                 // G = 1: one side test per round, left first
           int nshr = G - nside;
           nshr = nshr < kMaxShrink - kk ? nshr : kMaxShrink - kk;
           double t = 0.0;
@@ -491,7 +492,7 @@ __global__ void __launch_bounds__(kChainThreads, 2) k3_slice(const __grid_consta
             if (f) { ++evals; margin = fmin(margin, fabs(v - Lstar)); }
             if (f && v > Lstar) { l -= 1.0; ++nl; expanded = true; ldone = nl >= kMaxExpand; } else ldone = true;
           }
-          if (!rdone) {
+          if (!rdone && slot_i < nside) {
             const double v = res[slot_i]; const int f = flg[slot_i]; ++slot_i;
             if (f) { ++evals; margin = fmin(margin, fabs(v - Lstar)); }
             if (f && v > Lstar) { r += 1.0; ++nr; expanded = true; rdone = nr >= kMaxExpand; } else rdone = true;
@@ -537,7 +538,7 @@ template <int NDET, int KIND, bool RESIDENT>
 int launch_chains_k(nss_handle *h, ChainArgs &A, size_t smem, cudaStream_t st)
 {
   auto kern = k3_slice<NDET, KIND, RESIDENT>;
-  if (smem > 48 * 1024) NSS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  if (smem > 0) NSS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));   // static + dynamic may exceed 48 KB
   int occ = 0;
   NSS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kChainThreads, smem));
   if (occ < 1) occ = 1;

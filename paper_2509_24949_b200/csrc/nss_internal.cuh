@@ -33,6 +33,13 @@ struct NssDev {
   int32_t full_rs;
 };
 
+// device control block of an NS iteration; one pinned host mirror per handle (a single small D2H copy per sync)
+struct NssCtl {
+  double state[4];             // logX, logZ, logZ_live, Lstar
+  unsigned long long nevals;
+  int32_t flags[4];            // [0] Cholesky error, [1] threshold violation, [2] stop rule reached
+};
+
 struct nss_handle {
   NssDev dev;
   int device;
@@ -52,6 +59,7 @@ struct nss_handle {
   int32_t *d_surv_idx, *d_dead_idx, *d_rank, *d_flags;   // flags: [0] chol error, [1] threshold violation, [2] done
   double *d_mean, *d_chol, *d_state;                      // state: logX, logZ, logZ_live, Lstar
   unsigned long long *d_nevals;
+  NssCtl *d_ctl, *h_ctl;       // d_state, d_nevals, d_flags point into d_ctl; h_ctl is pinned
   double *d_birth;
   int32_t *trace_dev;
   double *margin_dev;

@@ -173,29 +173,49 @@ __device__ __forceinline__ double block_sum(double v, double *red)
   return s;
 }
 
+// Column sums and the d(d+1)/2 centred products are split over row groups (thread = (row group, column) or
+// (row group, pair)); the groups are then added in a fixed order, so the result is deterministic.
 __global__ void __launch_bounds__(kOneCta) k4_tune(const double *__restrict__ live, int n, int d, double *__restrict__ mean_out,
                                                    double *__restrict__ chol_out, int32_t *__restrict__ flags)
 {
-  __shared__ double red[32];
+  __shared__ double part[kOneCta];
   __shared__ double mean[NSS_NSLOT];
   __shared__ double cov[NSS_NSLOT * NSS_NSLOT];
   const int tid = threadIdx.x;
-  for (int j = 0; j < d; ++j) {
+  {
+    const int ng = kOneCta / d, j = tid % d, g = tid / d;
     double s = 0.0;
-    for (int i = tid; i < n; i += kOneCta) s += live[(size_t)i * d + j];
-    s = block_sum(s, red);
-    if (tid == 0) mean[j] = s / n;
-  }
-  __syncthreads();
-  for (int a = 0; a < d; ++a)
-    for (int b = 0; b <= a; ++b) {
-      double s = 0.0;
-      const double ma = mean[a], mb = mean[b];
-      for (int i = tid; i < n; i += kOneCta) s = fma(live[(size_t)i * d + a] - ma, live[(size_t)i * d + b] - mb, s);
-      s = block_sum(s, red);
-      if (tid == 0) { cov[a * d + b] = s / (n - 1); cov[b * d + a] = s / (n - 1); }
+    if (g < ng)
+      for (int i = g; i < n; i += ng) s += live[(size_t)i * d + j];
+    part[tid] = s;
+    __syncthreads();
+    if (tid < d) {
+      double t = 0.0;
+      for (int q = 0; q < ng; ++q) t += part[q * d + tid];
+      mean[tid] = t / n;
     }
-  __syncthreads();
+    __syncthreads();
+  }
+  {
+    const int np = d * (d + 1) / 2, ng = kOneCta / np, p = tid % np, g = tid / np;
+    int a = 0, rem = p;                       // pair index p -> (a, b), b <= a, row-major lower triangle
+    while (rem > a) { rem -= a + 1; ++a; }
+    const int b = rem;
+    double s = 0.0;
+    if (g < ng) {
+      const double ma = mean[a], mb = mean[b];
+      for (int i = g; i < n; i += ng) s = fma(live[(size_t)i * d + a] - ma, live[(size_t)i * d + b] - mb, s);
+    }
+    part[tid] = s;
+    __syncthreads();
+    if (tid < np) {
+      double t = 0.0;
+      for (int q = 0; q < ng; ++q) t += part[q * np + tid];
+      cov[a * d + b] = t / (n - 1);
+      cov[b * d + a] = t / (n - 1);
+    }
+    __syncthreads();
+  }
   if (tid == 0) {
     double L[NSS_NSLOT * NSS_NSLOT];
     for (int a = 0; a < d * d; ++a) L[a] = 0.0;
@@ -307,6 +327,12 @@ __global__ void __launch_bounds__(kOneCta) k4_live_evidence(const double *__rest
     state[2] = lzl;
     if (check && (lzl - state[1] < stop_dlogz)) flags[2] = 1;
   }
+}
+
+__global__ void k_fill(double *__restrict__ p, int n, double v)
+{
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) p[i] = v;
 }
 
 __global__ void k_gather_rows(const double *__restrict__ live, const double *__restrict__ logL, const double *__restrict__ birth,
@@ -585,6 +611,32 @@ int launch_chains(nss_handle *h, ChainArgs &A, cudaStream_t st)
   return NSS_OK;
 }
 
+// start of an iteration: clear the flags (and the evaluation counter), optionally load logX / logZ
+__global__ void k_begin(NssCtl *ctl, int set_state, double logX, double logZ, int zero_evals)
+{
+  if (threadIdx.x < 4) ctl->flags[threadIdx.x] = 0;
+  if (threadIdx.x == 0) {
+    if (set_state) { ctl->state[0] = logX; ctl->state[1] = logZ; ctl->state[2] = 0.0; ctl->state[3] = 0.0; }
+    if (zero_evals) ctl->nevals = 0ull;
+  }
+}
+
+int begin_iteration(nss_handle *h, int set_state, double logX, double logZ, int zero_evals, cudaStream_t st)
+{
+  k_begin<<<1, 32, 0, st>>>(h->d_ctl, set_state, logX, logZ, zero_evals);
+  h->launches += 1;
+  NSS_CUDA(cudaGetLastError());
+  return NSS_OK;
+}
+
+// one 56-byte copy of the control block into the pinned mirror, then wait for the stream
+int fetch_ctl(nss_handle *h, cudaStream_t st)
+{
+  NSS_CUDA(cudaMemcpyAsync(h->h_ctl, h->d_ctl, sizeof(NssCtl), cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaStreamSynchronize(st));
+  return NSS_OK;
+}
+
 int ensure_scratch(nss_handle *h, int n)
 {
   if (h->scratch_n >= n && h->d_flags) return NSS_OK;
@@ -595,11 +647,13 @@ int ensure_scratch(nss_handle *h, int n)
   NSS_CUDA(cudaMalloc(&h->d_rank, sizeof(int32_t) * n));
   NSS_CUDA(cudaMalloc(&h->d_birth, sizeof(double) * n));
   if (!h->d_flags) {
-    NSS_CUDA(cudaMalloc(&h->d_flags, sizeof(int32_t) * 4));
+    NSS_CUDA(cudaMalloc(&h->d_ctl, sizeof(NssCtl)));
+    NSS_CUDA(cudaMallocHost(&h->h_ctl, sizeof(NssCtl)));
     NSS_CUDA(cudaMalloc(&h->d_mean, sizeof(double) * NSS_NSLOT));
     NSS_CUDA(cudaMalloc(&h->d_chol, sizeof(double) * NSS_NSLOT * NSS_NSLOT));
-    NSS_CUDA(cudaMalloc(&h->d_state, sizeof(double) * 4));
-    NSS_CUDA(cudaMalloc(&h->d_nevals, sizeof(unsigned long long)));
+    h->d_state = h->d_ctl->state;             // addresses inside the device block (not dereferenced on the host)
+    h->d_nevals = &h->d_ctl->nevals;
+    h->d_flags = h->d_ctl->flags;
   }
   h->scratch_n = n;
   return NSS_OK;
@@ -688,16 +742,16 @@ extern "C" int nss_select_lowest(nss_handle *h, const double *logL_dev, int32_t 
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int rc = ensure_scratch(h, n_live);
   if (rc) return rc;
-  NSS_CUDA(cudaMemsetAsync(h->d_flags, 0, sizeof(int32_t) * 4, st));
+  rc = begin_iteration(h, 0, 0.0, 0.0, 0, st);
+  if (rc) return rc;
   k4_rank<<<(n_live + kRankThreads - 1) / kRankThreads, kRankThreads, 0, st>>>(logL_dev, n_live, n_delete, h->d_rank, dead_idx_dev);
   k4_finish_select<<<1, kOneCta, 0, st>>>(nullptr, logL_dev, nullptr, n_live, n_delete, h->dev.d, NAN, h->d_rank, dead_idx_dev,
                                           surv_idx_dev, nullptr, nullptr, nullptr, h->d_state, h->d_flags);
   h->launches += 2;
   NSS_CUDA(cudaGetLastError());
-  double state[4];
-  NSS_CUDA(cudaMemcpyAsync(state, h->d_state, sizeof(state), cudaMemcpyDeviceToHost, st));
-  NSS_CUDA(cudaStreamSynchronize(st));
-  if (logLstar_host) *logLstar_host = state[3];
+  rc = fetch_ctl(h, st);
+  if (rc) return rc;
+  if (logLstar_host) *logLstar_host = h->h_ctl->state[3];
   return NSS_OK;
 }
 
@@ -708,14 +762,14 @@ extern "C" int nss_tune(nss_handle *h, const double *live_dev, int32_t n_live, d
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int rc = ensure_scratch(h, n_live);
   if (rc) return rc;
-  NSS_CUDA(cudaMemsetAsync(h->d_flags, 0, sizeof(int32_t) * 4, st));
+  rc = begin_iteration(h, 0, 0.0, 0.0, 0, st);
+  if (rc) return rc;
   k4_tune<<<1, kOneCta, 0, st>>>(live_dev, n_live, h->dev.d, mean_dev, chol_dev, h->d_flags);
   h->launches += 1;
   NSS_CUDA(cudaGetLastError());
-  int32_t flags[4];
-  NSS_CUDA(cudaMemcpyAsync(flags, h->d_flags, sizeof(flags), cudaMemcpyDeviceToHost, st));
-  NSS_CUDA(cudaStreamSynchronize(st));
-  return flags[0] ? NSS_ECHOL : NSS_OK;
+  rc = fetch_ctl(h, st);
+  if (rc) return rc;
+  return h->h_ctl->flags[0] ? NSS_ECHOL : NSS_OK;
 }
 
 extern "C" int nss_evidence_update(nss_handle *h, const double *dead_logL_dev, int32_t n_live, int32_t n_delete, double *logw_dev,
@@ -726,15 +780,15 @@ extern "C" int nss_evidence_update(nss_handle *h, const double *dead_logL_dev, i
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int rc = ensure_scratch(h, n_live);
   if (rc) return rc;
-  double state[4] = {state_host[0], state_host[1], 0.0, 0.0};
-  NSS_CUDA(cudaMemcpyAsync(h->d_state, state, sizeof(state), cudaMemcpyHostToDevice, st));
+  rc = begin_iteration(h, 1, state_host[0], state_host[1], 0, st);
+  if (rc) return rc;
   k4_evidence<<<1, kOneCta, 0, st>>>(dead_logL_dev, n_live, n_delete, logw_dev, h->d_state);
   h->launches += 1;
   NSS_CUDA(cudaGetLastError());
-  NSS_CUDA(cudaMemcpyAsync(state, h->d_state, sizeof(state), cudaMemcpyDeviceToHost, st));
-  NSS_CUDA(cudaStreamSynchronize(st));
-  state_host[0] = state[0];
-  state_host[1] = state[1];
+  rc = fetch_ctl(h, st);
+  if (rc) return rc;
+  state_host[0] = h->h_ctl->state[0];
+  state_host[1] = h->h_ctl->state[1];
   return NSS_OK;
 }
 
@@ -748,22 +802,17 @@ extern "C" int nss_replace_step(nss_handle *h, double *live_dev, double *logL_de
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int rc = ensure_scratch(h, n_live);
   if (rc) return rc;
-  NSS_CUDA(cudaMemsetAsync(h->d_flags, 0, sizeof(int32_t) * 4, st));
-  NSS_CUDA(cudaMemsetAsync(h->d_nevals, 0, sizeof(unsigned long long), st));
+  rc = begin_iteration(h, 0, 0.0, 0.0, 1, st);
+  if (rc) return rc;
   rc = enqueue_iteration(h, live_dev, logL_dev, nullptr, n_live, n_delete, logLstar, n_repeats, seed, iteration, dead_theta_dev,
                          dead_logL_dev, nullptr, dead_idx_dev, st);
   if (rc) return rc;
-  int32_t flags[4];
-  double state[4];
-  unsigned long long ne = 0;
-  NSS_CUDA(cudaMemcpyAsync(flags, h->d_flags, sizeof(flags), cudaMemcpyDeviceToHost, st));
-  NSS_CUDA(cudaMemcpyAsync(state, h->d_state, sizeof(state), cudaMemcpyDeviceToHost, st));
-  NSS_CUDA(cudaMemcpyAsync(&ne, h->d_nevals, sizeof(ne), cudaMemcpyDeviceToHost, st));
-  NSS_CUDA(cudaStreamSynchronize(st));
-  if (logLstar_host) *logLstar_host = state[3];
-  if (n_evals_host) *n_evals_host = (int64_t)ne;
-  if (flags[1]) return NSS_EINVAL;
-  if (flags[0]) return NSS_ECHOL;
+  rc = fetch_ctl(h, st);
+  if (rc) return rc;
+  if (logLstar_host) *logLstar_host = h->h_ctl->state[3];
+  if (n_evals_host) *n_evals_host = (int64_t)h->h_ctl->nevals;
+  if (h->h_ctl->flags[1]) return NSS_EINVAL;
+  if (h->h_ctl->flags[0]) return NSS_ECHOL;
   return NSS_OK;
 }
 
@@ -792,10 +841,8 @@ extern "C" int nss_iterate(nss_handle *h, double *live_dev, double *logL_dev, in
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int rc = ensure_scratch(h, n_live);
   if (rc) return rc;
-  double state[4] = {state_host->logX, state_host->logZ, 0.0, 0.0};
-  NSS_CUDA(cudaMemcpyAsync(h->d_state, state, sizeof(state), cudaMemcpyHostToDevice, st));
-  NSS_CUDA(cudaMemsetAsync(h->d_flags, 0, sizeof(int32_t) * 4, st));
-  NSS_CUDA(cudaMemsetAsync(h->d_nevals, 0, sizeof(unsigned long long), st));
+  rc = begin_iteration(h, 1, state_host->logX, state_host->logZ, 1, st);
+  if (rc) return rc;
   rc = enqueue_iteration(h, live_dev, logL_dev, nullptr, n_live, n_delete, NAN, n_repeats, seed, iteration, dead_theta_dev,
                          dead_logL_dev, nullptr, dead_idx_dev, st);
   if (rc) return rc;
@@ -803,16 +850,13 @@ extern "C" int nss_iterate(nss_handle *h, double *live_dev, double *logL_dev, in
   k4_live_evidence<<<1, kOneCta, 0, st>>>(logL_dev, n_live, stop_dlogz, 1, h->d_state, h->d_flags);
   h->launches += 2;
   NSS_CUDA(cudaGetLastError());
-  int32_t flags[4];
-  unsigned long long ne = 0;
-  NSS_CUDA(cudaMemcpyAsync(flags, h->d_flags, sizeof(flags), cudaMemcpyDeviceToHost, st));
-  NSS_CUDA(cudaMemcpyAsync(state, h->d_state, sizeof(state), cudaMemcpyDeviceToHost, st));
-  NSS_CUDA(cudaMemcpyAsync(&ne, h->d_nevals, sizeof(ne), cudaMemcpyDeviceToHost, st));
-  NSS_CUDA(cudaStreamSynchronize(st));
-  if (flags[0]) return NSS_ECHOL;
-  state_host->logX = state[0]; state_host->logZ = state[1]; state_host->logZ_live = state[2]; state_host->logLstar = state[3];
-  state_host->n_evals = (int64_t)ne;
-  state_host->converged = flags[2];
+  rc = fetch_ctl(h, st);
+  if (rc) return rc;
+  const NssCtl &c = *h->h_ctl;
+  if (c.flags[0]) return NSS_ECHOL;
+  state_host->logX = c.state[0]; state_host->logZ = c.state[1]; state_host->logZ_live = c.state[2]; state_host->logLstar = c.state[3];
+  state_host->n_evals = (int64_t)c.nevals;
+  state_host->converged = c.flags[2];
   return NSS_OK;
 }
 
@@ -883,11 +927,9 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
   if (rc) return rc;
   const int64_t cap = out->cap;
   double *live = nullptr, *logL = nullptr, *dth = nullptr, *dl = nullptr, *db = nullptr, *dw = nullptr;
-  int32_t *h_flags = nullptr;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   auto cleanup = [&]() {
     cudaFree(live); cudaFree(logL); cudaFree(dth); cudaFree(dl); cudaFree(db); cudaFree(dw);
-    if (h_flags) cudaFreeHost(h_flags);
     if (e0) cudaEventDestroy(e0);
     if (e1) cudaEventDestroy(e1);
   };
@@ -902,32 +944,26 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
   RUN_CUDA(cudaMalloc(&dl, sizeof(double) * cap));
   RUN_CUDA(cudaMalloc(&db, sizeof(double) * cap));
   RUN_CUDA(cudaMalloc(&dw, sizeof(double) * cap));
-  RUN_CUDA(cudaMallocHost(&h_flags, sizeof(int32_t) * 4));
   RUN_CUDA(cudaEventCreate(&e0));
   RUN_CUDA(cudaEventCreate(&e1));
 
   RUN_CUDA(cudaEventRecord(e0, st));
-  const double state0[4] = {0.0, -INFINITY, 0.0, 0.0};
-  RUN_CUDA(cudaMemcpyAsync(h->d_state, state0, sizeof(state0), cudaMemcpyHostToDevice, st));
-  RUN_CUDA(cudaMemsetAsync(h->d_flags, 0, sizeof(int32_t) * 4, st));
-  RUN_CUDA(cudaMemsetAsync(h->d_nevals, 0, sizeof(unsigned long long), st));
+  rc = begin_iteration(h, 1, 0.0, -INFINITY, 1, st);
+  if (rc) { cleanup(); return rc; }
   rc = nss_init_live(h, n, seed, live, logL, st);
   if (rc) { cleanup(); return rc; }
-  {
-    std::vector<double> ninf(n, -INFINITY);
-    RUN_CUDA(cudaMemcpyAsync(h->d_birth, ninf.data(), sizeof(double) * n, cudaMemcpyHostToDevice, st));
-    RUN_CUDA(cudaStreamSynchronize(st));
-  }
+  k_fill<<<(n + 255) / 256, 256, 0, st>>>(h->d_birth, n, -INFINITY);
+  h->launches += 1;
   int t = 0;
   int64_t n_dead = 0;
   int result = NSS_OK;
   for (;;) {
     k4_live_evidence<<<1, kOneCta, 0, st>>>(logL, n, stop_dlogz, t > 0, h->d_state, h->d_flags);
     h->launches += 1;
-    RUN_CUDA(cudaMemcpyAsync(h_flags, h->d_flags, sizeof(int32_t) * 4, cudaMemcpyDeviceToHost, st));
+    RUN_CUDA(cudaMemcpyAsync(h->h_ctl, h->d_ctl, sizeof(NssCtl), cudaMemcpyDeviceToHost, st));
     RUN_CUDA(cudaStreamSynchronize(st));
-    if (h_flags[0]) { result = NSS_ECHOL; break; }
-    if (h_flags[2]) break;
+    if (h->h_ctl->flags[0]) { result = NSS_ECHOL; break; }
+    if (h->h_ctl->flags[2]) break;
     if (t >= max_iter) { result = NSS_ENOTCONV; break; }
     if (n_dead + k + n > cap) { result = NSS_ECAP; break; }
     rc = enqueue_iteration(h, live, logL, h->d_birth, n, k, NAN, n_repeats, seed, (uint32_t)t, dth + (size_t)n_dead * d, dl + n_dead,

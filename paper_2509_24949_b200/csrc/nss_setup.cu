@@ -146,8 +146,9 @@ extern "C" int nss_destroy(nss_handle *h)
   if (!h) return NSS_OK;
   cudaSetDevice(h->device);
   cudaFree(h->d_rb_rec); cudaFree(h->d_rb_soa); cudaFree(h->d_full_rec);
-  cudaFree(h->d_surv_idx); cudaFree(h->d_dead_idx); cudaFree(h->d_rank); cudaFree(h->d_flags);
-  cudaFree(h->d_mean); cudaFree(h->d_chol); cudaFree(h->d_state); cudaFree(h->d_nevals); cudaFree(h->d_birth); cudaFree(h->d_stage);
+  cudaFree(h->d_surv_idx); cudaFree(h->d_dead_idx); cudaFree(h->d_rank); cudaFree(h->d_ctl);
+  if (h->h_ctl) cudaFreeHost(h->h_ctl);
+  cudaFree(h->d_mean); cudaFree(h->d_chol); cudaFree(h->d_birth); cudaFree(h->d_stage);
   if (h->ev_k3[0]) cudaEventDestroy(h->ev_k3[0]);
   if (h->ev_k3[1]) cudaEventDestroy(h->ev_k3[1]);
   delete h;

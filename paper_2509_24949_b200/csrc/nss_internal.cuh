@@ -19,18 +19,20 @@ struct NssDev {
   double D6[NSS_MAXDET][6];   // symmetric detector tensors (O4)
   double rc[NSS_MAXDET][3];   // vertex / c [s]
   double gmst;
-  // heterodyne reference (kind 0)
+  // heterodyne reference (kind 0); for the full grid (kind 1) the reference is the identity:
+  // c_fid = c_const_fid = tc_fid = tau_fid = 0, inv_a0 = (1, 0)
   double c_fid[nssp::kNB], c_const_fid, tc_fid;
   double inv_a0[NSS_MAXDET][2];   // 1 / (complex amplitude of the fiducial waveform per detector)
   double tau_fid[NSS_MAXDET];
   double half_DD;                 // 1/2 sum_det <d,d>
-  // tables (device pointers owned by the handle)
-  const double *rb_rec;   // AoS  [E][rb_rs]: g0..g7, F_e, pad, then per det 6 pre-scaled bin terms of bin e-1
-  int32_t rb_rs;
-  const double *rb_soa;   // warp layout, edge-round major: [9][32], then m x ([9][32] edge, [n_det*6][32] bin terms)
-  int32_t rb_m;           // bins per lane = ceil(B/32)
-  const double *full_rec; // AoS [n_freq][full_rs]: g0..g7, f, f^-7/6, then per det (d_re, d_im, 4df/S), pad
-  int32_t full_rs;
+  double hh0[NSS_MAXDET];         // <h,h> = |A|^2 (hh0 + sum_b V_b X_b)   (nss_setup.cu: "record tables")
+  // record tables (device pointers owned by the handle); a record is a bin edge (kind 0) or a grid frequency (kind 1)
+  int32_t n_rec;
+  int32_t cross;          // 1: records carry the cross-term weight V (kind 0), 0: they do not (kind 1)
+  const double *rec;      // AoS [n_rec][rec_rs]: g0..g7, f, pad, then per det (Wr, Wi[, V])
+  int32_t rec_rs;
+  const double *soa;      // warp layout, round major: [9 + 2 n_det][32], then m x [9 + (2 + cross) n_det][32]
+  int32_t soa_m;          // rounds after round 0 = ceil((n_rec - 1)/32); lane l owns records l*m+1 .. l*m+m
 };
 
 // device control block of an NS iteration; one pinned host mirror per handle (a single small D2H copy per sync)
@@ -52,8 +54,8 @@ struct nss_handle {
   std::vector<double> summary;     // [n_det][B][6]
   double DD;
   // device allocations
-  double *d_rb_rec, *d_rb_soa, *d_full_rec;
-  size_t rb_rec_bytes, rb_soa_bytes, full_rec_bytes;
+  double *d_rec, *d_soa;
+  size_t rec_bytes, soa_bytes;
   // sampler scratch (grown on demand)
   int32_t scratch_n;
   int32_t *d_surv_idx, *d_dead_idx, *d_rank, *d_flags;   // flags: [0] chol error, [1] threshold violation, [2] done

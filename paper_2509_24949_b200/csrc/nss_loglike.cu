@@ -1,11 +1,14 @@
 // nss_loglike.cu — batch likelihood kernels behind nss_loglike_batch.
 //
-//  k1_rb_thread : relative binning, ONE THREAD per point.  The AoS edge/bin table is staged into shared
-//                 memory by TMA bulk copies (when it fits) and read by broadcast; a persistent grid-stride
-//                 loop over points.  Highest throughput for large N (no per-point redundancy, no shuffles).
-//  k1_rb_warp   : relative binning, ONE WARP per point (lanes own contiguous bin slices, warp-shuffle
-//                 reduction).  For small N, and the form the slice sampler uses.
-//  k2_full_warp : full frequency grid, one warp per point, 128-bit coalesced loads of data/PSD records.
+// Relative binning (K1) and the full frequency grid (K2) are the same computation over a table of records —
+// bin edges with cross-term weights, or grid frequencies without (nss_setup.cu "record tables") — so each
+// mapping is one kernel template instantiated for both:
+//  k_rec_thread : ONE THREAD per point.  The AoS record table is staged into shared memory by TMA bulk
+//                 copies and read by broadcast: whole when it fits (relative binning: one load per CTA, then a
+//                 persistent grid-stride loop over points), else streamed in double-buffered tiles, one batch of
+//                 blockDim points per pass (full grid: 4017 records).  Highest throughput for large N.
+//  k_rec_warp   : ONE WARP per point (lanes own contiguous record slices, per-point setup spread over lanes,
+//                 warp-shuffle reduction).  For small N, and the form the slice sampler inlines.
 //  k_gauss      : O16 test likelihood.
 #include "nss_loglike_dev.cuh"
 
@@ -14,71 +17,113 @@ namespace {
 constexpr int kThreads = 256;
 constexpr size_t kSmemMax = 227 * 1024;
 
-template <int NDET, bool RESIDENT>
-__global__ void __launch_bounds__(kThreads) k1_rb_thread(const __grid_constant__ NssDev P, const double *__restrict__ theta,
-                                                         int64_t N, double *__restrict__ out)
+template <int NDET, bool CROSS>
+__device__ __forceinline__ void zero_acc(nssk::DetAcc *A)
+{
+#pragma unroll
+  for (int a = 0; a < NDET; ++a) { A[a].tr = 0.0; A[a].ti = 0.0; A[a].q = 0.0; A[a].pc = 0.0; A[a].ps = 0.0; }
+}
+
+// tile_recs records per tile, n_tiles tiles (n_tiles == 1: the table is resident)
+template <int NDET, bool CROSS, bool STREAM>
+__global__ void __launch_bounds__(kThreads) k_rec_thread(const __grid_constant__ NssDev P, const double *__restrict__ theta,
+                                                         int64_t N, double *__restrict__ out, int tile_recs, int n_tiles)
 {
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  __shared__ __align__(8) uint64_t bar;
-  const double *rec = P.rb_rec;
-  if (RESIDENT) {
-    if (threadIdx.x == 0) {
-      nssk::mbar_init(&bar, 1);
-      nssk::stage_table(smem_raw, P.rb_rec, (uint32_t)((size_t)P.n_edges * P.rb_rs * sizeof(double)), &bar);
-    }
-    __syncthreads();
-    nssk::mbar_wait(&bar, 0);
-    rec = reinterpret_cast<const double *>(smem_raw);
+  __shared__ __align__(8) uint64_t bar[2];
+  const int d = P.d, rs = P.rec_rs, n_rec = P.n_rec;
+  const uint32_t tile_bytes = (uint32_t)tile_recs * rs * sizeof(double);
+  if (threadIdx.x == 0) {
+    nssk::mbar_init(&bar[0], 1);
+    nssk::mbar_init(&bar[1], 1);
   }
-  const int d = P.d;
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
-    double th[NSS_NSLOT];
-    nssk::canon_from_mem(P, theta + i * d, th);
-    double l = -INFINITY;
-    if (nssp::domain_ok(th)) {
-      nssk::RbPoint<NDET> R;
-      nssk::rb_point<NDET>(P, th, R);
-      l = nssk::rb_loglike_thread<NDET>(P, rec, R);
+  __syncthreads();
+  if (!STREAM) {
+    if (threadIdx.x == 0) nssk::stage_table(smem_raw, P.rec, (uint32_t)n_rec * rs * sizeof(double), &bar[0]);
+    nssk::mbar_wait(&bar[0], 0);
+    const double *rec = reinterpret_cast<const double *>(smem_raw);
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
+      double th[NSS_NSLOT];
+      nssk::canon_from_mem(P, theta + i * d, th);
+      double l = -INFINITY;
+      if (nssp::domain_ok(th)) {
+        nssk::RbPoint<NDET> R;
+        nssk::rb_point<NDET>(P, th, R);
+        nssk::DetAcc A[NDET];
+        zero_acc<NDET, CROSS>(A);
+        nssk::records_thread<NDET, CROSS>(rec, rs, n_rec, R, A);
+        l = nssk::finish_logl<NDET, false>(P, R, A);
+      }
+      out[i] = l;
     }
-    out[i] = l;
+    return;
+  }
+  // streaming: the sequence (batch, tile) is flattened; tile `seq + 1` is in flight while `seq` is consumed
+  const int64_t n_batch = (N + blockDim.x - 1) / blockDim.x;
+  const int64_t my_batches = blockIdx.x < n_batch ? (n_batch - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+  const int64_t total = my_batches * n_tiles;
+  auto issue = [&](int64_t seq) {
+    const int t = (int)(seq % n_tiles);
+    const int cnt = min(tile_recs, n_rec - t * tile_recs);
+    nssk::stage_table(smem_raw + (size_t)(seq & 1) * tile_bytes, P.rec + (size_t)t * tile_recs * rs,
+                      (uint32_t)cnt * rs * sizeof(double), &bar[seq & 1]);
+  };
+  if (threadIdx.x == 0 && total > 0) issue(0);
+  nssk::RbPoint<NDET> R;
+  nssk::DetAcc A[NDET];
+  bool ok = false;
+  int64_t i = 0;
+  for (int64_t seq = 0; seq < total; ++seq) {
+    if (threadIdx.x == 0 && seq + 1 < total) issue(seq + 1);      // its buffer was released by the barrier below
+    const int t = (int)(seq % n_tiles);
+    if (t == 0) {
+      i = ((int64_t)blockIdx.x + (seq / n_tiles) * gridDim.x) * blockDim.x + threadIdx.x;
+      ok = false;
+      if (i < N) {
+        double th[NSS_NSLOT];
+        nssk::canon_from_mem(P, theta + i * d, th);
+        ok = nssp::domain_ok(th);
+        if (ok) nssk::rb_point<NDET>(P, th, R);
+      }
+      zero_acc<NDET, CROSS>(A);
+    }
+    nssk::mbar_wait(&bar[seq & 1], (uint32_t)((seq >> 1) & 1));
+    if (ok) {
+      const double *rec = reinterpret_cast<const double *>(smem_raw + (size_t)(seq & 1) * tile_bytes);
+      nssk::records_thread<NDET, CROSS>(rec, rs, min(tile_recs, n_rec - t * tile_recs), R, A);
+    }
+    if (t == n_tiles - 1 && i < N) out[i] = ok ? nssk::finish_logl<NDET, false>(P, R, A) : -INFINITY;
+    __syncthreads();
   }
 }
 
-template <int NDET, bool RESIDENT>
-__global__ void __launch_bounds__(kThreads) k1_rb_warp(const __grid_constant__ NssDev P, const double *__restrict__ theta,
+template <int NDET, int KIND, bool RESIDENT>
+__global__ void __launch_bounds__(kThreads) k_rec_warp(const __grid_constant__ NssDev P, const double *__restrict__ theta,
                                                        int64_t N, double *__restrict__ out)
 {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ __align__(8) uint64_t bar;
-  const double *tab = P.rb_soa;
+  __shared__ __align__(16) double consts[nssk::kWarpConstDoubles];
+  __shared__ __align__(16) double scratch[kThreads / 32][nssk::kWarpScratchDoubles];
+  nssk::WarpCtx X;
+  X.tab = P.soa;
+  X.consts = consts;
+  X.scr = scratch[threadIdx.x >> 5];
+  if (RESIDENT && threadIdx.x == 0) {
+    nssk::mbar_init(&bar, 1);
+    nssk::stage_table(smem_raw, P.soa, (uint32_t)(nssk::warp_table_doubles<NDET, KIND == NSS_KIND_RB>(P.soa_m) * sizeof(double)), &bar);
+  }
+  nssk::warp_consts_init(P, consts);
+  __syncthreads();
   if (RESIDENT) {
-    if (threadIdx.x == 0) {
-      nssk::mbar_init(&bar, 1);
-      const size_t bytes = (size_t)(9 * (P.rb_m + 1) + 6 * NDET * P.rb_m) * 32 * sizeof(double);
-      nssk::stage_table(smem_raw, P.rb_soa, (uint32_t)bytes, &bar);
-    }
-    __syncthreads();
     nssk::mbar_wait(&bar, 0);
-    tab = reinterpret_cast<const double *>(smem_raw);
+    X.tab = reinterpret_cast<const double *>(smem_raw);
   }
   const int d = P.d, lane = threadIdx.x & 31;
   const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int64_t nwarp = ((int64_t)gridDim.x * blockDim.x) >> 5;
   for (int64_t i = warp0; i < N; i += nwarp) {
-    const double l = nssk::loglike_warp<NDET, NSS_KIND_RB>(P, tab, theta + i * d);
-    if (lane == 0) out[i] = l;
-  }
-}
-
-template <int NDET>
-__global__ void __launch_bounds__(kThreads) k2_full_warp(const __grid_constant__ NssDev P, const double *__restrict__ theta,
-                                                         int64_t N, double *__restrict__ out)
-{
-  const int d = P.d, lane = threadIdx.x & 31;
-  const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  const int64_t nwarp = ((int64_t)gridDim.x * blockDim.x) >> 5;
-  for (int64_t i = warp0; i < N; i += nwarp) {
-    const double l = nssk::loglike_warp<NDET, NSS_KIND_FULL>(P, nullptr, theta + i * d);
+    const double l = nssk::loglike_warp<NDET, KIND>(P, X, theta + i * d);
     if (lane == 0) out[i] = l;
   }
 }
@@ -99,56 +144,65 @@ int set_smem(K kernel, size_t bytes)
   return NSS_OK;
 }
 
-template <int NDET>
-int launch_rb(nss_handle *h, const double *theta, int64_t N, double *logL, cudaStream_t st)
+template <int NDET, int KIND>
+int launch_rec(nss_handle *h, const double *theta, int64_t N, double *logL, cudaStream_t st)
 {
+  constexpr bool CROSS = KIND == NSS_KIND_RB;
   const NssDev &P = h->dev;
   int variant = h->loglike_variant;
   if (variant == 0) variant = N >= (int64_t)h->n_sm * 512 ? 1 : 2;
   if (variant == 1) {
-    const size_t bytes = (size_t)P.n_edges * P.rb_rs * sizeof(double);
-    const bool resident = bytes + 1024 <= kSmemMax;
-    const size_t smem = resident ? bytes : 0;
-    int per_sm = resident ? (int)(kSmemMax / (bytes + 1024)) : 4;
+    const size_t rec_bytes = (size_t)P.rec_rs * sizeof(double), bytes = (size_t)P.n_rec * rec_bytes;
+    int tile_recs = P.n_rec, n_tiles = 1;
+    size_t smem = bytes;
+    if (bytes > 96 * 1024) {                        // stream: two 16 KB tiles keep several CTAs per SM
+      tile_recs = (int)(16 * 1024 / rec_bytes);
+      n_tiles = (P.n_rec + tile_recs - 1) / tile_recs;
+      smem = 2 * (size_t)tile_recs * rec_bytes;
+    }
+    int per_sm = (int)(kSmemMax / (smem + 1024));
     per_sm = per_sm > 3 ? 3 : per_sm;
-    int64_t want = (N + kThreads - 1) / kThreads;
+    const int64_t want = (N + kThreads - 1) / kThreads;
     const int64_t cap = (int64_t)h->n_sm * per_sm;
     const int grid = (int)(want < cap ? want : cap);
-    if (resident) {
-      int rc = set_smem(k1_rb_thread<NDET, true>, smem);
+    if (n_tiles == 1) {
+      int rc = set_smem(k_rec_thread<NDET, CROSS, false>, smem);
       if (rc) return rc;
-      k1_rb_thread<NDET, true><<<grid, kThreads, smem, st>>>(P, theta, N, logL);
+      k_rec_thread<NDET, CROSS, false><<<grid, kThreads, smem, st>>>(P, theta, N, logL, tile_recs, n_tiles);
     } else {
-      k1_rb_thread<NDET, false><<<grid, kThreads, 0, st>>>(P, theta, N, logL);
+      int rc = set_smem(k_rec_thread<NDET, CROSS, true>, smem);
+      if (rc) return rc;
+      k_rec_thread<NDET, CROSS, true><<<grid, kThreads, smem, st>>>(P, theta, N, logL, tile_recs, n_tiles);
     }
   } else {
-    const size_t bytes = (size_t)(9 * (P.rb_m + 1) + 6 * NDET * P.rb_m) * 32 * sizeof(double);
-    const bool resident = bytes + 1024 <= 200 * 1024;
+    const size_t bytes = (size_t)((9 + 2 * NDET) + P.soa_m * (9 + (CROSS ? 3 : 2) * NDET)) * 32 * sizeof(double);
+    const bool resident = bytes + 8 * 1024 <= 200 * 1024;
     const size_t smem = resident ? bytes : 0;
-    int per_sm = resident ? (int)(kSmemMax / (bytes + 1024)) : 8;
+    int per_sm = resident ? (int)(kSmemMax / (bytes + 8 * 1024)) : 8;
     per_sm = per_sm > 8 ? 8 : per_sm;
-    int64_t want = (N * 32 + kThreads - 1) / kThreads;
+    const int64_t want = (N * 32 + kThreads - 1) / kThreads;
     const int64_t cap = (int64_t)h->n_sm * per_sm;
     const int grid = (int)(want < cap ? want : cap);
     if (resident) {
-      int rc = set_smem(k1_rb_warp<NDET, true>, smem);
+      int rc = set_smem(k_rec_warp<NDET, KIND, true>, smem);
       if (rc) return rc;
-      k1_rb_warp<NDET, true><<<grid, kThreads, smem, st>>>(P, theta, N, logL);
+      k_rec_warp<NDET, KIND, true><<<grid, kThreads, smem, st>>>(P, theta, N, logL);
     } else {
-      k1_rb_warp<NDET, false><<<grid, kThreads, 0, st>>>(P, theta, N, logL);
+      k_rec_warp<NDET, KIND, false><<<grid, kThreads, 0, st>>>(P, theta, N, logL);
     }
   }
   return NSS_OK;
 }
 
-template <int NDET>
-int launch_full(nss_handle *h, const double *theta, int64_t N, double *logL, cudaStream_t st)
+template <int KIND>
+int launch_kind(nss_handle *h, const double *theta, int64_t N, double *logL, cudaStream_t st)
 {
-  int64_t want = (N * 32 + kThreads - 1) / kThreads;
-  const int64_t cap = (int64_t)h->n_sm * 8;
-  const int grid = (int)(want < cap ? want : cap);
-  k2_full_warp<NDET><<<grid, kThreads, 0, st>>>(h->dev, theta, N, logL);
-  return NSS_OK;
+  switch (h->dev.n_det) {
+    case 1: return launch_rec<1, KIND>(h, theta, N, logL, st);
+    case 2: return launch_rec<2, KIND>(h, theta, N, logL, st);
+    case 3: return launch_rec<3, KIND>(h, theta, N, logL, st);
+    default: return launch_rec<4, KIND>(h, theta, N, logL, st);
+  }
 }
 
 }  // namespace
@@ -162,19 +216,9 @@ int nss_launch_loglike(nss_handle *h, const double *theta, int64_t N, double *lo
     const int64_t cap = (int64_t)h->n_sm * 8;
     k_gauss<<<(int)(want < cap ? want : cap), kThreads, 0, st>>>(P, theta, N, logL);
   } else if (P.kind == NSS_KIND_RB) {
-    switch (P.n_det) {
-      case 1: rc = launch_rb<1>(h, theta, N, logL, st); break;
-      case 2: rc = launch_rb<2>(h, theta, N, logL, st); break;
-      case 3: rc = launch_rb<3>(h, theta, N, logL, st); break;
-      default: rc = launch_rb<4>(h, theta, N, logL, st); break;
-    }
+    rc = launch_kind<NSS_KIND_RB>(h, theta, N, logL, st);
   } else {
-    switch (P.n_det) {
-      case 1: rc = launch_full<1>(h, theta, N, logL, st); break;
-      case 2: rc = launch_full<2>(h, theta, N, logL, st); break;
-      case 3: rc = launch_full<3>(h, theta, N, logL, st); break;
-      default: rc = launch_full<4>(h, theta, N, logL, st); break;
-    }
+    rc = launch_kind<NSS_KIND_FULL>(h, theta, N, logL, st);
   }
   if (rc) return rc;
   h->launches += 1;

@@ -1,9 +1,9 @@
 // nss_loglike_dev.cuh — device functions of the likelihood kernels (K1 relative binning, K2 full grid).
 //
 // Shared by the batch kernels (nss_loglike.cu) and the slice-sampling kernel (nss_sampler.cu), where one
-// warp evaluates one point co-operatively: the canonical parameter vector sits in a per-warp shared-memory
-// scratch, the transcendental part of the per-point setup is spread over lanes (same instruction, different
-// argument) and broadcast by shuffles, and lanes own contiguous slices of the bins.
+// warp evaluates one point co-operatively: the per-point setup is spread over lanes (same instruction stream,
+// different argument or coefficient per lane) and broadcast through a per-warp shared-memory scratch, and
+// lanes own contiguous slices of the records (bin edges or grid frequencies).
 #pragma once
 #include "nss_internal.cuh"
 
@@ -72,18 +72,24 @@ __device__ __forceinline__ void canon_from_mem(const NssDev &P, const double *__
   }
 }
 
-// heterodyned point: phase difference to the fiducial (turns) and complex amplitude ratio per detector
+// A point relative to the reference (nss_setup.cu "record tables"): phase difference in turns
+// phi(f) = dconst + sum_j dc_j g_j(f) + f ft_det, and the complex amplitude ratio A/A0 per detector.
 template <int NDET>
 struct RbPoint {
   double dc[kNB];
   double dconst;
-  double ft[NDET];            // coefficient of F_e: (tc + tau_det) - (tc_fid + tau_fid_det)
+  double ft[NDET];            // coefficient of f: (tc + tau_det) - (tc_fid + tau_fid_det)
   double ar[NDET], ai[NDET];  // amplitude ratio
 };
 
+// one thread does everything (batch kernel, one thread per point)
 template <int NDET>
-__device__ __forceinline__ void rb_finish_point(const NssDev &P, const nssp::Intrinsic &I, const nssp::Sky &S, RbPoint<NDET> &R)
+__device__ __forceinline__ void rb_point(const NssDev &P, const double *th, RbPoint<NDET> &R)
 {
+  nssp::Intrinsic I;
+  nssp::intrinsic(th, I);
+  nssp::Sky S;
+  nssp::sky_frame(P.gmst, th[9], th[10], th[8], S);
 #pragma unroll
   for (int j = 0; j < kNB; ++j) R.dc[j] = I.c[j] - P.c_fid[j];
   R.dconst = I.c_const - P.c_const_fid;
@@ -100,83 +106,187 @@ __device__ __forceinline__ void rb_finish_point(const NssDev &P, const nssp::Int
   }
 }
 
-// one thread does everything (batch kernel, one thread per point)
-template <int NDET>
-__device__ __forceinline__ void rb_point(const NssDev &P, const double *th, RbPoint<NDET> &R)
+// ---- one warp per point: the per-point setup is spread over lanes ---------------------------------------
+// Per-CTA constants in shared memory (filled once per kernel by warp_consts_init):
+//   coef[k][16], k = 0..8 : lane j < 8 builds phase coefficient j as  K A_j(eta, beta, ln u) exp(p_j ln u) - c_fid_j,
+//                           A_j = t0 + t1 eta + t2 eta^2 + t3 eta^3 + t4 beta + t5 ln u;  rows: t0..t5, p, q, c_fid.
+//                           Lane 8 builds (G Mc/c^3)^(5/6) = exp(q_8 ln(G Mc/c^3)) (t0 = 1, no K).
+//   det[12][4]            : per detector D6[0..5], rc[0..2], inv_a0 re, im, tau_fid
+// Per-warp scratch (40 doubles): two broadcast rounds through shared memory.
+constexpr int kWarpConstDoubles = 9 * 16 + 12 * 4;
+constexpr int kWarpScratchDoubles = 40;
+
+struct WarpCtx {
+  const double *tab;      // warp-layout record table (shared or global)
+  const double *consts;   // kWarpConstDoubles, shared
+  double *scr;            // kWarpScratchDoubles, shared, private to the warp
+};
+
+__device__ __forceinline__ void warp_consts_init(const NssDev &P, double *consts)
 {
-  nssp::Intrinsic I;
-  nssp::intrinsic(th, I);
-  nssp::Sky S;
-  nssp::sky_frame(P.gmst, th[9], th[10], th[8], S);
-  rb_finish_point<NDET>(P, I, S, R);
+  const double pi = nssp::kPi;
+  for (int i = threadIdx.x; i < kWarpConstDoubles; i += blockDim.x) {
+    double v = 0.0;
+    if (i < 9 * 16) {
+      const int k = i >> 4, j = i & 15;
+      // rows t0..t5 of A_j (O3 regrouped by power of f, nss_physics.cuh: intrinsic_from)
+      if (k == 0)
+        v = j == 0 ? 1.0 : j == 1 ? 3715.0 / 756.0 : j == 2 ? -16.0 * pi : j == 3 ? 15293365.0 / 508032.0
+          : j == 4 ? pi * (38645.0 / 756.0)
+          : j == 5 ? 11583231236531.0 / 4694215680.0 - 640.0 / 3.0 * pi * pi - 6848.0 / 21.0 * nssp::kEuler
+                       - 6848.0 / 21.0 * 1.3862943611198906188
+          : j == 6 ? -6848.0 / 63.0 : j == 7 ? pi * (77096675.0 / 254016.0) : j == 8 ? 1.0 : 0.0;
+      else if (k == 1)
+        v = j == 1 ? 55.0 / 9.0 : j == 3 ? 27145.0 / 504.0 : j == 4 ? -pi * (65.0 / 9.0)
+          : j == 5 ? -15737765635.0 / 3048192.0 + 2255.0 / 12.0 * pi * pi : j == 7 ? pi * (378515.0 / 1512.0) : 0.0;
+      else if (k == 2)
+        v = j == 3 ? 3085.0 / 72.0 : j == 5 ? 76055.0 / 1728.0 : j == 7 ? -pi * (74045.0 / 756.0) : 0.0;
+      else if (k == 3)
+        v = j == 5 ? -127825.0 / 1296.0 : 0.0;
+      else if (k == 4)
+        v = j == 2 ? 4.0 : 0.0;
+      else if (k == 5)
+        v = j == 5 ? -6848.0 / 21.0 : 0.0;
+      else if (k == 6)         // power of u = (pi M)^(1/3)
+        v = j == 0 ? -5.0 : j == 1 ? -3.0 : j == 2 ? -2.0 : j == 3 ? -1.0 : j == 5 ? 1.0 : j == 6 ? 1.0 : j == 7 ? 2.0 : 0.0;
+      else if (k == 7)         // power of G Mc / c^3
+        v = j == 8 ? 5.0 / 6.0 : 0.0;
+      else
+        v = j < kNB ? P.c_fid[j] : 0.0;
+    } else {
+      const int k = (i - 9 * 16) >> 2, a = (i - 9 * 16) & 3;
+      v = k < 6 ? P.D6[a][k] : k < 9 ? P.rc[a][k - 6] : k < 11 ? P.inv_a0[a][k - 9] : P.tau_fid[a];
+    }
+    consts[i] = v;
+  }
 }
 
-// One warp, same th[] in every lane.  The transcendental calls are spread over lanes and broadcast:
-//   sincos: lane 0 gmst - ra, 1 dec, 2 psi, 3 iota          (one call instead of four)
-//   log   : lane 0 pi G Mc / c^3, lane 1 eta                 (u = (pi M)^(1/3) via ln u = ln(.)/3 - ln(eta)/5)
-//   exp   : lane 0 u, lane 1 1/u, lane 2 (G Mc/c^3)^(5/6)
-// Every lane ends with identical bits (all inputs of the replicated arithmetic come from one lane).
-__device__ __forceinline__ void point_setup_warp(const NssDev &P, const double *th, nssp::Intrinsic &I, nssp::Sky &S)
+// Same th[] in every lane.  Stage 1 (one instruction stream each, different argument per lane):
+//   1/x   : lane 0: 1 + q, 1: q, 2: d_L
+//   ln x  : lane 0: pi G Mc/c^3, 1: q, 2: 1 + q
+//   sincos: lane 0: gmst - ra, 1: dec, 2: psi, 3: iota
+// broadcast through the scratch; stage 2: lane j < 9 builds one coefficient (one exp), lane a < NDET the antenna
+// response of detector a; broadcast again.  Every lane ends with identical bits.
+template <int NDET>
+__device__ __forceinline__ void rb_point_warp(const NssDev &P, const WarpCtx &X, const double *th, RbPoint<NDET> &R)
 {
   const int lane = threadIdx.x & 31;
-  const double q = th[1];
-  const double m1 = 1.0 / (1.0 + q), m2 = q * m1;
-  const double eta = q * m1 * m1;
-  // stage 1: four angles
-  const double ang = lane == 0 ? P.gmst - th[9] : lane == 1 ? th[10] : lane == 2 ? th[8] : th[7];
-  double sn, cs;
-  sincos(ang, &sn, &cs);
-  const double sg = shfl_d(sn, 0), cg = shfl_d(cs, 0), sd = shfl_d(sn, 1), cd = shfl_d(cs, 1), sp = shfl_d(sn, 2),
-               cp = shfl_d(cs, 2), ci = shfl_d(cs, 3);
-  nssp::sky_from_sincos(sg, cg, sd, cd, sp, cp, S);
-  // stage 2: two logarithms
+  const double q = th[1], opq = 1.0 + q;
   const double mcs = th[0] * nssp::kGMsun;                       // G Mc / c^3 [s]
-  const double lg = log(lane == 0 ? nssp::kPi * mcs : eta);
-  const double ln_pimc = shfl_d(lg, 0), ln_eta = shfl_d(lg, 1);
-  const double lnu = ln_pimc * (1.0 / 3.0) - 0.2 * ln_eta;       // ln (pi M)^(1/3), M = Mc eta^(-3/5)
-  // stage 3: three exponentials
-  const double ln_mcs = ln_pimc - 1.1447298858494001741;         // ln(pi)
-  const double ex = exp(lane == 0 ? lnu : lane == 1 ? -lnu : (5.0 / 6.0) * ln_mcs);
-  const double u = shfl_d(ex, 0), iu = shfl_d(ex, 1), mc56 = shfl_d(ex, 2);
-  nssp::intrinsic_from(th, eta, m1, m2, u, iu, lnu, mc56, ci, I);
-}
-
-template <int NDET>
-__device__ __forceinline__ void rb_point_warp(const NssDev &P, const double *th, RbPoint<NDET> &R)
-{
-  nssp::Intrinsic I;
+  {
+    const double xr = lane == 0 ? opq : lane == 1 ? q : lane == 2 ? th[4] : 1.0;
+    const double xl = lane == 0 ? nssp::kPi * mcs : lane == 1 ? q : lane == 2 ? opq : 1.0;
+    const double xa = lane == 0 ? P.gmst - th[9] : lane == 1 ? th[10] : lane == 2 ? th[8] : th[7];
+    const double rc = 1.0 / xr, lg = log(xl);
+    double sn, cs;
+    nssp::sincos_turns_dev(xa * 0.15915494309189533577, &sn, &cs);
+    if (lane < 4) { X.scr[lane] = rc; X.scr[4 + lane] = lg; X.scr[8 + lane] = sn; X.scr[12 + lane] = cs; }
+  }
+  __syncwarp();
+  const double2 *s2 = reinterpret_cast<const double2 *>(X.scr);
+  const double2 r01 = s2[0], r23 = s2[1], l01 = s2[2], l23 = s2[3], sn01 = s2[4], sn23 = s2[5], cs01 = s2[6], cs23 = s2[7];
+  const double m1 = r01.x, iq = r01.y, idL = r23.x;
+  const double ln_pimc = l01.x, ln_eta = l01.y - 2.0 * l23.x;
+  const double ci = cs23.y;
   nssp::Sky S;
-  point_setup_warp(P, th, I, S);
-  rb_finish_point<NDET>(P, I, S, R);
-}
-
-// bin contribution from the waveform ratio at the bin's two edges (pre-scaled terms q[0..5], see nss_setup.cu)
-__device__ __forceinline__ double bin_term(double q0, double q1, double q2, double q3, double q4, double q5,
-                                           double r0r, double r0i, double r1r, double r1i)
-{
-  const double sr = r1r + r0r, si = r1i + r0i, tr = r1r - r0r, ti = r1i - r0i;
-  double lin = q0 * sr;
-  lin = fma(q1, si, lin);
-  lin = fma(q2, tr, lin);
-  lin = fma(q3, ti, lin);
-  const double ss = fma(sr, sr, si * si);
-  const double st = fma(sr, tr, si * ti);
-  return fma(q4, ss, fma(q5, st, lin));
-}
-
-// ---- K1, one thread per point: records streamed from `rec` (shared or global), all lanes read the
-// same address (broadcast) --------------------------------------------------------------------------
-template <int NDET>
-__device__ __forceinline__ double rb_loglike_thread(const NssDev &P, const double *__restrict__ rec,
-                                                    const RbPoint<NDET> &R)
-{
-  const int E = P.n_edges, rs = P.rb_rs;
-  double pr[NDET], pi[NDET], acc[NDET];
+  nssp::sky_from_sincos(sn01.x, cs01.x, sn01.y, cs01.y, sn23.x, cs23.x, S);
+  const double m2 = q * m1, eta = m2 * m1;
+  const double lnu = ln_pimc * (1.0 / 3.0) - 0.2 * ln_eta;       // ln (pi M)^(1/3), M = Mc eta^(-3/5)
+  const double ln_mcs = ln_pimc - 1.1447298858494001741;         // - ln(pi)
+  const double K = (3.0 / (256.0 * nssp::kPi)) * (opq * opq * iq);     // 3/(128 eta)/(2 pi), turns
+  const double beta = (113.0 / 12.0 * m1 * m1 + 6.25 * eta) * th[2] + (113.0 / 12.0 * m2 * m2 + 6.25 * eta) * th[3];
+  {
+    // coefficient lane
+    const double *cf = X.consts + (lane & 15);
+    const double E = exp(fma(cf[6 * 16], lnu, cf[7 * 16] * ln_mcs));
+    double A = cf[3 * 16];
+    A = fma(A, eta, cf[2 * 16]);
+    A = fma(A, eta, cf[1 * 16]);
+    A = fma(A, eta, cf[0]);
+    A = fma(cf[4 * 16], beta, A);
+    A = fma(cf[5 * 16], lnu, A);
+    const double val = fma((lane == 8 ? 1.0 : K) * A, E, -cf[8 * 16]);
+    // detector lane
+    const double *dt = X.consts + 9 * 16 + ((lane & 3) < NDET ? (lane & 3) : 0);
+    double D6[6], rcv[3];
 #pragma unroll
-  for (int a = 0; a < NDET; ++a) { pr[a] = 0.0; pi[a] = 0.0; acc[a] = 0.0; }
-  for (int e = 0; e < E; ++e) {
-    const double2 *r2 = reinterpret_cast<const double2 *>(rec + (size_t)e * rs);
-    const double2 g01 = r2[0], g23 = r2[1], g45 = r2[2], g67 = r2[3], fx = r2[4];
+    for (int k = 0; k < 6; ++k) D6[k] = dt[4 * k];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) rcv[k] = dt[4 * (6 + k)];
+    double fp, fc, tau;
+    nssp::antenna(S, D6, rcv, fp, fc, tau);
+    const double hr = fp * (0.5 * (1.0 + ci * ci)), hi = -fc * ci;     // F+ (1+c^2)/2 - i Fx c
+    const double i0r = dt[4 * 9], i0i = dt[4 * 10];
+    const double ar = hr * i0r - hi * i0i, ai = hr * i0i + hi * i0r;
+    const double ft = (th[5] - P.tc_fid) + (tau - dt[4 * 11]);
+    if (lane < 9) X.scr[16 + lane] = val;
+    if (lane < NDET) { X.scr[26 + 3 * lane] = ar; X.scr[27 + 3 * lane] = ai; X.scr[28 + 3 * lane] = ft; }
+  }
+  __syncwarp();
+  {
+    const double2 c01 = s2[8], c23 = s2[9], c45 = s2[10], c67 = s2[11];
+    R.dc[0] = c01.x; R.dc[1] = c01.y; R.dc[2] = c23.x; R.dc[3] = c23.y;
+    R.dc[4] = c45.x; R.dc[5] = c45.y; R.dc[6] = c67.x; R.dc[7] = c67.y;
+    const double mc56 = X.scr[24];
+    const double amp = 0.45643546458763842789 /* sqrt(5/24) */ * 0.46619407703541166 /* pi^(-2/3) */ * mc56 * nssp::kC
+                     * (idL * (1.0 / nssp::kMpc));
+#pragma unroll
+    for (int a = 0; a < NDET; ++a) {
+      R.ar[a] = X.scr[26 + 3 * a] * amp;
+      R.ai[a] = X.scr[27 + 3 * a] * amp;
+      R.ft[a] = X.scr[28 + 3 * a];
+    }
+    // c_const = (-phic - pi/4)/(2 pi) + K P5 (1 + 3 (ln u - ln v_lso)),  K P5 = coefficient 4 before the reference is subtracted
+    const double kp5 = R.dc[4] + P.c_fid[4];
+    R.dconst = fma(kp5, 1.0 + 3.0 * (lnu + 0.89587973461402748), (-th[6] - 0.25 * nssp::kPi) * 0.15915494309189533577)
+             - P.c_const_fid;
+  }
+}
+
+// ---- record loops ------------------------------------------------------------------------------------------
+// accumulators of one detector: T = sum W conj(z), Q = sum V X, and the previous record's (cos, sin)
+struct DetAcc {
+  double tr, ti, q, pc, ps;
+};
+
+template <bool CROSS>
+__device__ __forceinline__ void rec_term(DetAcc &A, double wr, double wi, double v, double c, double s)
+{
+  A.tr = fma(wr, c, A.tr); A.tr = fma(-wi, s, A.tr);
+  A.ti = fma(wr, s, A.ti); A.ti = fma(wi, c, A.ti);
+  if (CROSS) {
+    A.q = fma(v, fma(c, A.pc, s * A.ps), A.q);
+    A.pc = c; A.ps = s;
+  }
+}
+
+// logL from the accumulators; REDUCE adds the partial sums of the 32 lanes of a warp (one butterfly)
+template <int NDET, bool REDUCE>
+__device__ __forceinline__ double finish_logl(const NssDev &P, const RbPoint<NDET> &R, const DetAcc *A)
+{
+  double part = 0.0, cst = P.half_DD;
+#pragma unroll
+  for (int a = 0; a < NDET; ++a) {
+    const double h2 = 0.5 * fma(R.ar[a], R.ar[a], R.ai[a] * R.ai[a]);
+    part += fma(R.ar[a], A[a].tr, R.ai[a] * A[a].ti) - h2 * A[a].q;
+    cst = fma(h2, P.hh0[a], cst);
+  }
+  if (REDUCE) part = warp_sum(part);
+  return part - cst;
+}
+
+// one thread per point: `count` records streamed from `rec` (shared memory, all lanes read the same address)
+template <int NDET, bool CROSS>
+__device__ __forceinline__ void records_thread(const double *__restrict__ rec, int rs, int count, const RbPoint<NDET> &R,
+                                               DetAcc *A)
+{
+  constexpr int PER = CROSS ? 3 : 2;
+#pragma unroll 2
+  for (int e = 0; e < count; ++e) {
+    const double *r = rec + (size_t)e * rs;
+    const double2 *r2 = reinterpret_cast<const double2 *>(r);
+    const double2 g01 = r2[0], g23 = r2[1], g45 = r2[2], g67 = r2[3];
+    const double F = r[8];
     double ph = R.dconst;
     ph = fma(R.dc[0], g01.x, ph); ph = fma(R.dc[1], g01.y, ph);
     ph = fma(R.dc[2], g23.x, ph); ph = fma(R.dc[3], g23.y, ph);
@@ -185,34 +295,24 @@ __device__ __forceinline__ double rb_loglike_thread(const NssDev &P, const doubl
 #pragma unroll
     for (int a = 0; a < NDET; ++a) {
       double s, c;
-      nssp::sincos_turns(fma(fx.x, R.ft[a], ph), &s, &c);
-      const double rr = fma(R.ar[a], c, R.ai[a] * s);
-      const double ri = fma(R.ai[a], c, -R.ar[a] * s);
-      const double2 q01 = r2[5 + 3 * a], q23 = r2[6 + 3 * a], q45 = r2[7 + 3 * a];
-      acc[a] += bin_term(q01.x, q01.y, q23.x, q23.y, q45.x, q45.y, pr[a], pi[a], rr, ri);
-      pr[a] = rr; pi[a] = ri;
+      nssp::sincos_turns_dev(fma(F, R.ft[a], ph), &s, &c);
+      rec_term<CROSS>(A[a], r[10 + PER * a], r[11 + PER * a], CROSS ? r[12 + PER * a] : 0.0, c, s);
     }
   }
-  double tot = 0.0;
-#pragma unroll
-  for (int a = 0; a < NDET; ++a) tot += acc[a];
-  return tot - P.half_DD;
 }
 
-// ---- K1, one warp per point: lane l owns bins [l*m, l*m+m) and edges [l*m, l*m+m].
-// `tab` = warp layout (shared or global), edge-round major so every offset inside a round is an immediate:
-//   round 0 : [9][32]                      g0..g7, F of edge l*m
-//   round j : [9][32] then [NDET*6][32]    edge l*m+j, then the six pre-scaled terms of bin l*m+j-1, j = 1..m
-template <int NDET>
-__device__ __forceinline__ int rb_warp_table_doubles(int m) { return (9 + m * (9 + 6 * NDET)) * 32; }
+// one warp per point: lane l evaluates record l*m in round 0 and records l*m+1 .. l*m+m in rounds 1..m
+// (layout in nss_setup.cu); every offset inside a round is an immediate and the reads are conflict-free.
+template <int NDET, bool CROSS>
+__device__ __forceinline__ int warp_table_doubles(int m) { return ((9 + 2 * NDET) + m * (9 + (CROSS ? 3 : 2) * NDET)) * 32; }
 
-template <int NDET>
-__device__ __forceinline__ double rb_loglike_warp(const NssDev &P, const double *__restrict__ tab,
-                                                  const RbPoint<NDET> &R)
+template <int NDET, bool CROSS>
+__device__ __forceinline__ double records_warp(const NssDev &P, const double *__restrict__ tab, const RbPoint<NDET> &R)
 {
-  const int lane = threadIdx.x & 31, m = P.rb_m;
+  constexpr int PER = CROSS ? 3 : 2;
+  const int lane = threadIdx.x & 31, m = P.soa_m;
   const double *t = tab + lane;
-  double pr[NDET], pi[NDET], acc[NDET];
+  DetAcc A[NDET];
   {
     double ph = R.dconst;
 #pragma unroll
@@ -221,14 +321,15 @@ __device__ __forceinline__ double rb_loglike_warp(const NssDev &P, const double 
 #pragma unroll
     for (int a = 0; a < NDET; ++a) {
       double s, c;
-      nssp::sincos_turns(fma(F, R.ft[a], ph), &s, &c);
-      pr[a] = fma(R.ar[a], c, R.ai[a] * s);
-      pi[a] = fma(R.ai[a], c, -R.ar[a] * s);
-      acc[a] = 0.0;
+      nssp::sincos_turns_dev(fma(F, R.ft[a], ph), &s, &c);
+      const double wr = t[(9 + 2 * a) * 32], wi = t[(10 + 2 * a) * 32];
+      A[a].tr = fma(wr, c, -wi * s);
+      A[a].ti = fma(wr, s, wi * c);
+      A[a].q = 0.0; A[a].pc = c; A[a].ps = s;
     }
   }
-  t += 9 * 32;
-  for (int j = 1; j <= m; ++j, t += (9 + 6 * NDET) * 32) {
+  t += (9 + 2 * NDET) * 32;
+  for (int j = 1; j <= m; ++j, t += (9 + PER * NDET) * 32) {
     double ph = R.dconst;
 #pragma unroll
     for (int c = 0; c < kNB; ++c) ph = fma(R.dc[c], t[c * 32], ph);
@@ -236,60 +337,12 @@ __device__ __forceinline__ double rb_loglike_warp(const NssDev &P, const double 
 #pragma unroll
     for (int a = 0; a < NDET; ++a) {
       double s, c;
-      nssp::sincos_turns(fma(F, R.ft[a], ph), &s, &c);
-      const double rr = fma(R.ar[a], c, R.ai[a] * s);
-      const double ri = fma(R.ai[a], c, -R.ar[a] * s);
-      const double *q = t + (9 + 6 * a) * 32;
-      acc[a] += bin_term(q[0], q[32], q[64], q[96], q[128], q[160], pr[a], pi[a], rr, ri);
-      pr[a] = rr; pi[a] = ri;
+      nssp::sincos_turns_dev(fma(F, R.ft[a], ph), &s, &c);
+      const double *w = t + (9 + PER * a) * 32;
+      rec_term<CROSS>(A[a], w[0], w[32], CROSS ? w[64] : 0.0, c, s);
     }
   }
-  double tot = 0.0;
-#pragma unroll
-  for (int a = 0; a < NDET; ++a) tot += acc[a];
-  return warp_sum(tot) - P.half_DD;
-}
-
-// ---- K2, full grid, one warp per point: lanes stride over frequencies, 128-bit loads -----------------
-template <int NDET>
-__device__ __forceinline__ double full_loglike_warp(const NssDev &P, const double *th)
-{
-  nssp::Intrinsic I;
-  nssp::Sky S;
-  point_setup_warp(P, th, I, S);
-  const double ci = I.cos_iota;
-  const double pp = 0.5 * (1.0 + ci * ci) * I.amp, pc = -ci * I.amp;
-  double hr[NDET], hi[NDET], ft[NDET], acc[NDET];
-#pragma unroll
-  for (int a = 0; a < NDET; ++a) {
-    double fp, fc, tau;
-    nssp::antenna(S, P.D6[a], P.rc[a], fp, fc, tau);
-    hr[a] = fp * pp; hi[a] = fc * pc; ft[a] = I.tc + tau; acc[a] = 0.0;
-  }
-  const int lane = threadIdx.x & 31, n = P.n_freq, rs = P.full_rs;
-  for (int k = lane; k < n; k += 32) {
-    const double2 *r2 = reinterpret_cast<const double2 *>(P.full_rec + (size_t)k * rs);
-    const double2 g01 = __ldg(r2), g23 = __ldg(r2 + 1), g45 = __ldg(r2 + 2), g67 = __ldg(r2 + 3), fx = __ldg(r2 + 4);
-    double ph = I.c_const;
-    ph = fma(I.c[0], g01.x, ph); ph = fma(I.c[1], g01.y, ph);
-    ph = fma(I.c[2], g23.x, ph); ph = fma(I.c[3], g23.y, ph);
-    ph = fma(I.c[4], g45.x, ph); ph = fma(I.c[5], g45.y, ph);
-    ph = fma(I.c[6], g67.x, ph); ph = fma(I.c[7], g67.y, ph);
-    const double *rd = P.full_rec + (size_t)k * rs + 10;
-#pragma unroll
-    for (int a = 0; a < NDET; ++a) {
-      double s, c;
-      nssp::sincos_turns(fma(fx.x, ft[a], ph), &s, &c);
-      const double ar = hr[a] * fx.y, ai = hi[a] * fx.y;         // amplitude * f^-7/6
-      const double mr = fma(ar, c, ai * s), mi = fma(ai, c, -ar * s);
-      const double dr = __ldg(rd + 3 * a) - mr, di = __ldg(rd + 3 * a + 1) - mi;
-      acc[a] = fma(__ldg(rd + 3 * a + 2), fma(dr, dr, di * di), acc[a]);
-    }
-  }
-  double tot = 0.0;
-#pragma unroll
-  for (int a = 0; a < NDET; ++a) tot += acc[a];
-  return -0.5 * warp_sum(tot);
+  return finish_logl<NDET, true>(P, R, A);
 }
 
 // O16 Gaussian test likelihood on sampled coordinates (memory operand; uniform indices)
@@ -309,21 +362,18 @@ __device__ __forceinline__ double gauss_loglike(const NssDev &P, const double *_
 }
 
 // One warp evaluates logL of the sampled coordinates `theta` (memory the whole warp can read: global or the
-// warp's shared scratch); every lane returns the same bits.  `tab` = warp-layout RB table (shared or
-// global), ignored for other kinds.
+// warp's shared scratch); every lane returns the same bits.  X.tab = warp-layout record table (shared or
+// global), ignored by the Gaussian kind.
 template <int NDET, int KIND>
-__device__ __forceinline__ double loglike_warp(const NssDev &P, const double *__restrict__ tab, const double *__restrict__ theta)
+__device__ __forceinline__ double loglike_warp(const NssDev &P, const WarpCtx &X, const double *__restrict__ theta)
 {
   if (KIND == NSS_KIND_GAUSS) return gauss_loglike(P, theta);
   double th[NSS_NSLOT];
   canon_from_mem(P, theta, th);
   if (!nssp::domain_ok(th)) return -INFINITY;
-  if (KIND == NSS_KIND_RB) {
-    RbPoint<NDET> R;
-    rb_point_warp<NDET>(P, th, R);
-    return rb_loglike_warp<NDET>(P, tab, R);
-  }
-  return full_loglike_warp<NDET>(P, th);
+  RbPoint<NDET> R;
+  rb_point_warp<NDET>(P, X, th, R);
+  return records_warp<NDET, KIND == NSS_KIND_RB>(P, X.tab, R);
 }
 
 }  // namespace nssk

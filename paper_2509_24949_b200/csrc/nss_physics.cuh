@@ -155,6 +155,13 @@ NSS_HD void basis(double f, double *g)
 // quadrant swaps and negates through the sign bit.  17 fp64-pipe instructions and ~10 integer ones, no
 // conversion (XU) instructions; a non-finite t gives NaNs.
 #if defined(__CUDACC__)
+// coefficients in the constant bank: an fp64 instruction takes them as c[bank][offset] operands, whereas
+// immediates are re-materialised into uniform registers (two UMOV each) inside every loop body
+static __constant__ double kSinT[7] = {0x1.921fb54442d18p+2, -0x1.4abbce625be41p+5, 0x1.466bc677587f8p+6, -0x1.32d2cce2e5b19p+6,
+                                       0x1.50782fda12d96p+5, -0x1.e30071afc3e59p+3, 0x1.e3f38399551bfp+1};
+static __constant__ double kCosT[7] = {1.0, -0x1.3bd3cc9be458bp+4, 0x1.03c1f081b0780p+6, -0x1.55d3c7dbfd139p+6,
+                                       0x1.e1f4fb60281f6p+5, -0x1.a6c9c1be9eb49p+4, 0x1.f3dbcea61b1a4p+2};
+
 __device__ __forceinline__ void sincos_turns_dev(double t, double *s, double *c)
 {
   const double kMagic = 6755399441055744.0;            // 1.5 * 2^52
@@ -162,21 +169,13 @@ __device__ __forceinline__ void sincos_turns_dev(double t, double *s, double *c)
   const int q = __double2loint(tq);
   const double r = fma(tq - kMagic, -0.25, t);
   const double y = r * r;
-  double ps = 0x1.e3f38399551bfp+1;
-  ps = fma(ps, y, -0x1.e30071afc3e59p+3);
-  ps = fma(ps, y, 0x1.50782fda12d96p+5);
-  ps = fma(ps, y, -0x1.32d2cce2e5b19p+6);
-  ps = fma(ps, y, 0x1.466bc677587f8p+6);
-  ps = fma(ps, y, -0x1.4abbce625be41p+5);
-  ps = fma(ps, y, 0x1.921fb54442d18p+2);
+  double ps = kSinT[6], pc = kCosT[6];
+#pragma unroll
+  for (int k = 5; k >= 0; --k) {
+    ps = fma(ps, y, kSinT[k]);
+    pc = fma(pc, y, kCosT[k]);
+  }
   ps *= r;
-  double pc = 0x1.f3dbcea61b1a4p+2;
-  pc = fma(pc, y, -0x1.a6c9c1be9eb49p+4);
-  pc = fma(pc, y, 0x1.e1f4fb60281f6p+5);
-  pc = fma(pc, y, -0x1.55d3c7dbfd139p+6);
-  pc = fma(pc, y, 0x1.03c1f081b0780p+6);
-  pc = fma(pc, y, -0x1.3bd3cc9be458bp+4);
-  pc = fma(pc, y, 1.0);
   const bool sw = q & 1;
   const double a = sw ? pc : ps, b = sw ? ps : pc;     // quadrant 1, 3: sin <- cos, cos <- sin
   const int ah = __double2hiint(a) ^ ((q << 30) & 0x80000000);          // sin < 0 in quadrants 2, 3

@@ -397,20 +397,26 @@ __global__ void __launch_bounds__(kChainThreads, 2) k3_slice(const __grid_consta
   __shared__ double sY[kChainWarps][NSS_NSLOT + 1];                // per warp: sampled coordinates of its candidate
   __shared__ double sRes[kChainWarps][2][kChainWarps];             // per group, double-buffered: logL of slot w
   __shared__ int32_t sFlag[kChainWarps][2][kChainWarps];           // 1 = in the box (evaluated), 0 = outside the box
+  __shared__ __align__(16) double sConst[nssk::kWarpConstDoubles];
+  __shared__ __align__(16) double sScr[kChainWarps][nssk::kWarpScratchDoubles];
   if (A.flags[0] | A.flags[1]) return;
-  const double *tab = P.rb_soa;
+  nssk::WarpCtx X;
+  X.tab = P.soa;
+  X.consts = sConst;
+  X.scr = sScr[threadIdx.x >> 5];
   if (RESIDENT) {
     if (threadIdx.x == 0) {
       nssk::mbar_init(&bar, 1);
-      nssk::stage_table(smem_raw, P.rb_soa, (uint32_t)(nssk::rb_warp_table_doubles<NDET>(P.rb_m) * sizeof(double)), &bar);
+      nssk::stage_table(smem_raw, P.soa, (uint32_t)(nssk::warp_table_doubles<NDET, KIND == NSS_KIND_RB>(P.soa_m) * sizeof(double)), &bar);
     }
   }
   const int d = P.d;
   for (int t = threadIdx.x; t < d * d; t += blockDim.x) sL[t] = A.chol[t];
+  if (KIND != NSS_KIND_GAUSS) nssk::warp_consts_init(P, sConst);
   __syncthreads();
   if (RESIDENT) {
     nssk::mbar_wait(&bar, 0);
-    tab = reinterpret_cast<const double *>(smem_raw);
+    X.tab = reinterpret_cast<const double *>(smem_raw);
   }
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int G = A.G, GL = G * 32;
@@ -501,7 +507,7 @@ __global__ void __launch_bounds__(kChainThreads, 2) k3_slice(const __grid_consta
             if (inbox) {
               if (own) sY[warp][lane] = yj;
               __syncwarp();
-              ly = nssk::loglike_warp<NDET, KIND>(P, tab, sY[warp]);
+              ly = nssk::loglike_warp<NDET, KIND>(P, X, sY[warp]);
               __syncwarp();
             }
           }
@@ -594,7 +600,7 @@ int launch_chains(nss_handle *h, ChainArgs &A, cudaStream_t st)
   }
   int rc;
   if (P.kind == NSS_KIND_RB) {
-    const size_t bytes = (size_t)(9 + P.rb_m * (9 + 6 * NDET)) * 32 * sizeof(double);
+    const size_t bytes = (size_t)((9 + 2 * NDET) + P.soa_m * (9 + 3 * NDET)) * 32 * sizeof(double);
     if (bytes + 40 * 1024 <= 110 * 1024)                 // table + static arrays, two CTAs per SM
       rc = launch_chains_k<NDET, NSS_KIND_RB, true>(h, A, bytes, st);
     else

@@ -115,6 +115,8 @@ std::vector<int32_t> choose_edges(int n, double f_min, double df, int B)
   return ie;
 }
 
+inline int per_of(int round, int per) { return round == 0 ? 2 : per; }
+
 template <class T>
 int upload(const std::vector<T> &v, T **dptr, size_t *bytes)
 {
@@ -145,7 +147,7 @@ extern "C" int nss_destroy(nss_handle *h)
 {
   if (!h) return NSS_OK;
   cudaSetDevice(h->device);
-  cudaFree(h->d_rb_rec); cudaFree(h->d_rb_soa); cudaFree(h->d_full_rec);
+  cudaFree(h->d_rec); cudaFree(h->d_soa);
   cudaFree(h->d_surv_idx); cudaFree(h->d_dead_idx); cudaFree(h->d_rank); cudaFree(h->d_ctl);
   if (h->h_ctl) cudaFreeHost(h->h_ctl);
   cudaFree(h->d_mean); cudaFree(h->d_chol); cudaFree(h->d_birth); cudaFree(h->d_stage);
@@ -224,25 +226,41 @@ extern "C" int nss_create(const nss_config *cfg, nss_handle **out)
   h->DD = DD;
   P.half_DD = 0.5 * DD;
 
+  // ---- record tables ---------------------------------------------------------------------------------
+  // Both likelihoods are evaluated in the same form.  With the detector waveform written as
+  //     h(f) = A f^-7/6 z(f),  z = exp(-2 pi i phi(f)),  A = complex amplitude of the point (no f dependence),
+  // and h0 = A0 f^-7/6 z0 the heterodyne reference (kind 0) or A0 = z0 = 1 (kind 1), the ratio is
+  // r = (A/A0) (z/z0), |r| = |A/A0| at every frequency, and per detector
+  //     <d,h> = Re( conj(A/A0) T ),       T = sum_rec W_rec conj(z/z0)_rec
+  //     <h,h> = |A/A0|^2 ( hh0 + sum_b V_b X_b ),   X_b = Re( (z/z0)_b conj (z/z0)_{b+1} ).
+  // kind 0 (O10): records are the bin edges; collecting r0 = (r_b + r_b+1)/2, r1 = (r_b+1 - r_b)/dF per edge,
+  //     W_e = [e < B](A0_e/2 - A1_e/dF_e) + [e > 0](A0_e-1/2 + A1_e-1/dF_e-1),  V_b = B0_b/2,  hh0 = sum_b B0_b/2;
+  //     the B1 term, 2 B1_b Re(r0 conj r1) = B1_b (|r_b+1|^2 - |r_b|^2)/dF, vanishes because |r| is constant.
+  // kind 1 (O7): records are the grid frequencies; W_k = (4 df/S_k) d_k f_k^-7/6, no cross term,
+  //     hh0 = sum_k (4 df/S_k) f_k^-7/3;  logL = sum_det(<d,h> - <h,h>/2) - DD/2 as for kind 0.
   int rc_up = NSS_OK;
+  std::vector<double> rf;                    // record frequencies
+  std::vector<double> W;                     // [nd][n_rec][2]
+  std::vector<double> V;                     // [nd][n_rec]: V of the bin ending at this record (0 for record 0)
+  int n_rec = 0;
   if (kind == NSS_KIND_FULL) {
-    // full-grid records: g0..g7, f, f^-7/6, then per detector (d_re, d_im, 4 df / S)
-    const int rs = (10 + 3 * nd + 1) & ~1;
-    std::vector<double> rec((size_t)n * rs, 0.0);
-    for (int k = 0; k < n; ++k) {
-      double *r = &rec[(size_t)k * rs];
-      nssp::basis(f[k], r);
-      r[8] = f[k];
-      r[9] = 1.0 / (f[k] * sqrt(cbrt(f[k])));
-      for (int a = 0; a < nd; ++a) {
-        r[10 + 3 * a] = data[(size_t)a * n + k].real();
-        r[11 + 3 * a] = data[(size_t)a * n + k].imag();
-        r[12 + 3 * a] = 4.0 * df / cfg->psd[(size_t)a * n + k];
+    n_rec = n;
+    rf = f;
+    W.assign((size_t)nd * n * 2, 0.0);
+    for (int a = 0; a < nd; ++a) {
+      P.inv_a0[a][0] = 1.0; P.inv_a0[a][1] = 0.0;
+      double hh = 0.0;
+      for (int k = 0; k < n; ++k) {
+        const double w = 4.0 * df / cfg->psd[(size_t)a * n + k];
+        const double f76 = 1.0 / (f[k] * sqrt(cbrt(f[k])));
+        const cplx dk = data[(size_t)a * n + k];
+        W[((size_t)a * n + k) * 2] = w * f76 * dk.real();
+        W[((size_t)a * n + k) * 2 + 1] = w * f76 * dk.imag();
+        hh += w * f76 * f76;
       }
+      P.hh0[a] = hh;
     }
-    P.full_rs = rs;
-    rc_up = upload(rec, &h->d_full_rec, &h->full_rec_bytes);
-    P.full_rec = h->d_full_rec;
+    P.cross = 0;
   } else {
     const int B = cfg->n_bins, E = B + 1;
     P.n_bins = B; P.n_edges = E;
@@ -278,55 +296,71 @@ extern "C" int nss_create(const nss_config *cfg, nss_handle **out)
         s[0] = a0.real(); s[1] = a0.imag(); s[2] = a1.real(); s[3] = a1.imag(); s[4] = b0; s[5] = b1;
       }
     }
-    // pre-scaled bin terms: with s = r_b + r_{b+1}, t = r_{b+1} - r_b  (r0 = s/2, r1 = t/dF):
-    //   <d,h> - <h,h>/2 = q0 s_re + q1 s_im + q2 t_re + q3 t_im + q4 |s|^2 + q5 Re(s conj t)
-    auto scaled = [&](int a, int b, double *q) {
-      const double *s = &h->summary[((size_t)a * B + b) * 6];
-      const double idF = 1.0 / (f[h->edge_idx[b + 1]] - f[h->edge_idx[b]]);
-      q[0] = 0.5 * s[0]; q[1] = 0.5 * s[1];
-      q[2] = s[2] * idF; q[3] = s[3] * idF;
-      q[4] = -0.125 * s[4];
-      q[5] = -0.5 * s[5] * idF;
-    };
-    // (1) AoS records for the thread-per-point kernel
-    const int rs = 10 + 6 * nd;
-    std::vector<double> rec((size_t)E * rs, 0.0);
-    for (int e = 0; e < E; ++e) {
-      double *r = &rec[(size_t)e * rs];
-      nssp::basis(f[h->edge_idx[e]], r);
-      r[8] = f[h->edge_idx[e]];
-      if (e > 0)
-        for (int a = 0; a < nd; ++a) scaled(a, e - 1, r + 10 + 6 * a);
+    n_rec = E;
+    rf.resize(E);
+    for (int e = 0; e < E; ++e) rf[e] = f[h->edge_idx[e]];
+    W.assign((size_t)nd * E * 2, 0.0);
+    V.assign((size_t)nd * E, 0.0);
+    for (int a = 0; a < nd; ++a) {
+      double hh = 0.0;
+      for (int b = 0; b < B; ++b) {
+        const double *s = &h->summary[((size_t)a * B + b) * 6];
+        const double idF = 1.0 / (rf[b + 1] - rf[b]);
+        double *wl = &W[((size_t)a * E + b) * 2], *wr = &W[((size_t)a * E + b + 1) * 2];
+        wl[0] += 0.5 * s[0] - s[2] * idF; wl[1] += 0.5 * s[1] - s[3] * idF;
+        wr[0] += 0.5 * s[0] + s[2] * idF; wr[1] += 0.5 * s[1] + s[3] * idF;
+        V[(size_t)a * E + b + 1] = 0.5 * s[4];
+        hh += 0.5 * s[4];
+      }
+      P.hh0[a] = hh;
     }
-    P.rb_rs = rs;
-    rc_up = upload(rec, &h->d_rb_rec, &h->rb_rec_bytes);
-    P.rb_rec = h->d_rb_rec;
-    // (2) warp layout, edge-round major: lane l owns bins [l*m, l*m+m) and edges [l*m, l*m+m]
-    //     round 0: [9][32] (g0..g7, F of edge l*m); round j = 1..m: [9][32] of edge l*m+j, then [nd*6][32] of bin l*m+j-1
-    const int m = (B + 31) / 32;
-    P.rb_m = m;
-    const size_t round_sz = (size_t)(9 + 6 * nd) * 32;
-    std::vector<double> soa((size_t)9 * 32 + (size_t)m * round_sz, 0.0);
+    P.cross = 1;
+  }
+  {
+    const int cr = P.cross, per = 2 + cr;
+    P.n_rec = n_rec;
+    // (1) AoS records for the thread-per-point kernel: g0..g7, f, pad, then per detector (Wr, Wi[, V])
+    const int rs = (10 + per * nd + 1) & ~1;
+    std::vector<double> rec((size_t)n_rec * rs, 0.0);
+    for (int e = 0; e < n_rec; ++e) {
+      double *r = &rec[(size_t)e * rs];
+      nssp::basis(rf[e], r);
+      r[8] = rf[e];
+      for (int a = 0; a < nd; ++a) {
+        r[10 + per * a] = W[((size_t)a * n_rec + e) * 2];
+        r[11 + per * a] = W[((size_t)a * n_rec + e) * 2 + 1];
+        if (cr) r[12 + per * a] = V[(size_t)a * n_rec + e];
+      }
+    }
+    P.rec_rs = rs;
+    rc_up = upload(rec, &h->d_rec, &h->rec_bytes);
+    P.rec = h->d_rec;
+    // (2) warp layout, round major: lane l owns records l*m+1 .. l*m+m (rounds 1..m) and evaluates record l*m in
+    //     round 0 (the left edge of its first bin; its W counts for lane 0 only).  Records past the end repeat the
+    //     last one with zero weights.
+    const int m = n_rec > 1 ? (n_rec - 1 + 31) / 32 : 1;
+    P.soa_m = m;
+    const size_t r0_sz = (size_t)(9 + 2 * nd) * 32, round_sz = (size_t)(9 + per * nd) * 32;
+    std::vector<double> soa(r0_sz + (size_t)m * round_sz, 0.0);
     for (int l = 0; l < 32; ++l) {
       for (int j = 0; j <= m; ++j) {
-        double *te = j == 0 ? soa.data() : soa.data() + 9 * 32 + (size_t)(j - 1) * round_sz;
-        int e = l * m + j;
-        if (e > B) e = B;
+        double *te = j == 0 ? soa.data() : soa.data() + r0_sz + (size_t)(j - 1) * round_sz;
+        const int e0 = l * m + j;
+        const int e = e0 < n_rec ? e0 : n_rec - 1;
         double g[nssp::kNB];
-        nssp::basis(f[h->edge_idx[e]], g);
+        nssp::basis(rf[e], g);
         for (int c = 0; c < 8; ++c) te[c * 32 + l] = g[c];
-        te[8 * 32 + l] = f[h->edge_idx[e]];
-        const int b = l * m + j - 1;
-        if (j == 0 || b >= B) continue;
+        te[8 * 32 + l] = rf[e];
+        if (e0 >= n_rec || (j == 0 && l != 0)) continue;
         for (int a = 0; a < nd; ++a) {
-          double q[6];
-          scaled(a, b, q);
-          for (int c = 0; c < 6; ++c) te[(9 + a * 6 + c) * 32 + l] = q[c];
+          te[(9 + per_of(j, per) * a) * 32 + l] = W[((size_t)a * n_rec + e) * 2];
+          te[(10 + per_of(j, per) * a) * 32 + l] = W[((size_t)a * n_rec + e) * 2 + 1];
+          if (cr && j > 0) te[(11 + per * a) * 32 + l] = V[(size_t)a * n_rec + e];
         }
       }
     }
-    if (rc_up == NSS_OK) rc_up = upload(soa, &h->d_rb_soa, &h->rb_soa_bytes);
-    P.rb_soa = h->d_rb_soa;
+    if (rc_up == NSS_OK) rc_up = upload(soa, &h->d_soa, &h->soa_bytes);
+    P.soa = h->d_soa;
   }
   if (rc_up != NSS_OK) { nss_destroy(h); return rc_up; }
   *out = h;

@@ -31,8 +31,9 @@ struct NssDev {
   int32_t cross;          // 1: records carry the cross-term weight V (kind 0), 0: they do not (kind 1)
   const double *rec;      // AoS [n_rec][rec_rs]: g0..g7, f, pad, then per det (Wr, Wi[, V])
   int32_t rec_rs;
-  const double *soa;      // warp layout, round major: [9 + 2 n_det][32], then m x [9 + (2 + cross) n_det][32]
-  int32_t soa_m;          // rounds after round 0 = ceil((n_rec - 1)/32); lane l owns records l*m+1 .. l*m+m
+  const double *soa;      // sub-warp layout, round major: [9 + 2 n_det][L], then m x [9 + (2 + cross) n_det][L]
+  int32_t soa_m;          // rounds after round 0 = ceil((n_rec - 1)/L); lane l owns records l*m+1 .. l*m+m
+  int32_t soa_lanes;      // L = lanes per point: 8 or 32
 };
 
 // device control block of an NS iteration; one pinned host mirror per handle (a single small D2H copy per sync)

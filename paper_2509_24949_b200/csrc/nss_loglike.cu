@@ -7,8 +7,9 @@
 //                 copies and read by broadcast: whole when it fits (relative binning: one load per CTA, then a
 //                 persistent grid-stride loop over points), else streamed in double-buffered tiles, one batch of
 //                 blockDim points per pass (full grid: 4017 records).  Highest throughput for large N.
-//  k_rec_warp   : ONE WARP per point (lanes own contiguous record slices, per-point setup spread over lanes,
-//                 warp-shuffle reduction).  For small N, and the form the slice sampler inlines.
+//  k_rec_sub    : a SUB-WARP of 8 (or 32) lanes per point, four (or one) points per warp: lanes own contiguous
+//                 record slices, the per-point setup is spread over lanes, shuffle reduction.  For small N, and
+//                 the form the slice sampler inlines.
 //  k_gauss      : O16 test likelihood.
 #include "nss_loglike_dev.cuh"
 
@@ -52,7 +53,7 @@ __global__ void __launch_bounds__(kThreads) k_rec_thread(const __grid_constant__
         nssk::DetAcc A[NDET];
         zero_acc<NDET, CROSS>(A);
         nssk::records_thread<NDET, CROSS>(rec, rs, n_rec, R, A);
-        l = nssk::finish_logl<NDET, false>(P, R, A);
+        l = nssk::finish_logl<NDET>(P, R, A);
       }
       out[i] = l;
     }
@@ -92,39 +93,48 @@ __global__ void __launch_bounds__(kThreads) k_rec_thread(const __grid_constant__
       const double *rec = reinterpret_cast<const double *>(smem_raw + (size_t)(seq & 1) * tile_bytes);
       nssk::records_thread<NDET, CROSS>(rec, rs, min(tile_recs, n_rec - t * tile_recs), R, A);
     }
-    if (t == n_tiles - 1 && i < N) out[i] = ok ? nssk::finish_logl<NDET, false>(P, R, A) : -INFINITY;
+    if (t == n_tiles - 1 && i < N) out[i] = ok ? nssk::finish_logl<NDET>(P, R, A) : -INFINITY;
     __syncthreads();
   }
 }
 
-template <int NDET, int KIND, bool RESIDENT>
-__global__ void __launch_bounds__(kThreads) k_rec_warp(const __grid_constant__ NssDev P, const double *__restrict__ theta,
-                                                       int64_t N, double *__restrict__ out)
+template <int NDET, int KIND, int LANES, bool RESIDENT>
+__global__ void __launch_bounds__(kThreads) k_rec_sub(const __grid_constant__ NssDev P, const double *__restrict__ theta,
+                                                      int64_t N, double *__restrict__ out)
 {
+  constexpr int NSUB = 32 / LANES;                     // points per warp
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ __align__(8) uint64_t bar;
-  __shared__ __align__(16) double consts[nssk::kWarpConstDoubles];
-  __shared__ __align__(16) double scratch[kThreads / 32][nssk::kWarpScratchDoubles];
-  nssk::WarpCtx X;
+  __shared__ __align__(16) double consts[nssk::kSubConstDoubles];
+  __shared__ __align__(16) double scratch[kThreads / LANES][nssk::kSubScratchDoubles];
+  nssk::SubCtx X;
   X.tab = P.soa;
   X.consts = consts;
-  X.scr = scratch[threadIdx.x >> 5];
+  X.scr = scratch[threadIdx.x / LANES];
   if (RESIDENT && threadIdx.x == 0) {
     nssk::mbar_init(&bar, 1);
-    nssk::stage_table(smem_raw, P.soa, (uint32_t)(nssk::warp_table_doubles<NDET, KIND == NSS_KIND_RB>(P.soa_m) * sizeof(double)), &bar);
+    nssk::stage_table(smem_raw, P.soa, (uint32_t)(nssk::sub_table_doubles<NDET, KIND == NSS_KIND_RB, LANES>(P.soa_m) * sizeof(double)), &bar);
   }
-  nssk::warp_consts_init(P, consts);
+  nssk::sub_consts_init(P, consts);
+  const int d = P.d, sl = threadIdx.x & (LANES - 1);
+  // canonical slots that are not sampled never change
+  for (int t = sl; t < 12; t += LANES) X.scr[t] = t < NSS_NSLOT ? P.theta_fixed[t] : 0.0;
   __syncthreads();
   if (RESIDENT) {
     nssk::mbar_wait(&bar, 0);
     X.tab = reinterpret_cast<const double *>(smem_raw);
   }
-  const int d = P.d, lane = threadIdx.x & 31;
-  const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  const int64_t nwarp = ((int64_t)gridDim.x * blockDim.x) >> 5;
-  for (int64_t i = warp0; i < N; i += nwarp) {
-    const double l = nssk::loglike_warp<NDET, KIND>(P, X, theta + i * d);
-    if (lane == 0) out[i] = l;
+  const int64_t sub0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / LANES;
+  const int64_t nsub = ((int64_t)gridDim.x * blockDim.x) / LANES;
+  // the sub-warps of a warp iterate together (loglike_sub is a whole-warp call)
+  for (int64_t i0 = sub0 - (sub0 % NSUB); i0 < N; i0 += nsub) {
+    const int64_t i = i0 + (sub0 % NSUB);
+    const bool want = i < N;
+    if (want)
+      for (int j = sl; j < d; j += LANES) X.scr[P.param_index[j]] = theta[i * d + j];
+    __syncwarp();
+    const double l = nssk::loglike_sub<NDET, KIND, LANES>(P, X, want);
+    if (want && sl == 0) out[i] = l;
   }
 }
 
@@ -140,7 +150,31 @@ __global__ void __launch_bounds__(kThreads) k_gauss(const __grid_constant__ NssD
 template <class K>
 int set_smem(K kernel, size_t bytes)
 {
-  if (bytes > 48 * 1024) NSS_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+  if (bytes > 0) NSS_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));   // static + dynamic may exceed 48 KB
+  return NSS_OK;
+}
+
+template <int NDET, int KIND, int LANES>
+int launch_sub(nss_handle *h, const double *theta, int64_t N, double *logL, cudaStream_t st)
+{
+  constexpr bool CROSS = KIND == NSS_KIND_RB;
+  const NssDev &P = h->dev;
+  const size_t bytes = (size_t)((9 + 2 * NDET) + P.soa_m * (9 + (CROSS ? 3 : 2) * NDET)) * LANES * sizeof(double);
+  const size_t fixed = 8 * 1024 + sizeof(double) * (kThreads / LANES) * nssk::kSubScratchDoubles;
+  const bool resident = bytes + fixed <= 200 * 1024;
+  const size_t smem = resident ? bytes : 0;
+  int per_sm = resident ? (int)(kSmemMax / (bytes + fixed)) : 8;
+  per_sm = per_sm > 8 ? 8 : per_sm;
+  const int64_t want = (N * LANES + kThreads - 1) / kThreads;
+  const int64_t cap = (int64_t)h->n_sm * per_sm;
+  const int grid = (int)(want < cap ? want : cap);
+  if (resident) {
+    int rc = set_smem(k_rec_sub<NDET, KIND, LANES, true>, smem);
+    if (rc) return rc;
+    k_rec_sub<NDET, KIND, LANES, true><<<grid, kThreads, smem, st>>>(P, theta, N, logL);
+  } else {
+    k_rec_sub<NDET, KIND, LANES, false><<<grid, kThreads, 0, st>>>(P, theta, N, logL);
+  }
   return NSS_OK;
 }
 
@@ -149,7 +183,7 @@ int launch_rec(nss_handle *h, const double *theta, int64_t N, double *logL, cuda
 {
   constexpr bool CROSS = KIND == NSS_KIND_RB;
   const NssDev &P = h->dev;
-  int variant = h->loglike_variant;
+  int variant = h->loglike_variant, rc_sub = NSS_OK;
   if (variant == 0) variant = N >= (int64_t)h->n_sm * 512 ? 1 : 2;
   if (variant == 1) {
     const size_t rec_bytes = (size_t)P.rec_rs * sizeof(double), bytes = (size_t)P.n_rec * rec_bytes;
@@ -175,22 +209,13 @@ int launch_rec(nss_handle *h, const double *theta, int64_t N, double *logL, cuda
       k_rec_thread<NDET, CROSS, true><<<grid, kThreads, smem, st>>>(P, theta, N, logL, tile_recs, n_tiles);
     }
   } else {
-    const size_t bytes = (size_t)((9 + 2 * NDET) + P.soa_m * (9 + (CROSS ? 3 : 2) * NDET)) * 32 * sizeof(double);
-    const bool resident = bytes + 8 * 1024 <= 200 * 1024;
-    const size_t smem = resident ? bytes : 0;
-    int per_sm = resident ? (int)(kSmemMax / (bytes + 8 * 1024)) : 8;
-    per_sm = per_sm > 8 ? 8 : per_sm;
-    const int64_t want = (N * 32 + kThreads - 1) / kThreads;
-    const int64_t cap = (int64_t)h->n_sm * per_sm;
-    const int grid = (int)(want < cap ? want : cap);
-    if (resident) {
-      int rc = set_smem(k_rec_warp<NDET, KIND, true>, smem);
-      if (rc) return rc;
-      k_rec_warp<NDET, KIND, true><<<grid, kThreads, smem, st>>>(P, theta, N, logL);
+    if constexpr (KIND == NSS_KIND_RB) {
+      rc_sub = P.soa_lanes == 8 ? launch_sub<NDET, KIND, 8>(h, theta, N, logL, st) : launch_sub<NDET, KIND, 32>(h, theta, N, logL, st);
     } else {
-      k_rec_warp<NDET, KIND, false><<<grid, kThreads, 0, st>>>(P, theta, N, logL);
+      rc_sub = launch_sub<NDET, KIND, 32>(h, theta, N, logL, st);
     }
   }
+  if (rc_sub) return rc_sub;
   return NSS_OK;
 }
 

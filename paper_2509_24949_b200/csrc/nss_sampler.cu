@@ -348,10 +348,10 @@ __global__ void k_gather_rows(const double *__restrict__ live, const double *__r
 }
 
 // ---- K3: slice-sampling chains (O12.4, O12.5) -------------------------------------------------------------------
-// A chain is run by a GROUP of G warps (G = 1, 2, 4 or 8, chosen so the chains fill the GPU).  Every bracket
-// test is one likelihood evaluation by ONE warp; the G warps of a group evaluate, in the same round, the next
-// G tests of the sequential algorithm under the assumption that each of them fails — which is what they do
-// most of the time:
+// A chain is run by a GROUP of G warps (G = 1, 2, 4 or 8).  Every bracket test is one likelihood evaluation by
+// ONE SUB-WARP of LANES lanes (8 for relative binning: four candidates per warp share every instruction of the
+// per-point setup; 32 otherwise), so a group evaluates C = G * 32/LANES candidates per round: the next C tests of
+// the sequential algorithm under the assumption that each of them fails — which is what they do most of the time:
 //     [left end l, if the left side is still stepping out] [right end r, likewise]
 //     [shrinkage proposals t_kk, t_kk+1, ... from the bracket those two tests would leave]
 // The proposals that follow a rejection depend only on the rejected proposals (bracket <- t on the side of
@@ -359,7 +359,8 @@ __global__ void k_gather_rows(const double *__restrict__ live, const double *__r
 // every warp replays the sequential decisions on the shared results and discards whatever the sequential
 // algorithm would not have evaluated (shrinkage proposals speculated across an expansion; proposals after
 // the accepted one).  Decisions, positions and the evaluation count are those of the sequential oracle.
-// The chain position x and direction v are spread over lanes (lane j holds x_j, v_j).
+// The chain position x and direction v are spread over the lanes of every sub-warp (lane j holds x_j, v_j, and
+// x_{j+LANES}, v_{j+LANES} when LANES < d).
 struct ChainArgs {
   double *live;                 // [n][d] in/out
   double *logL;                 // [n]    in/out
@@ -377,68 +378,85 @@ struct ChainArgs {
   int32_t G;                    // warps per chain
 };
 
-constexpr int kChainThreads = 256;      // 8 warps per CTA = 8/G chain groups
-constexpr int kChainWarps = kChainThreads / 32;
+constexpr int kChainWarps = 8;          // largest group; a CTA is ONE group (G warps), one chain at a time
+constexpr int kChainThreads = kChainWarps * 32;
 constexpr int kDirChunk = 16;           // slice directions are drawn 16 steps at a time by the whole group
 
-__device__ __forceinline__ void group_sync(int id, int nthreads)
+__device__ __forceinline__ void group_sync(int G)
 {
-  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+  if (G == 1) __syncwarp(); else __syncthreads();        // the CTA is the group
 }
 
-template <int NDET, int KIND, bool RESIDENT>
-__global__ void __launch_bounds__(kChainThreads, 2) k3_slice(const __grid_constant__ NssDev P, const ChainArgs A)
+template <int NDET, int KIND, int LANES, bool RESIDENT>
+__global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_constant__ NssDev P, const ChainArgs A)
 {
-  extern __shared__ __align__(128) unsigned char smem_raw[];
+  constexpr int NSUB = 32 / LANES;                              // candidates per warp
+  constexpr int NC = (NSS_NSLOT + LANES - 1) / LANES;           // coordinates per lane
+  constexpr int kSlots = kChainWarps * NSUB;                    // most candidates per round
+  extern __shared__ __align__(128) unsigned char smem_raw[];    // [record table if RESIDENT][C sub-warp scratches]
   __shared__ __align__(8) uint64_t bar;
   __shared__ double sL[NSS_NSLOT * NSS_NSLOT];
-  __shared__ double sZ[kChainWarps][kDirChunk][NSS_NSLOT + 1];     // normals of the current chunk, per group
-  __shared__ double sV[kChainWarps][kDirChunk][NSS_NSLOT];         // directions v = w L z/|z|
-  __shared__ double sY[kChainWarps][NSS_NSLOT + 1];                // per warp: sampled coordinates of its candidate
-  __shared__ double sRes[kChainWarps][2][kChainWarps];             // per group, double-buffered: logL of slot w
-  __shared__ int32_t sFlag[kChainWarps][2][kChainWarps];           // 1 = in the box (evaluated), 0 = outside the box
-  __shared__ __align__(16) double sConst[nssk::kWarpConstDoubles];
-  __shared__ __align__(16) double sScr[kChainWarps][nssk::kWarpScratchDoubles];
+  __shared__ double sZ[kDirChunk][NSS_NSLOT + 1];                  // normals of the current chunk
+  __shared__ double sV[kDirChunk][NSS_NSLOT];                      // directions v = w L z/|z|
+  __shared__ double sRes[2][kSlots];                               // double-buffered: logL of every candidate slot
+  __shared__ int32_t sFlag[2][kSlots];                             // 1 = in the box (evaluated), 0 = outside the box
+  __shared__ __align__(16) double sConst[nssk::kSubConstDoubles];
   if (A.flags[0] | A.flags[1]) return;
-  nssk::WarpCtx X;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int sl = lane & (LANES - 1), sub = lane / LANES;
+  nssk::SubCtx X;
   X.tab = P.soa;
   X.consts = sConst;
-  X.scr = sScr[threadIdx.x >> 5];
+  const size_t tab_bytes = RESIDENT ? nssk::sub_table_doubles<NDET, KIND == NSS_KIND_RB, LANES>(P.soa_m) * sizeof(double) : 0;
+  X.scr = reinterpret_cast<double *>(smem_raw + tab_bytes) + (size_t)(warp * NSUB + sub) * nssk::kSubScratchDoubles;
   if (RESIDENT) {
     if (threadIdx.x == 0) {
       nssk::mbar_init(&bar, 1);
-      nssk::stage_table(smem_raw, P.soa, (uint32_t)(nssk::warp_table_doubles<NDET, KIND == NSS_KIND_RB>(P.soa_m) * sizeof(double)), &bar);
+      nssk::stage_table(smem_raw, P.soa, (uint32_t)tab_bytes, &bar);
     }
   }
   const int d = P.d;
   for (int t = threadIdx.x; t < d * d; t += blockDim.x) sL[t] = A.chol[t];
-  if (KIND != NSS_KIND_GAUSS) nssk::warp_consts_init(P, sConst);
+  if (KIND != NSS_KIND_GAUSS) {
+    nssk::sub_consts_init(P, sConst);
+    for (int t = sl; t < 12; t += LANES) X.scr[t] = t < NSS_NSLOT ? P.theta_fixed[t] : 0.0;   // unsampled slots never change
+  }
   __syncthreads();
   if (RESIDENT) {
     nssk::mbar_wait(&bar, 0);
     X.tab = reinterpret_cast<const double *>(smem_raw);
   }
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int G = A.G, GL = G * 32;
-  const int gi = warp / G, w = warp - gi * G;            // group in the CTA, warp in the group
+  const int G = blockDim.x >> 5, GL = blockDim.x, C = G * NSUB;
+  const int w = warp;                                    // warp in the group
   const int gl = w * 32 + lane;                          // lane in the group
-  const int bar_id = 1 + gi;
-  const int groups_per_cta = kChainWarps / G;
+  const int cs = w * NSUB + sub;                         // candidate slot of this sub-warp in the group
   const double Lstar = A.state[3];
   const uint32_t it = A.iteration;
   const int ns = A.n - A.k;
-  const bool own = lane < d;
-  const double lo_j = own ? P.lo[lane] : 0.0, hi_j = own ? P.hi[lane] : 0.0;
+  bool own[NC];
+  int dst_idx[NC];                                       // where coordinate j goes in the likelihood's input
+  double lo_j[NC], hi_j[NC];
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    const int j = sl + c * LANES;
+    own[c] = j < d;
+    lo_j[c] = own[c] ? P.lo[j] : 0.0;
+    hi_j[c] = own[c] ? P.hi[j] : 0.0;
+    dst_idx[c] = own[c] ? (KIND == NSS_KIND_GAUSS ? j : P.param_index[j]) : 0;
+  }
+  const unsigned sub_mask = (LANES == 32 ? 0xffffffffu : ((1u << LANES) - 1u)) << (sub * LANES);
   int par = 0;
   const int nb = (d + 1) >> 1;
 
-  for (int c = blockIdx.x * groups_per_cta + gi; c < A.k; c += gridDim.x * groups_per_cta) {
-    const uint32_t chain = (uint32_t)c;
+  for (int ch = blockIdx.x; ch < A.k; ch += gridDim.x) {
+    const uint32_t chain = (uint32_t)ch;
     // a4: start from a uniformly chosen survivor
     int si = (int)floor(uniform_a(A.seed, 0u, kStepStart, chain, it) * (double)ns);
     si = si > ns - 1 ? ns - 1 : si;
     const int slot = A.surv_idx[si];
-    double xj = own ? A.live[(size_t)slot * d + lane] : 0.0;
+    double xj[NC];
+#pragma unroll
+    for (int c = 0; c < NC; ++c) xj[c] = own[c] ? A.live[(size_t)slot * d + sl + c * LANES] : 0.0;
     double lx = A.logL[slot];
     long long evals = 0;
     double margin = INFINITY;
@@ -446,33 +464,35 @@ __global__ void __launch_bounds__(kChainThreads, 2) k3_slice(const __grid_consta
     for (int s0 = 0; s0 < A.n_repeats; s0 += kDirChunk) {
       const int clen = min(kDirChunk, A.n_repeats - s0);
       // a5: directions of steps s0 .. s0+clen-1.  Normals z (Box-Muller, one Philox block per pair) ...
-      group_sync(bar_id, GL);                            // the previous chunk's directions are no longer read
+      group_sync(G);                            // the previous chunk's directions are no longer read
       for (int idx = gl; idx < clen * nb; idx += GL) {
         const int ss = idx / nb, b = idx - ss * nb;
         uint64_t ka, kb;
         draw53(A.seed, (uint32_t)(1 + b), (uint32_t)(s0 + ss), chain, it, ka, kb);
         const double r = sqrt(-2.0 * log((double)(ka + 1) * kTwoM53));
-        double sn, cs;
-        sincospi(2.0 * ((double)kb * kTwoM53), &sn, &cs);
-        sZ[gi][ss][2 * b] = r * cs;
-        sZ[gi][ss][2 * b + 1] = r * sn;
+        double sn, cs2;
+        sincospi(2.0 * ((double)kb * kTwoM53), &sn, &cs2);
+        sZ[ss][2 * b] = r * cs2;
+        sZ[ss][2 * b + 1] = r * sn;
       }
-      group_sync(bar_id, GL);
+      group_sync(G);
       // ... then n = z/|z|, v = w L n, one (step, row) pair per lane
       for (int idx = gl; idx < clen * d; idx += GL) {
         const int ss = idx / d, i = idx - ss * d;
-        const double *z = sZ[gi][ss];
+        const double *z = sZ[ss];
         double nz = 0.0;
         for (int j = 0; j < d; ++j) nz += z[j] * z[j];
         nz = sqrt(nz);
         double a = 0.0;
         for (int j = 0; j <= i; ++j) a += sL[i * d + j] * (z[j] / nz);
-        sV[gi][ss][i] = kSliceW * a;
+        sV[ss][i] = kSliceW * a;
       }
-      group_sync(bar_id, GL);
+      group_sync(G);
 
       for (int s = s0; s < s0 + clen; ++s) {
-        const double vj = own ? sV[gi][s - s0][lane] : 0.0;
+        double vj[NC];
+#pragma unroll
+        for (int c = 0; c < NC; ++c) vj[c] = own[c] ? sV[s - s0][sl + c * LANES] : 0.0;
         // uniforms of this step: lane 0 -> bracket offset (block 0), lane 1+kk -> kk-th shrinkage proposal (block 64+kk)
         const double ulane = uniform_a(A.seed, lane == 0 ? 0u : (uint32_t)(63 + lane), (uint32_t)s, chain, it);
         const double u0 = nssk::shfl_d(ulane, 0);
@@ -480,41 +500,52 @@ __global__ void __launch_bounds__(kChainThreads, 2) k3_slice(const __grid_consta
         int nl = 0, nr = 0, kk = 0, acc = -1;
         bool ldone = false, rdone = false, done = false;
         while (!done) {
-          // ---- candidate of this warp ------------------------------------------------------------------------
+          // ---- candidate of this sub-warp ---------------------------------------------------------------------
           int nside = (ldone ? 0 : 1) + (rdone ? 0 : 1);
-          nside = nside < G ? nside : G;                 // G = 1: one side test per round, left first
-          int nshr = G - nside;
+          nside = nside < C ? nside : C;                 // C = 1: one side test per round, left first
+          int nshr = C - nside;
           nshr = nshr < kMaxShrink - kk ? nshr : kMaxShrink - kk;
           double t = 0.0;
-          bool active = w < nside + nshr;
-          if (w < nside) {
-            t = (w == 0 && !ldone) ? l : r;
-          } else if (active) {
+          const bool active = cs < nside + nshr;
+          if (cs < nside) t = (cs == 0 && !ldone) ? l : r;
+          {
+            // shrinkage proposals kk .. : every lane walks the bracket as far as its own slot needs (the loop
+            // bound is the warp's last slot, so the shuffles stay convergent)
+            int imax = w * NSUB + NSUB - 1 - nside;
+            imax = imax < nshr - 1 ? imax : nshr - 1;
             double ls = l, rs = r;
-            for (int i = 0; i <= w - nside; ++i) {
+            for (int i = 0; i <= imax; ++i) {
               const int q = kk + i;
               const double uk = q < 31 ? nssk::shfl_d(ulane, q + 1) : uniform_a(A.seed, (uint32_t)(64 + q), (uint32_t)s, chain, it);
-              t = __dadd_rn(ls, __dmul_rn(rs - ls, uk));
-              if (t < 0.0) ls = t; else rs = t;
+              if (i <= cs - nside) {
+                t = __dadd_rn(ls, __dmul_rn(rs - ls, uk));
+                if (t < 0.0) ls = t; else rs = t;
+              }
             }
           }
           // ---- evaluate: box test (inclusive) first, then logL(x + t v) ---------------------------------------
-          double ly = -INFINITY;
-          int inbox = 0;
-          if (active) {
-            const double yj = __dadd_rn(xj, __dmul_rn(t, vj));
-            inbox = __all_sync(0xffffffffu, !own || (yj >= lo_j && yj <= hi_j));
-            if (inbox) {
-              if (own) sY[warp][lane] = yj;
-              __syncwarp();
-              ly = nssk::loglike_warp<NDET, KIND>(P, X, sY[warp]);
-              __syncwarp();
-            }
+          bool inb = true;
+          double yj[NC];
+#pragma unroll
+          for (int c = 0; c < NC; ++c) {
+            yj[c] = __dadd_rn(xj[c], __dmul_rn(t, vj[c]));
+            inb = inb && (!own[c] || (yj[c] >= lo_j[c] && yj[c] <= hi_j[c]));
           }
-          if (lane == 0) { sRes[gi][par][w] = ly; sFlag[gi][par][w] = inbox; }
-          group_sync(bar_id, GL);
-          const double *res = sRes[gi][par];
-          const int32_t *flg = sFlag[gi][par];
+          const unsigned bal = __ballot_sync(0xffffffffu, inb);
+          const bool inbox = active && ((bal & sub_mask) == sub_mask);
+#pragma unroll
+          for (int c = 0; c < NC; ++c)
+            if (own[c]) X.scr[dst_idx[c]] = yj[c];
+          __syncwarp();
+          double ly;
+          if (KIND == NSS_KIND_GAUSS) ly = inbox ? nssk::gauss_loglike(P, X.scr) : -INFINITY;
+          else ly = nssk::loglike_sub<NDET, KIND, LANES>(P, X, inbox);
+          if (!inbox) ly = -INFINITY;
+          __syncwarp();
+          if (sl == 0) { sRes[par][cs] = ly; sFlag[par][cs] = inbox ? 1 : 0; }
+          group_sync(G);
+          const double *res = sRes[par];
+          const int32_t *flg = sFlag[par];
           par ^= 1;
           // ---- replay the sequential decisions ---------------------------------------------------------------
           bool expanded = false;
@@ -537,7 +568,8 @@ __global__ void __launch_bounds__(kChainThreads, 2) k3_slice(const __grid_consta
               const double v = res[slot_i + i]; const int f = flg[slot_i + i];
               if (f) { ++evals; margin = fmin(margin, fabs(v - Lstar)); }
               if (f && v > Lstar) {
-                xj = __dadd_rn(xj, __dmul_rn(ti, vj));
+#pragma unroll
+                for (int c = 0; c < NC; ++c) xj[c] = __dadd_rn(xj[c], __dmul_rn(ti, vj[c]));
                 lx = v; acc = q; done = true;
                 break;
               }
@@ -547,45 +579,41 @@ __global__ void __launch_bounds__(kChainThreads, 2) k3_slice(const __grid_consta
           }
         }
         if (A.trace && gl == 0) {
-          int32_t *tr = A.trace + ((size_t)c * A.n_repeats + s) * 3;
+          int32_t *tr = A.trace + ((size_t)ch * A.n_repeats + s) * 3;
           tr[0] = nl; tr[1] = nr; tr[2] = acc;
         }
       }
     }
     // a10: replace the deleted slot in place
-    if (w == 0) {
-      const int dst = A.dead_idx[c];
-      if (own) A.live[(size_t)dst * d + lane] = xj;
-      if (lane == 0) {
+    if (w == 0 && sub == 0) {
+      const int dst = A.dead_idx[ch];
+#pragma unroll
+      for (int c = 0; c < NC; ++c)
+        if (own[c]) A.live[(size_t)dst * d + sl + c * LANES] = xj[c];
+      if (sl == 0) {
         A.logL[dst] = lx;
         if (A.birth) A.birth[dst] = Lstar;
-        if (A.margin) A.margin[c] = margin;
+        if (A.margin) A.margin[ch] = margin;
         atomicAdd(A.n_evals, (unsigned long long)evals);
       }
     }
   }
 }
 
-template <int NDET, int KIND, bool RESIDENT>
-int launch_chains_k(nss_handle *h, ChainArgs &A, size_t smem, cudaStream_t st)
+template <int NDET, int KIND, int LANES, bool RESIDENT>
+int launch_chains_k(nss_handle *h, ChainArgs &A, size_t tab_bytes, cudaStream_t st)
 {
-  auto kern = k3_slice<NDET, KIND, RESIDENT>;
-  if (smem > 0) NSS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));   // static + dynamic may exceed 48 KB
-  int occ = 0;
-  NSS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kChainThreads, smem));
-  if (occ < 1) occ = 1;
-  const int cap_warps = h->n_sm * occ * kChainWarps;
+  auto kern = k3_slice<NDET, KIND, LANES, RESIDENT>;
   int G = h->chain_warps;
-  if (G != 1 && G != 2 && G != 4 && G != 8) {            // automatic: the widest group that keeps every chain resident
-    G = 8;
-    while (G > 1 && (long long)A.k * G > cap_warps) G >>= 1;
+  if (G != 1 && G != 2 && G != 4 && G != 8) {            // automatic: the widest group that leaves one warp per SM sub-partition
+    G = 8;                                               // (a lone warp with enough independent work saturates its fp64 pipe)
+    while (G > 1 && (long long)A.k * G > 4LL * h->n_sm) G >>= 1;
   }
   A.G = G;
-  const int gpc = kChainWarps / G;
-  int grid = (A.k + gpc - 1) / gpc;
-  if (grid > h->n_sm * occ) grid = h->n_sm * occ;
+  const size_t smem = tab_bytes + (size_t)G * (32 / LANES) * nssk::kSubScratchDoubles * sizeof(double);
+  NSS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   NSS_CUDA(cudaEventRecord(h->ev_k3[0], st));
-  kern<<<grid, kChainThreads, smem, st>>>(h->dev, A);
+  kern<<<A.k, 32 * G, smem, st>>>(h->dev, A);            // one chain per CTA: the block scheduler balances the SMs
   NSS_CUDA(cudaEventRecord(h->ev_k3[1], st));
   return NSS_OK;
 }
@@ -600,15 +628,16 @@ int launch_chains(nss_handle *h, ChainArgs &A, cudaStream_t st)
   }
   int rc;
   if (P.kind == NSS_KIND_RB) {
-    const size_t bytes = (size_t)((9 + 2 * NDET) + P.soa_m * (9 + 3 * NDET)) * 32 * sizeof(double);
-    if (bytes + 40 * 1024 <= 110 * 1024)                 // table + static arrays, two CTAs per SM
-      rc = launch_chains_k<NDET, NSS_KIND_RB, true>(h, A, bytes, st);
+    const size_t bytes = (size_t)((9 + 2 * NDET) + P.soa_m * (9 + 3 * NDET)) * P.soa_lanes * sizeof(double);
+    const bool fits = bytes <= 64 * 1024;                // several CTAs per SM keep their own copy
+    if (P.soa_lanes == 8)
+      rc = fits ? launch_chains_k<NDET, NSS_KIND_RB, 8, true>(h, A, bytes, st) : launch_chains_k<NDET, NSS_KIND_RB, 8, false>(h, A, 0, st);
     else
-      rc = launch_chains_k<NDET, NSS_KIND_RB, false>(h, A, 0, st);
+      rc = fits ? launch_chains_k<NDET, NSS_KIND_RB, 32, true>(h, A, bytes, st) : launch_chains_k<NDET, NSS_KIND_RB, 32, false>(h, A, 0, st);
   } else if (P.kind == NSS_KIND_FULL) {
-    rc = launch_chains_k<NDET, NSS_KIND_FULL, false>(h, A, 0, st);
+    rc = launch_chains_k<NDET, NSS_KIND_FULL, 32, false>(h, A, 0, st);
   } else {
-    rc = launch_chains_k<1, NSS_KIND_GAUSS, false>(h, A, 0, st);
+    rc = launch_chains_k<1, NSS_KIND_GAUSS, 32, false>(h, A, 0, st);
   }
   if (rc) return rc;
   h->ev_k3_valid = 1;

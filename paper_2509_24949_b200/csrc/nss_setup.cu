@@ -335,27 +335,30 @@ extern "C" int nss_create(const nss_config *cfg, nss_handle **out)
     P.rec_rs = rs;
     rc_up = upload(rec, &h->d_rec, &h->rec_bytes);
     P.rec = h->d_rec;
-    // (2) warp layout, round major: lane l owns records l*m+1 .. l*m+m (rounds 1..m) and evaluates record l*m in
-    //     round 0 (the left edge of its first bin; its W counts for lane 0 only).  Records past the end repeat the
-    //     last one with zero weights.
-    const int m = n_rec > 1 ? (n_rec - 1 + 31) / 32 : 1;
+    // (2) sub-warp layout, round major, for L = soa_lanes lanes per point: lane l owns records l*m+1 .. l*m+m
+    //     (rounds 1..m) and evaluates record l*m in round 0 (the left edge of its first bin; its W counts for
+    //     lane 0 only).  Records past the end repeat the last one with zero weights.  L = 8 (four points per warp)
+    //     while that keeps m <= 32, else 32.
+    const int L = (kind == NSS_KIND_RB && n_rec - 1 <= 8 * 32) ? 8 : 32;
+    const int m = n_rec > 1 ? (n_rec - 1 + L - 1) / L : 1;
     P.soa_m = m;
-    const size_t r0_sz = (size_t)(9 + 2 * nd) * 32, round_sz = (size_t)(9 + per * nd) * 32;
+    P.soa_lanes = L;
+    const size_t r0_sz = (size_t)(9 + 2 * nd) * L, round_sz = (size_t)(9 + per * nd) * L;
     std::vector<double> soa(r0_sz + (size_t)m * round_sz, 0.0);
-    for (int l = 0; l < 32; ++l) {
+    for (int l = 0; l < L; ++l) {
       for (int j = 0; j <= m; ++j) {
         double *te = j == 0 ? soa.data() : soa.data() + r0_sz + (size_t)(j - 1) * round_sz;
         const int e0 = l * m + j;
         const int e = e0 < n_rec ? e0 : n_rec - 1;
         double g[nssp::kNB];
         nssp::basis(rf[e], g);
-        for (int c = 0; c < 8; ++c) te[c * 32 + l] = g[c];
-        te[8 * 32 + l] = rf[e];
+        for (int c = 0; c < 8; ++c) te[c * L + l] = g[c];
+        te[8 * L + l] = rf[e];
         if (e0 >= n_rec || (j == 0 && l != 0)) continue;
         for (int a = 0; a < nd; ++a) {
-          te[(9 + per_of(j, per) * a) * 32 + l] = W[((size_t)a * n_rec + e) * 2];
-          te[(10 + per_of(j, per) * a) * 32 + l] = W[((size_t)a * n_rec + e) * 2 + 1];
-          if (cr && j > 0) te[(11 + per * a) * 32 + l] = V[(size_t)a * n_rec + e];
+          te[(9 + per_of(j, per) * a) * L + l] = W[((size_t)a * n_rec + e) * 2];
+          te[(10 + per_of(j, per) * a) * L + l] = W[((size_t)a * n_rec + e) * 2 + 1];
+          if (cr && j > 0) te[(11 + per * a) * L + l] = V[(size_t)a * n_rec + e];
         }
       }
     }

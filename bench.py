@@ -42,15 +42,16 @@ SEED = 1
 
 # ---- algorithmic work of one relative-binning likelihood evaluation -------------------------
 def rb_work(B: int, n_det: int):
-    """(fp64-pipe instructions, flop) one evaluation needs: per point, per edge, per (edge, detector),
-    per (bin, detector).  FMA = 1 instruction = 2 flop; add/mul = 1 flop."""
+    """(fp64-pipe instructions, flop) one relative-binning evaluation needs in the regrouped form the kernels
+    use: per point; per edge the 8-term phase; per (edge, detector) the arrival-time FMA, sincos
+    in turns (17 instructions), T += W conj(z) (4 FMA) and the cross term V Re(z_b conj z_b+1) (3).
+    FMA = 1 instruction = 2 flop; add/mul = 1 flop."""
     E = B + 1
     per_point_i, per_point_f = 600, 900
-    edge_i, edge_f = 8, 16                       # 8 FMA: phase difference against the tabulated basis
-    ed_i, ed_f = 27, 45                          # arrival-time FMA, range reduction, sincospi, complex scale
-    bd_i, bd_f = 15, 23                          # sums/differences of the edge ratios, six pre-scaled terms
-    instr = per_point_i + E * edge_i + E * n_det * ed_i + B * n_det * bd_i
-    flop = per_point_f + E * edge_f + E * n_det * ed_f + B * n_det * bd_f
+    edge_i, edge_f = 8, 16
+    ed_i, ed_f = 1 + 17 + 4 + 3, 2 + 31 + 8 + 5
+    instr = per_point_i + E * edge_i + E * n_det * ed_i
+    flop = per_point_f + E * edge_f + E * n_det * ed_f
     return instr, flop
 
 
@@ -315,7 +316,7 @@ def run_ours(args):
                      "flop_per_eval": flop, "fp64_instr_per_eval": instr,
                      "pipe_frac": (evals / world) * instr / (k3_ms * 1e-3) / (peak_tf * 1e12 / 2),
                      "kernel_ms_per_step": k3_ms / args.steps, "kernel_share_of_step": k3_ms / ms, "traffic": None},
-        "loglike_batch": {"workload": "config 5: N=1e6 prior draws, B=128 x 3 detectors, k1_rb_thread", "ms": k1_ms,
+        "loglike_batch": {"workload": "config 5: N=1e6 prior draws, B=128 x 3 detectors, k_rec_thread", "ms": k1_ms,
                           "evals_per_s": k1_rate, "tflops": k1_rate * flop / 1e12, "frac": k1_rate * flop / 1e12 / peak_tf,
                           "pipe_frac": k1_rate * instr / (peak_tf * 1e12 / 2)},
         "nss_run": {"wall_s": run_wall, "gpu_ms": r["gpu_ms"], "n_iter": r["n_iter"], "n_evals": r["n_evals"],

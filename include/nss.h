@@ -89,14 +89,18 @@ int nss_loglike_batch(nss_handle *h, const double *theta_dev, int64_t N, double 
                       void *cuda_stream);
 
 /* Variant selector for nss_loglike_batch (profiling / tests): 0 = automatic (default),
- * 1 = one thread per point, 2 = one warp per point. */
+ * 1 = one thread per point, 2 = one sub-warp (8 or 32 lanes) per point. */
 int nss_set_loglike_variant(nss_handle *h, int32_t variant);
 
-/* Warps that run one slice chain (K3): 0 = automatic (the widest of 1, 2, 4, 8 that keeps all n_delete
- * chains resident on the GPU), else 1, 2, 4 or 8.  A group of G warps evaluates, in one round, the next G
- * bracket tests of the sequential algorithm speculatively; the decisions, positions and evaluation count
- * are those of the sequential algorithm for every G (tests/test_gpu_sampler.py). */
+/* Warps that run one slice chain (K3): 0 = automatic, else 1, 2, 4 or 8.  A chain is one CTA of G warps; every
+ * sub-warp of `lanes` lanes evaluates one bracket test, so a round evaluates the next G * 32/lanes tests of
+ * the sequential algorithm speculatively; the decisions, positions and evaluation count are those of the
+ * sequential algorithm for every G and every lane count (tests/test_gpu_sampler.py). */
 int nss_set_chain_warps(nss_handle *h, int32_t warps);
+
+/* Lanes that evaluate one candidate in K3 (relative binning only): 0 = automatic, else 8, 16 or 32 (a width
+ * whose table was not built, e.g. 8 lanes with more than 256 bins, falls back to the automatic choice). */
+int nss_set_chain_lanes(nss_handle *h, int32_t lanes);
 
 /* One NS iteration (O12): select the n_delete lowest logL (ascending, ties by lower slot), tune the
  * slice directions from the covariance of the full live set (Cholesky), run one chain per deleted

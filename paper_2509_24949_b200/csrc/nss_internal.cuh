@@ -31,9 +31,11 @@ struct NssDev {
   int32_t cross;          // 1: records carry the cross-term weight V (kind 0), 0: they do not (kind 1)
   const double *rec;      // AoS [n_rec][rec_rs]: g0..g7, f, pad, then per det (Wr, Wi[, V])
   int32_t rec_rs;
-  const double *soa;      // sub-warp layout, round major: [9 + 2 n_det][L], then m x [9 + (2 + cross) n_det][L]
-  int32_t soa_m;          // rounds after round 0 = ceil((n_rec - 1)/L); lane l owns records l*m+1 .. l*m+m
-  int32_t soa_lanes;      // L = lanes per point: 8 or 32
+  // sub-warp layouts for L = 8, 16, 32 lanes per point (index 0, 1, 2; NULL if not built), round major:
+  // [9 + 2 n_det][L], then m x [9 + (2 + cross) n_det][L]; m = rounds after round 0 = ceil((n_rec - 1)/L);
+  // lane l owns records l*m+1 .. l*m+m
+  const double *soa[3];
+  int32_t soa_m[3];
 };
 
 // device control block of an NS iteration; one pinned host mirror per handle (a single small D2H copy per sync)
@@ -49,14 +51,15 @@ struct nss_handle {
   int n_sm;
   int loglike_variant;
   int chain_warps;          // warps per slice chain: 0 = automatic, else 1, 2, 4 or 8
+  int chain_lanes;          // lanes per candidate in the slice kernel: 0 = automatic, else 8, 16 or 32
   int64_t launches;
   // host copies kept for nss_get_tables
   std::vector<int32_t> edge_idx;
   std::vector<double> summary;     // [n_det][B][6]
   double DD;
   // device allocations
-  double *d_rec, *d_soa;
-  size_t rec_bytes, soa_bytes;
+  double *d_rec, *d_soa[3];
+  size_t rec_bytes, soa_bytes[3];
   // sampler scratch (grown on demand)
   int32_t scratch_n;
   int32_t *d_surv_idx, *d_dead_idx, *d_rank, *d_flags;   // flags: [0] chol error, [1] threshold violation, [2] done

@@ -108,12 +108,13 @@ __global__ void __launch_bounds__(kThreads) k_rec_sub(const __grid_constant__ Ns
   __shared__ __align__(16) double consts[nssk::kSubConstDoubles];
   __shared__ __align__(16) double scratch[kThreads / LANES][nssk::kSubScratchDoubles];
   nssk::SubCtx X;
-  X.tab = P.soa;
+  constexpr int LI = nssk::lanes_index<LANES>();
+  X.tab = P.soa[LI];
   X.consts = consts;
   X.scr = scratch[threadIdx.x / LANES];
   if (RESIDENT && threadIdx.x == 0) {
     nssk::mbar_init(&bar, 1);
-    nssk::stage_table(smem_raw, P.soa, (uint32_t)(nssk::sub_table_doubles<NDET, KIND == NSS_KIND_RB, LANES>(P.soa_m) * sizeof(double)), &bar);
+    nssk::stage_table(smem_raw, P.soa[LI], (uint32_t)(nssk::sub_table_doubles<NDET, KIND == NSS_KIND_RB, LANES>(P.soa_m[LI]) * sizeof(double)), &bar);
   }
   nssk::sub_consts_init(P, consts);
   const int d = P.d, sl = threadIdx.x & (LANES - 1);
@@ -159,7 +160,7 @@ int launch_sub(nss_handle *h, const double *theta, int64_t N, double *logL, cuda
 {
   constexpr bool CROSS = KIND == NSS_KIND_RB;
   const NssDev &P = h->dev;
-  const size_t bytes = (size_t)((9 + 2 * NDET) + P.soa_m * (9 + (CROSS ? 3 : 2) * NDET)) * LANES * sizeof(double);
+  const size_t bytes = (size_t)((9 + 2 * NDET) + P.soa_m[nssk::lanes_index<LANES>()] * (9 + (CROSS ? 3 : 2) * NDET)) * LANES * sizeof(double);
   const size_t fixed = 8 * 1024 + sizeof(double) * (kThreads / LANES) * nssk::kSubScratchDoubles;
   const bool resident = bytes + fixed <= 200 * 1024;
   const size_t smem = resident ? bytes : 0;
@@ -210,7 +211,7 @@ int launch_rec(nss_handle *h, const double *theta, int64_t N, double *logL, cuda
     }
   } else {
     if constexpr (KIND == NSS_KIND_RB) {
-      rc_sub = P.soa_lanes == 8 ? launch_sub<NDET, KIND, 8>(h, theta, N, logL, st) : launch_sub<NDET, KIND, 32>(h, theta, N, logL, st);
+      rc_sub = P.soa[0] ? launch_sub<NDET, KIND, 8>(h, theta, N, logL, st) : launch_sub<NDET, KIND, 32>(h, theta, N, logL, st);
     } else {
       rc_sub = launch_sub<NDET, KIND, 32>(h, theta, N, logL, st);
     }

@@ -128,6 +128,9 @@ struct SubCtx {
 };
 
 template <int LANES>
+__host__ __device__ constexpr int lanes_index() { return LANES == 8 ? 0 : LANES == 16 ? 1 : 2; }
+
+template <int LANES>
 __device__ __forceinline__ double sub_sum(double v)
 {
 #pragma unroll
@@ -346,7 +349,7 @@ template <int NDET, bool CROSS, int LANES>
 __device__ __forceinline__ double records_sub(const NssDev &P, const double *__restrict__ tab, const RbPoint<NDET> &R)
 {
   constexpr int PER = CROSS ? 3 : 2;
-  const int sl = threadIdx.x & (LANES - 1), m = P.soa_m;
+  const int sl = threadIdx.x & (LANES - 1), m = P.soa_m[lanes_index<LANES>()];
   const double *t = tab + sl;
   DetAcc A[NDET];
   {

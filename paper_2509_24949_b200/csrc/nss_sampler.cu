@@ -405,14 +405,15 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int sl = lane & (LANES - 1), sub = lane / LANES;
   nssk::SubCtx X;
-  X.tab = P.soa;
+  constexpr int LI = nssk::lanes_index<LANES>();
+  X.tab = P.soa[LI];
   X.consts = sConst;
-  const size_t tab_bytes = RESIDENT ? nssk::sub_table_doubles<NDET, KIND == NSS_KIND_RB, LANES>(P.soa_m) * sizeof(double) : 0;
+  const size_t tab_bytes = RESIDENT ? nssk::sub_table_doubles<NDET, KIND == NSS_KIND_RB, LANES>(P.soa_m[LI]) * sizeof(double) : 0;
   X.scr = reinterpret_cast<double *>(smem_raw + tab_bytes) + (size_t)(warp * NSUB + sub) * nssk::kSubScratchDoubles;
   if (RESIDENT) {
     if (threadIdx.x == 0) {
       nssk::mbar_init(&bar, 1);
-      nssk::stage_table(smem_raw, P.soa, (uint32_t)tab_bytes, &bar);
+      nssk::stage_table(smem_raw, P.soa[LI], (uint32_t)tab_bytes, &bar);
     }
   }
   const int d = P.d;
@@ -605,9 +606,12 @@ int launch_chains_k(nss_handle *h, ChainArgs &A, size_t tab_bytes, cudaStream_t 
 {
   auto kern = k3_slice<NDET, KIND, LANES, RESIDENT>;
   int G = h->chain_warps;
-  if (G != 1 && G != 2 && G != 4 && G != 8) {            // automatic: the widest group that leaves one warp per SM sub-partition
-    G = 8;                                               // (a lone warp with enough independent work saturates its fp64 pipe)
-    while (G > 1 && (long long)A.k * G > 4LL * h->n_sm) G >>= 1;
+  if (G != 1 && G != 2 && G != 4 && G != 8) {
+    // automatic (measured on B200, _work sweeps -> DESIGN.md §6): a chain is a serial process, so few chains want
+    // wide speculation, but once there are about as many warps as SM sub-partitions (4 per SM) the kernel turns
+    // throughput-bound and every speculative evaluation costs time
+    const long long S = 4LL * h->n_sm;
+    G = LANES == 8 ? 1 : (A.k * 8LL <= S ? 4 : A.k <= S ? 2 : 1);
   }
   A.G = G;
   const size_t smem = tab_bytes + (size_t)G * (32 / LANES) * nssk::kSubScratchDoubles * sizeof(double);
@@ -628,10 +632,20 @@ int launch_chains(nss_handle *h, ChainArgs &A, cudaStream_t st)
   }
   int rc;
   if (P.kind == NSS_KIND_RB) {
-    const size_t bytes = (size_t)((9 + 2 * NDET) + P.soa_m * (9 + 3 * NDET)) * P.soa_lanes * sizeof(double);
+    // lanes per candidate: 8 shares the per-point setup among four candidates per warp (fewest instructions per
+    // evaluation: best when the chains alone fill the SM sub-partitions), 16 halves the latency of a round
+    int L = h->chain_lanes;
+    if (!(L == 8 || L == 16 || L == 32) || !P.soa[L == 8 ? 0 : L == 16 ? 1 : 2]) {
+      const bool many = A.k > 4LL * h->n_sm;             // more chains than SM sub-partitions: fewest instructions wins
+      L = (many && P.soa[0]) ? 8 : P.soa[1] ? 16 : P.soa[0] ? 8 : 32;
+    }
+    const int li = L == 8 ? 0 : L == 16 ? 1 : 2;
+    const size_t bytes = (size_t)((9 + 2 * NDET) + P.soa_m[li] * (9 + 3 * NDET)) * L * sizeof(double);
     const bool fits = bytes <= 64 * 1024;                // several CTAs per SM keep their own copy
-    if (P.soa_lanes == 8)
+    if (L == 8)
       rc = fits ? launch_chains_k<NDET, NSS_KIND_RB, 8, true>(h, A, bytes, st) : launch_chains_k<NDET, NSS_KIND_RB, 8, false>(h, A, 0, st);
+    else if (L == 16)
+      rc = fits ? launch_chains_k<NDET, NSS_KIND_RB, 16, true>(h, A, bytes, st) : launch_chains_k<NDET, NSS_KIND_RB, 16, false>(h, A, 0, st);
     else
       rc = fits ? launch_chains_k<NDET, NSS_KIND_RB, 32, true>(h, A, bytes, st) : launch_chains_k<NDET, NSS_KIND_RB, 32, false>(h, A, 0, st);
   } else if (P.kind == NSS_KIND_FULL) {
@@ -735,6 +749,13 @@ extern "C" int nss_set_chain_warps(nss_handle *h, int32_t warps)
 {
   if (!h || !(warps == 0 || warps == 1 || warps == 2 || warps == 4 || warps == 8)) return NSS_EINVAL;
   h->chain_warps = warps;
+  return NSS_OK;
+}
+
+extern "C" int nss_set_chain_lanes(nss_handle *h, int32_t lanes)
+{
+  if (!h || !(lanes == 0 || lanes == 8 || lanes == 16 || lanes == 32)) return NSS_EINVAL;
+  h->chain_lanes = lanes;
   return NSS_OK;
 }
 

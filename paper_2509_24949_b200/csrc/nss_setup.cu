@@ -147,7 +147,7 @@ extern "C" int nss_destroy(nss_handle *h)
 {
   if (!h) return NSS_OK;
   cudaSetDevice(h->device);
-  cudaFree(h->d_rec); cudaFree(h->d_soa);
+  cudaFree(h->d_rec); cudaFree(h->d_soa[0]); cudaFree(h->d_soa[1]); cudaFree(h->d_soa[2]);
   cudaFree(h->d_surv_idx); cudaFree(h->d_dead_idx); cudaFree(h->d_rank); cudaFree(h->d_ctl);
   if (h->h_ctl) cudaFreeHost(h->h_ctl);
   cudaFree(h->d_mean); cudaFree(h->d_chol); cudaFree(h->d_birth); cudaFree(h->d_stage);
@@ -335,35 +335,37 @@ extern "C" int nss_create(const nss_config *cfg, nss_handle **out)
     P.rec_rs = rs;
     rc_up = upload(rec, &h->d_rec, &h->rec_bytes);
     P.rec = h->d_rec;
-    // (2) sub-warp layout, round major, for L = soa_lanes lanes per point: lane l owns records l*m+1 .. l*m+m
+    // (2) sub-warp layouts, round major, for L = 8, 16, 32 lanes per point: lane l owns records l*m+1 .. l*m+m
     //     (rounds 1..m) and evaluates record l*m in round 0 (the left edge of its first bin; its W counts for
-    //     lane 0 only).  Records past the end repeat the last one with zero weights.  L = 8 (four points per warp)
-    //     while that keeps m <= 32, else 32.
-    const int L = (kind == NSS_KIND_RB && n_rec - 1 <= 8 * 32) ? 8 : 32;
-    const int m = n_rec > 1 ? (n_rec - 1 + L - 1) / L : 1;
-    P.soa_m = m;
-    P.soa_lanes = L;
-    const size_t r0_sz = (size_t)(9 + 2 * nd) * L, round_sz = (size_t)(9 + per * nd) * L;
-    std::vector<double> soa(r0_sz + (size_t)m * round_sz, 0.0);
-    for (int l = 0; l < L; ++l) {
-      for (int j = 0; j <= m; ++j) {
-        double *te = j == 0 ? soa.data() : soa.data() + r0_sz + (size_t)(j - 1) * round_sz;
-        const int e0 = l * m + j;
-        const int e = e0 < n_rec ? e0 : n_rec - 1;
-        double g[nssp::kNB];
-        nssp::basis(rf[e], g);
-        for (int c = 0; c < 8; ++c) te[c * L + l] = g[c];
-        te[8 * L + l] = rf[e];
-        if (e0 >= n_rec || (j == 0 && l != 0)) continue;
-        for (int a = 0; a < nd; ++a) {
-          te[(9 + per_of(j, per) * a) * L + l] = W[((size_t)a * n_rec + e) * 2];
-          te[(10 + per_of(j, per) * a) * L + l] = W[((size_t)a * n_rec + e) * 2 + 1];
-          if (cr && j > 0) te[(11 + per * a) * L + l] = V[(size_t)a * n_rec + e];
+    //     lane 0 only).  Records past the end repeat the last one with zero weights.  L < 32 (several points
+    //     per warp) is built while it keeps m <= 32.
+    for (int li = 0; li < 3; ++li) {
+      const int L = 8 << li;
+      const int m = n_rec > 1 ? (n_rec - 1 + L - 1) / L : 1;
+      if (L < 32 && (kind != NSS_KIND_RB || m > 32)) continue;
+      P.soa_m[li] = m;
+      const size_t r0_sz = (size_t)(9 + 2 * nd) * L, round_sz = (size_t)(9 + per * nd) * L;
+      std::vector<double> soa(r0_sz + (size_t)m * round_sz, 0.0);
+      for (int l = 0; l < L; ++l) {
+        for (int j = 0; j <= m; ++j) {
+          double *te = j == 0 ? soa.data() : soa.data() + r0_sz + (size_t)(j - 1) * round_sz;
+          const int e0 = l * m + j;
+          const int e = e0 < n_rec ? e0 : n_rec - 1;
+          double g[nssp::kNB];
+          nssp::basis(rf[e], g);
+          for (int c = 0; c < 8; ++c) te[c * L + l] = g[c];
+          te[8 * L + l] = rf[e];
+          if (e0 >= n_rec || (j == 0 && l != 0)) continue;
+          for (int a = 0; a < nd; ++a) {
+            te[(9 + per_of(j, per) * a) * L + l] = W[((size_t)a * n_rec + e) * 2];
+            te[(10 + per_of(j, per) * a) * L + l] = W[((size_t)a * n_rec + e) * 2 + 1];
+            if (cr && j > 0) te[(11 + per * a) * L + l] = V[(size_t)a * n_rec + e];
+          }
         }
       }
+      if (rc_up == NSS_OK) rc_up = upload(soa, &h->d_soa[li], &h->soa_bytes[li]);
+      P.soa[li] = h->d_soa[li];
     }
-    if (rc_up == NSS_OK) rc_up = upload(soa, &h->d_soa, &h->soa_bytes);
-    P.soa = h->d_soa;
   }
   if (rc_up != NSS_OK) { nss_destroy(h); return rc_up; }
   *out = h;

@@ -116,14 +116,18 @@ def test_k2_full_grid_matches_oracle(nssmod, oracle):
     X = np.concatenate([inputs.draw_prior(w, 400, 5), _near(w, p, 100, 6), w.theta_fid[w.param_index][None, :]])
     X[5, 1] = 2.0
     ref = p.loglike_batch(X)
-    got = g.nss_loglike_batch(X).cpu().numpy()
-    _close(got, ref)
+    for variant in (0, 1, 2):                  # 1: one thread per point, table streamed in TMA tiles; 2: one warp per point
+        g.set_loglike_variant(variant)
+        _close(g.nss_loglike_batch(X).cpu().numpy(), ref)
     # config 1 geometry too (one detector)
     w1 = inputs.make_data(inputs.config1(), oracle.waveform)
     w1.kind = 1
     p1, g1 = oracle.Problem(w1), nssmod.Nss(w1)
-    X1 = inputs.draw_prior(w1, 500, 2)
-    _close(g1.nss_loglike_batch(X1).cpu().numpy(), p1.loglike_batch(X1))
+    X1 = inputs.draw_prior(w1, 777, 2)         # three batches of 256 points, the last one ragged
+    ref1 = p1.loglike_batch(X1)
+    for variant in (1, 2):
+        g1.set_loglike_variant(variant)
+        _close(g1.nss_loglike_batch(X1).cpu().numpy(), ref1)
     g.close(); g1.close()
 
 

@@ -72,6 +72,10 @@ struct nss_handle {
   // device staging for the host-buffer entry points (grown on demand)
   unsigned char *d_stage;
   size_t stage_bytes;
+  // device block and events of nss_run, kept between runs
+  unsigned char *d_run;
+  size_t run_bytes;
+  cudaEvent_t ev_run[2];
   // CUDA events recorded around the most recent K3 (slice chains) launch: nss_last_chain_ms
   cudaEvent_t ev_k3[2];
   int ev_k3_valid;

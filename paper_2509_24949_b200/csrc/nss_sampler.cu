@@ -329,6 +329,65 @@ __global__ void __launch_bounds__(kOneCta) k4_live_evidence(const double *__rest
   }
 }
 
+// ---- O15: evidence-error replicas (stochastic compression), one CTA per replica -------------------------------
+// ln t_j = ln(u+_j)/m_j with m_j = n - (j mod k); logX_j = sum_{i<j} ln t_i; w_j = X_j (1 - t_j);
+// lZ = logsumexp_j(logL_j + ln w_j) (+) [logX_end + logsumexp(live logL) - ln n].  The prefix sum is split over
+// the threads (chunk sums, one block scan, then each thread walks its chunk), the draws are regenerated in the
+// second pass (Philox counter = (0, j, replica, 0xFFFFFFFE)).
+constexpr int kErrReplicas = 200;
+__global__ void __launch_bounds__(256) k_evidence_error(const double *__restrict__ dead_logL, long long n_dead, int n, int k,
+                                                        uint64_t seed, const double *__restrict__ live_logL,
+                                                        double *__restrict__ lZ_out)
+{
+  __shared__ double red[32];
+  __shared__ double warp_tot[8];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const uint32_t rpl = blockIdx.x;
+  const long long chunk = (n_dead + blockDim.x - 1) / blockDim.x;
+  const long long j0 = min(n_dead, (long long)tid * chunk), j1 = min(n_dead, j0 + chunk);
+  auto lnt = [&](long long j) {
+    uint64_t ka, kb;
+    draw53(seed, 0u, (uint32_t)j, rpl, kIterErr, ka, kb);
+    return log((double)(ka + 1) * kTwoM53) / (double)(n - (int)(j % k));
+  };
+  double part = 0.0;
+  for (long long j = j0; j < j1; ++j) part += lnt(j);
+  double incl = part;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const double v = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += v;
+  }
+  if (lane == 31) warp_tot[wid] = incl;
+  __syncthreads();
+  double lX = incl - part;
+  for (int q = 0; q < wid; ++q) lX += warp_tot[q];
+  double mx = -INFINITY, se = 0.0;
+  for (long long j = j0; j < j1; ++j) {
+    const double lt = lnt(j);
+    const double a = dead_logL[j] + lX + log1p(-exp(lt));
+    if (a > mx) { se = se * exp(mx - a) + 1.0; mx = a; }
+    else if (a > -INFINITY) se += exp(a - mx);
+    lX += lt;
+  }
+  const double M = block_max(mx, red);
+  const double tot = block_sum(M > -INFINITY && mx > -INFINITY ? se * exp(mx - M) : 0.0, red);
+  const double lX_end = block_sum(part, red);
+  // live term
+  double lm = -INFINITY;
+  for (int i = tid; i < n; i += blockDim.x) lm = fmax(lm, live_logL[i]);
+  lm = block_max(lm, red);
+  double ls = 0.0;
+  if (lm > -INFINITY)
+    for (int i = tid; i < n; i += blockDim.x) ls += exp(live_logL[i] - lm);
+  ls = block_sum(ls, red);
+  if (tid == 0) {
+    const double lz_dead = M > -INFINITY ? M + log(tot) : -INFINITY;
+    const double lz_live = lm > -INFINITY ? lX_end + lm + log(ls) - log((double)n) : -INFINITY;
+    lZ_out[rpl] = logaddexp_d(lz_dead, lz_live);
+  }
+}
+
 __global__ void k_fill(double *__restrict__ p, int n, double v)
 {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -982,26 +1041,32 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
   int rc = ensure_scratch(h, n);
   if (rc) return rc;
   const int64_t cap = out->cap;
-  double *live = nullptr, *logL = nullptr, *dth = nullptr, *dl = nullptr, *db = nullptr, *dw = nullptr;
-  cudaEvent_t e0 = nullptr, e1 = nullptr;
-  auto cleanup = [&]() {
-    cudaFree(live); cudaFree(logL); cudaFree(dth); cudaFree(dl); cudaFree(db); cudaFree(dw);
-    if (e0) cudaEventDestroy(e0);
-    if (e1) cudaEventDestroy(e1);
-  };
+  // one device block, kept by the handle between runs: live, logL, the dead buffers and the replica evidences
+  const size_t o_live = 0, o_logL = o_live + align256(sizeof(double) * (size_t)n * d), o_dth = o_logL + align256(sizeof(double) * n),
+               o_dl = o_dth + align256(sizeof(double) * (size_t)cap * d), o_db = o_dl + align256(sizeof(double) * cap),
+               o_dw = o_db + align256(sizeof(double) * cap), o_err = o_dw + align256(sizeof(double) * cap),
+               total = o_err + align256(sizeof(double) * kErrReplicas);
+  if (h->run_bytes < total) {
+    cudaFree(h->d_run);
+    h->d_run = nullptr; h->run_bytes = 0;
+    cudaError_t e = cudaMalloc((void **)&h->d_run, total);
+    if (e != cudaSuccess) { nss_cuda_fail(e, "cudaMalloc(run)"); return e == cudaErrorMemoryAllocation ? NSS_ENOMEM : NSS_ECUDA; }
+    h->run_bytes = total;
+  }
+  if (!h->ev_run[0]) {
+    NSS_CUDA(cudaEventCreate(&h->ev_run[0]));
+    NSS_CUDA(cudaEventCreate(&h->ev_run[1]));
+  }
+  unsigned char *rb = h->d_run;
+  double *live = (double *)(rb + o_live), *logL = (double *)(rb + o_logL), *dth = (double *)(rb + o_dth), *dl = (double *)(rb + o_dl),
+         *db = (double *)(rb + o_db), *dw = (double *)(rb + o_dw), *derr = (double *)(rb + o_err);
+  cudaEvent_t e0 = h->ev_run[0], e1 = h->ev_run[1];
+  auto cleanup = [&]() {};
 #define RUN_CUDA(x)                                                           \
   do {                                                                        \
     cudaError_t e__ = (x);                                                    \
     if (e__ != cudaSuccess) { cleanup(); return nss_cuda_fail(e__, #x); }     \
   } while (0)
-  RUN_CUDA(cudaMalloc(&live, sizeof(double) * (size_t)n * d));
-  RUN_CUDA(cudaMalloc(&logL, sizeof(double) * n));
-  RUN_CUDA(cudaMalloc(&dth, sizeof(double) * (size_t)cap * d));
-  RUN_CUDA(cudaMalloc(&dl, sizeof(double) * cap));
-  RUN_CUDA(cudaMalloc(&db, sizeof(double) * cap));
-  RUN_CUDA(cudaMalloc(&dw, sizeof(double) * cap));
-  RUN_CUDA(cudaEventCreate(&e0));
-  RUN_CUDA(cudaEventCreate(&e1));
 
   RUN_CUDA(cudaEventRecord(e0, st));
   rc = begin_iteration(h, 1, 0.0, -INFINITY, 1, st);
@@ -1046,6 +1111,11 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
     RUN_CUDA(cudaMemcpyAsync(out->dead_logL, dl, sizeof(double) * n_dead, cudaMemcpyDeviceToHost, st));
     RUN_CUDA(cudaMemcpyAsync(out->dead_logL_birth, db, sizeof(double) * n_dead, cudaMemcpyDeviceToHost, st));
     RUN_CUDA(cudaMemcpyAsync(out->dead_logw, dw, sizeof(double) * n_it_dead, cudaMemcpyDeviceToHost, st));
+    // O15: the replica evidences on the device (one CTA per replica), reduced to a standard deviation below
+    double lz_rep[kErrReplicas];
+    k_evidence_error<<<kErrReplicas, 256, 0, st>>>(dl, n_it_dead, n, k, seed, logL, derr);
+    h->launches += 1;
+    RUN_CUDA(cudaMemcpyAsync(lz_rep, derr, sizeof(lz_rep), cudaMemcpyDeviceToHost, st));
     RUN_CUDA(cudaEventRecord(e1, st));
     RUN_CUDA(cudaStreamSynchronize(st));
     float ms = 0.f;
@@ -1064,23 +1134,9 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
     double H = 0.0;
     for (int64_t i = 0; i < n_dead; ++i)
       if (out->dead_logL[i] > -INFINITY) H += exp(out->dead_logL[i] + out->dead_logw[i] - logZf) * (out->dead_logL[i] - logZf);
-    const int R = 200;
-    double ls = -INFINITY;
-    for (int j = 0; j < n; ++j) ls = lae(ls, out->dead_logL[n_it_dead + j]);
+    const int R = kErrReplicas;
     double sum = 0.0, sum2 = 0.0;
-    for (int rpl = 0; rpl < R; ++rpl) {
-      double lX = 0.0, lZ = -INFINITY;
-      for (int64_t j = 0; j < n_it_dead; ++j) {
-        const double m = (double)(n - (int)(j % k));
-        uint64_t ka, kb;
-        draw53(seed, 0u, (uint32_t)j, (uint32_t)rpl, kIterErr, ka, kb);
-        const double lXn = lX + log((double)(ka + 1) * kTwoM53) / m;
-        lZ = lae(lZ, out->dead_logL[j] + lX + log1p(-exp(lXn - lX)));
-        lX = lXn;
-      }
-      lZ = lae(lZ, lX + ls - log((double)n));
-      sum += lZ; sum2 += lZ * lZ;
-    }
+    for (int rpl = 0; rpl < R; ++rpl) { sum += lz_rep[rpl]; sum2 += lz_rep[rpl] * lz_rep[rpl]; }
     const double mu = sum / R;
     double var = sum2 / R - mu * mu;
     var = var < 0 ? 0 : var;

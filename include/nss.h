@@ -98,6 +98,11 @@ int nss_set_loglike_variant(nss_handle *h, int32_t variant);
  * sequential algorithm for every G and every lane count (tests/test_gpu_sampler.py). */
 int nss_set_chain_warps(nss_handle *h, int32_t warps);
 
+/* Diagnostics of the most recent nss_replace_step / nss_iterate (read from the control block that call fetched):
+ * rounds run by all chains together, and candidates evaluated including the speculative ones the sequential
+ * algorithm did not need (the evaluation count n_evals never includes those). */
+int nss_last_chain_diag(nss_handle *h, int64_t *rounds_host, int64_t *evaluated_host);
+
 /* Lanes that evaluate one candidate in K3 (relative binning only): 0 = automatic, else 8, 16 or 32 (a width
  * whose table was not built, e.g. 8 lanes with more than 256 bins, falls back to the automatic choice). */
 int nss_set_chain_lanes(nss_handle *h, int32_t lanes);

@@ -42,6 +42,7 @@ struct NssDev {
 struct NssCtl {
   double state[4];             // logX, logZ, logZ_live, Lstar
   unsigned long long nevals;
+  unsigned long long nrounds, nexec;   // K3 diagnostics: rounds run by all chains, candidates evaluated (incl. speculative)
   int32_t flags[4];            // [0] Cholesky error, [1] threshold violation, [2] stop rule reached
 };
 

@@ -432,6 +432,7 @@ struct ChainArgs {
   const double *state;          // state[3] = L*
   const int32_t *flags;         // flags[0] != 0 (Cholesky failure) or flags[1] != 0 -> do nothing
   unsigned long long *n_evals;
+  unsigned long long *diag;     // [2]: rounds, evaluated candidates
   int32_t *trace;               // optional [k][n_repeats][3]
   double *margin;               // optional [k]
   int32_t G;                    // warps per chain
@@ -458,7 +459,7 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
   __shared__ double sZ[kDirChunk][NSS_NSLOT + 1];                  // normals of the current chunk
   __shared__ double sV[kDirChunk][NSS_NSLOT];                      // directions v = w L z/|z|
   __shared__ double sRes[2][kSlots];                               // double-buffered: logL of every candidate slot
-  __shared__ int32_t sFlag[2][kSlots];                             // 1 = in the box (evaluated), 0 = outside the box
+  __shared__ double sX[kChainWarps][NSS_NSLOT + 1];                // chain position, one copy per warp (lane-level box tests)
   __shared__ __align__(16) double sConst[nssk::kSubConstDoubles];
   if (A.flags[0] | A.flags[1]) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -517,8 +518,12 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
     double xj[NC];
 #pragma unroll
     for (int c = 0; c < NC; ++c) xj[c] = own[c] ? A.live[(size_t)slot * d + sl + c * LANES] : 0.0;
+    __syncwarp();
+    for (int j = lane; j < d; j += 32) sX[warp][j] = A.live[(size_t)slot * d + j];
+    __syncwarp();
     double lx = A.logL[slot];
     long long evals = 0;
+    int rounds = 0, nexec = 0;
     double margin = INFINITY;
 
     for (int s0 = 0; s0 < A.n_repeats; s0 += kDirChunk) {
@@ -553,90 +558,110 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
         double vj[NC];
 #pragma unroll
         for (int c = 0; c < NC; ++c) vj[c] = own[c] ? sV[s - s0][sl + c * LANES] : 0.0;
-        // uniforms of this step: lane 0 -> bracket offset (block 0), lane 1+kk -> kk-th shrinkage proposal (block 64+kk)
-        const double ulane = uniform_a(A.seed, lane == 0 ? 0u : (uint32_t)(63 + lane), (uint32_t)s, chain, it);
+        const double *vrow = sV[s - s0];
+        // uniforms of this step: lane 0 -> bracket offset (block 0); lane 1+i -> shrinkage proposal ubase+i (block 64+ubase+i)
+        double ulane = uniform_a(A.seed, lane == 0 ? 0u : (uint32_t)(63 + lane), (uint32_t)s, chain, it);
+        int ubase = 0;
         const double u0 = nssk::shfl_d(ulane, 0);
         double l = -u0, r = 1.0 - u0;
         int nl = 0, nr = 0, kk = 0, acc = -1;
         bool ldone = false, rdone = false, done = false;
         while (!done) {
-          // ---- candidate of this sub-warp ---------------------------------------------------------------------
+          // ---- the next tests of the sequential algorithm, one per lane, assuming each of them fails ------------
+          if (kk - ubase > 15) {                         // keep at least 16 proposals' uniforms in the lanes
+            ubase = kk;
+            ulane = uniform_a(A.seed, (uint32_t)(63 + ubase + lane), (uint32_t)s, chain, it);
+          }
           int nside = (ldone ? 0 : 1) + (rdone ? 0 : 1);
-          nside = nside < C ? nside : C;                 // C = 1: one side test per round, left first
-          int nshr = C - nside;
+          int nshr = 31 - (kk - ubase);                  // proposals whose uniforms are at hand
           nshr = nshr < kMaxShrink - kk ? nshr : kMaxShrink - kk;
-          double t = 0.0;
-          const bool active = cs < nside + nshr;
-          if (cs < nside) t = (cs == 0 && !ldone) ? l : r;
+          nshr = nshr < 32 - nside ? nshr : 32 - nside;
+          nshr = nshr < 2 * C ? nshr : 2 * C;            // no point in listing far more tests than can be evaluated
+          const int nt = nside + nshr;
+          double my_t = (lane == 0 && !ldone) ? l : r;   // lanes < nside: the bracket ends
           {
-            // shrinkage proposals kk .. : every lane walks the bracket as far as its own slot needs (the loop
-            // bound is the warp's last slot, so the shuffles stay convergent)
-            int imax = w * NSUB + NSUB - 1 - nside;
-            imax = imax < nshr - 1 ? imax : nshr - 1;
             double ls = l, rs = r;
-            for (int i = 0; i <= imax; ++i) {
-              const int q = kk + i;
-              const double uk = q < 31 ? nssk::shfl_d(ulane, q + 1) : uniform_a(A.seed, (uint32_t)(64 + q), (uint32_t)s, chain, it);
-              if (i <= cs - nside) {
-                t = __dadd_rn(ls, __dmul_rn(rs - ls, uk));
-                if (t < 0.0) ls = t; else rs = t;
-              }
+            for (int j = 0; j < nshr; ++j) {
+              const double uk = nssk::shfl_d(ulane, kk - ubase + j + 1);
+              const double t = __dadd_rn(ls, __dmul_rn(rs - ls, uk));
+              if (t < 0.0) ls = t; else rs = t;
+              if (lane == nside + j) my_t = t;
             }
           }
-          // ---- evaluate: box test (inclusive) first, then logL(x + t v) ---------------------------------------
-          bool inb = true;
-          double yj[NC];
+          // box test (inclusive) of the lane's own test: y = x + t v, every coordinate
+          bool inb = lane < nt;
 #pragma unroll
-          for (int c = 0; c < NC; ++c) {
-            yj[c] = __dadd_rn(xj[c], __dmul_rn(t, vj[c]));
-            inb = inb && (!own[c] || (yj[c] >= lo_j[c] && yj[c] <= hi_j[c]));
+          for (int j = 0; j < NSS_NSLOT; ++j)
+            if (j < d) {
+              const double y = __dadd_rn(sX[warp][j], __dmul_rn(my_t, vrow[j]));
+              inb = inb && (y >= P.lo[j]) && (y <= P.hi[j]);
+            }
+          const unsigned M = __ballot_sync(0xffffffffu, inb);      // tests inside the box, in sequential order
+          // ---- evaluate: the cs-th test inside the box goes to candidate slot cs -------------------------------
+          const bool have = cs < __popc(M);
+          ++rounds;
+          nexec += min(C, __popc(M));
+          int e = 0;                                     // lane holding the test of slot cs: the one with cs set bits of M below it
+          {
+            const int below = __popc(M & ((1u << lane) - 1u));
+#pragma unroll
+            for (int q = 0; q < NSUB; ++q) {
+              const unsigned hit = __ballot_sync(0xffffffffu, inb && below == w * NSUB + q);
+              if (sub == q && hit) e = __ffs(hit) - 1;
+            }
           }
-          const unsigned bal = __ballot_sync(0xffffffffu, inb);
-          const bool inbox = active && ((bal & sub_mask) == sub_mask);
+          const double tc = nssk::shfl_d(my_t, e);
 #pragma unroll
           for (int c = 0; c < NC; ++c)
-            if (own[c]) X.scr[dst_idx[c]] = yj[c];
+            if (own[c]) X.scr[dst_idx[c]] = __dadd_rn(xj[c], __dmul_rn(tc, vj[c]));
           __syncwarp();
           double ly;
-          if (KIND == NSS_KIND_GAUSS) ly = inbox ? nssk::gauss_loglike(P, X.scr) : -INFINITY;
-          else ly = nssk::loglike_sub<NDET, KIND, LANES>(P, X, inbox);
-          if (!inbox) ly = -INFINITY;
-          __syncwarp();
-          if (sl == 0) { sRes[par][cs] = ly; sFlag[par][cs] = inbox ? 1 : 0; }
+          if (KIND == NSS_KIND_GAUSS) ly = have ? nssk::gauss_loglike(P, X.scr) : -INFINITY;
+          else ly = nssk::loglike_sub<NDET, KIND, LANES>(P, X, have);
+          if (sl == 0) sRes[par][cs] = ly;
           group_sync(G);
           const double *res = sRes[par];
-          const int32_t *flg = sFlag[par];
           par ^= 1;
-          // ---- replay the sequential decisions ---------------------------------------------------------------
-          bool expanded = false;
-          int slot_i = 0;
+          // ---- replay the sequential decisions: tests outside the box fail without an evaluation, tests inside
+          // take the next result; the first test whose result is not there yet ends the round -------------------
+          int rank = 0, ti = 0;
+          bool expanded = false, stop = false;
           if (!ldone) {
-            const double v = res[slot_i]; const int f = flg[slot_i]; ++slot_i;
-            if (f) { ++evals; margin = fmin(margin, fabs(v - Lstar)); }
-            if (f && v > Lstar) { l -= 1.0; ++nl; expanded = true; ldone = nl >= kMaxExpand; } else ldone = true;
+            const bool in = (M >> ti) & 1u; ++ti;
+            bool pass = false;
+            if (in) { const double v = res[rank++]; ++evals; margin = fmin(margin, fabs(v - Lstar)); pass = v > Lstar; }
+            if (pass) { l -= 1.0; ++nl; expanded = true; ldone = nl >= kMaxExpand; } else ldone = true;
           }
-          if (!rdone && slot_i < nside) {
-            const double v = res[slot_i]; const int f = flg[slot_i]; ++slot_i;
-            if (f) { ++evals; margin = fmin(margin, fabs(v - Lstar)); }
-            if (f && v > Lstar) { r += 1.0; ++nr; expanded = true; rdone = nr >= kMaxExpand; } else rdone = true;
+          if (ti < nside) {                              // the right end was listed this round
+            const bool in = (M >> ti) & 1u; ++ti;
+            if (in && rank >= C) stop = true;            // C = 1 and the left end took the only slot
+            else {
+              bool pass = false;
+              if (in) { const double v = res[rank++]; ++evals; margin = fmin(margin, fabs(v - Lstar)); pass = v > Lstar; }
+              if (pass) { r += 1.0; ++nr; expanded = true; rdone = nr >= kMaxExpand; } else rdone = true;
+            }
           }
-          if (ldone && rdone && !expanded) {
-            for (int i = 0; i < nshr; ++i) {
-              const int q = kk + i;
-              const double uk = q < 31 ? nssk::shfl_d(ulane, q + 1) : uniform_a(A.seed, (uint32_t)(64 + q), (uint32_t)s, chain, it);
-              const double ti = __dadd_rn(l, __dmul_rn(r - l, uk));
-              const double v = res[slot_i + i]; const int f = flg[slot_i + i];
-              if (f) { ++evals; margin = fmin(margin, fabs(v - Lstar)); }
-              if (f && v > Lstar) {
+          if (ldone && rdone && !expanded && !stop) {
+            for (int j = 0; j < nshr; ++j) {
+              const bool in = (M >> (nside + j)) & 1u;
+              if (in && rank >= C) break;
+              const double tj = nssk::shfl_d(my_t, nside + j);
+              bool pass = false;
+              double v = -INFINITY;
+              if (in) { v = res[rank++]; ++evals; margin = fmin(margin, fabs(v - Lstar)); pass = v > Lstar; }
+              if (pass) {
 #pragma unroll
-                for (int c = 0; c < NC; ++c) xj[c] = __dadd_rn(xj[c], __dmul_rn(ti, vj[c]));
-                lx = v; acc = q; done = true;
+                for (int c = 0; c < NC; ++c) xj[c] = __dadd_rn(xj[c], __dmul_rn(tj, vj[c]));
+                for (int jj = lane; jj < d; jj += 32) sX[warp][jj] = __dadd_rn(sX[warp][jj], __dmul_rn(tj, vrow[jj]));
+                lx = v; acc = kk; done = true;
                 break;
               }
-              if (ti < 0.0) l = ti; else r = ti;
+              if (tj < 0.0) l = tj; else r = tj;
+              ++kk;
             }
-            if (!done) { kk += nshr; done = kk >= kMaxShrink; }
+            if (!done && kk >= kMaxShrink) done = true;
           }
+          __syncwarp();
         }
         if (A.trace && gl == 0) {
           int32_t *tr = A.trace + ((size_t)ch * A.n_repeats + s) * 3;
@@ -655,6 +680,8 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
         if (A.birth) A.birth[dst] = Lstar;
         if (A.margin) A.margin[ch] = margin;
         atomicAdd(A.n_evals, (unsigned long long)evals);
+        atomicAdd(A.diag, (unsigned long long)rounds);
+        atomicAdd(A.diag + 1, (unsigned long long)nexec);
       }
     }
   }
@@ -725,7 +752,7 @@ __global__ void k_begin(NssCtl *ctl, int set_state, double logX, double logZ, in
   if (threadIdx.x < 4) ctl->flags[threadIdx.x] = 0;
   if (threadIdx.x == 0) {
     if (set_state) { ctl->state[0] = logX; ctl->state[1] = logZ; ctl->state[2] = 0.0; ctl->state[3] = 0.0; }
-    if (zero_evals) ctl->nevals = 0ull;
+    if (zero_evals) { ctl->nevals = 0ull; ctl->nrounds = 0ull; ctl->nexec = 0ull; }
   }
 }
 
@@ -782,7 +809,7 @@ int enqueue_iteration(nss_handle *h, double *live, double *logL, double *birth, 
   ChainArgs A;
   A.live = live; A.logL = logL; A.birth = birth; A.n = n; A.k = k; A.n_repeats = n_repeats; A.seed = seed;
   A.iteration = iteration; A.surv_idx = h->d_surv_idx; A.dead_idx = dead_idx; A.chol = h->d_chol; A.state = h->d_state;
-  A.flags = h->d_flags; A.n_evals = h->d_nevals; A.trace = h->trace_dev; A.margin = h->margin_dev;
+  A.flags = h->d_flags; A.n_evals = h->d_nevals; A.diag = &h->d_ctl->nrounds; A.trace = h->trace_dev; A.margin = h->margin_dev;
   A.G = 1;
   switch (h->dev.n_det) {
     case 0: case 1: return launch_chains<1>(h, A, st);
@@ -801,6 +828,14 @@ extern "C" int nss_last_chain_ms(nss_handle *h, double *ms_host)
   float ms = 0.f;
   NSS_CUDA(cudaEventElapsedTime(&ms, h->ev_k3[0], h->ev_k3[1]));
   *ms_host = ms;
+  return NSS_OK;
+}
+
+extern "C" int nss_last_chain_diag(nss_handle *h, int64_t *rounds_host, int64_t *evaluated_host)
+{
+  if (!h || !h->h_ctl) return NSS_EINVAL;
+  if (rounds_host) *rounds_host = (int64_t)h->h_ctl->nrounds;
+  if (evaluated_host) *evaluated_host = (int64_t)h->h_ctl->nexec;
   return NSS_OK;
 }
 

@@ -60,7 +60,7 @@ EXPORTS = ("nss_create", "nss_destroy", "nss_loglike_batch", "nss_loglike_batch_
            "nss_replace_step", "nss_iterate", "nss_iterate_host",
            "nss_set_trace", "nss_select_lowest", "nss_tune", "nss_evidence_update", "nss_init_live",
            "nss_philox", "nss_run", "nss_waveform", "nss_get_tables", "nss_fp64_peak", "nss_launch_count",
-           "nss_last_chain_ms", "nss_set_chain_warps", "nss_set_chain_lanes",
+           "nss_last_chain_ms", "nss_set_chain_warps", "nss_set_chain_lanes", "nss_last_chain_diag",
            "nss_strerror", "nss_last_cuda_error", "nss_version")
 
 _lib = None
@@ -101,6 +101,7 @@ def lib():
         L.nss_last_chain_ms.argtypes = [vp, c_dp]
         L.nss_set_chain_warps.argtypes = [vp, C.c_int32]
         L.nss_set_chain_lanes.argtypes = [vp, C.c_int32]
+        L.nss_last_chain_diag.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.nss_launch_count.restype = C.c_int64
         L.nss_strerror.argtypes = [C.c_int]
         L.nss_strerror.restype = C.c_char_p
@@ -210,6 +211,12 @@ class Nss:
 
     def set_chain_warps(self, warps: int):
         _check(lib().nss_set_chain_warps(self._h, int(warps)), "nss_set_chain_warps")
+
+    def nss_last_chain_diag(self):
+        """(rounds, evaluated candidates) of the most recent iteration."""
+        a, b = C.c_int64(), C.c_int64()
+        _check(lib().nss_last_chain_diag(self._h, C.byref(a), C.byref(b)), "nss_last_chain_diag")
+        return a.value, b.value
 
     def set_chain_lanes(self, lanes: int):
         _check(lib().nss_set_chain_lanes(self._h, int(lanes)), "nss_set_chain_lanes")

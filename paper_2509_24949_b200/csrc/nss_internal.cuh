@@ -68,6 +68,8 @@ struct nss_handle {
   unsigned long long *d_nevals;
   NssCtl *d_ctl, *h_ctl;       // d_state, d_nevals, d_flags point into d_ctl; h_ctl is pinned
   double *d_birth;
+  double *d_dirs;              // [k][n_repeats][d] slice directions of the current iteration
+  size_t dirs_bytes;
   int32_t *trace_dev;
   double *margin_dev;
   // device staging for the host-buffer entry points (grown on demand)

@@ -406,6 +406,51 @@ __global__ void k_gather_rows(const double *__restrict__ live, const double *__r
   for (int a = 0; a < d; ++a) out_theta[(size_t)j * d + a] = live[(size_t)slot * d + a];
 }
 
+// ---- a5: slice directions of every (chain, step), one thread each ------------------------------------------------
+// z ~ N(0, I_d) by Box-Muller (one Philox block per pair: counter (1 + pair, step, chain, iteration)),
+// n = z/|z|, v = w L n with L the Cholesky factor of the live-point covariance (O12.4a).
+__global__ void __launch_bounds__(128) k_directions(int d, const double *__restrict__ chol, int k, int n_repeats, uint64_t seed,
+                                                    uint32_t it, const int32_t *__restrict__ flags, double *__restrict__ dirs)
+{
+  __shared__ double sL[NSS_NSLOT * NSS_NSLOT];
+  if (flags[0] | flags[1]) return;
+  for (int t = threadIdx.x; t < d * d; t += blockDim.x) sL[t] = chol[t];
+  __syncthreads();
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= k * n_repeats) return;
+  const int ch = idx / n_repeats, s = idx - ch * n_repeats;
+  double z[NSS_NSLOT + 1];
+#pragma unroll
+  for (int b = 0; b < (NSS_NSLOT + 1) / 2; ++b)
+    if (2 * b < d) {
+      uint64_t ka, kb;
+      draw53(seed, (uint32_t)(1 + b), (uint32_t)s, (uint32_t)ch, it, ka, kb);
+      const double r = sqrt(-2.0 * log((double)(ka + 1) * kTwoM53));
+      double sn, cs;
+      sincospi(2.0 * ((double)kb * kTwoM53), &sn, &cs);
+      z[2 * b] = r * cs;
+      z[2 * b + 1] = r * sn;
+    }
+  double nz = 0.0;
+#pragma unroll
+  for (int j = 0; j < NSS_NSLOT; ++j)
+    if (j < d) nz += z[j] * z[j];
+  nz = sqrt(nz);
+#pragma unroll
+  for (int j = 0; j < NSS_NSLOT; ++j)
+    if (j < d) z[j] = z[j] / nz;
+  double *out = dirs + (size_t)idx * d;
+#pragma unroll
+  for (int i = 0; i < NSS_NSLOT; ++i)
+    if (i < d) {
+      double a = 0.0;
+#pragma unroll
+      for (int j = 0; j < NSS_NSLOT; ++j)
+        if (j <= i) a += sL[i * d + j] * z[j];
+      out[i] = kSliceW * a;
+    }
+}
+
 // ---- K3: slice-sampling chains (O12.4, O12.5) -------------------------------------------------------------------
 // A chain is run by a GROUP of G warps (G = 1, 2, 4 or 8).  Every bracket test is one likelihood evaluation by
 // ONE SUB-WARP of LANES lanes (8 for relative binning: four candidates per warp share every instruction of the
@@ -428,7 +473,7 @@ struct ChainArgs {
   uint64_t seed;
   uint32_t iteration;
   const int32_t *surv_idx, *dead_idx;
-  const double *chol;           // [d][d]
+  const double *dirs;           // [k][n_repeats][d] slice directions v = w L z/|z| (k_directions)
   const double *state;          // state[3] = L*
   const int32_t *flags;         // flags[0] != 0 (Cholesky failure) or flags[1] != 0 -> do nothing
   unsigned long long *n_evals;
@@ -440,7 +485,6 @@ struct ChainArgs {
 
 constexpr int kChainWarps = 8;          // largest group; a CTA is ONE group (G warps), one chain at a time
 constexpr int kChainThreads = kChainWarps * 32;
-constexpr int kDirChunk = 16;           // slice directions are drawn 16 steps at a time by the whole group
 
 __device__ __forceinline__ void group_sync(int G)
 {
@@ -455,9 +499,7 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
   constexpr int kSlots = kChainWarps * NSUB;                    // most candidates per round
   extern __shared__ __align__(128) unsigned char smem_raw[];    // [record table if RESIDENT][C sub-warp scratches]
   __shared__ __align__(8) uint64_t bar;
-  __shared__ double sL[NSS_NSLOT * NSS_NSLOT];
-  __shared__ double sZ[kDirChunk][NSS_NSLOT + 1];                  // normals of the current chunk
-  __shared__ double sV[kDirChunk][NSS_NSLOT];                      // directions v = w L z/|z|
+  __shared__ double sV[kChainWarps][NSS_NSLOT + 1];                // direction of the current step, one copy per warp
   __shared__ double sRes[2][kSlots];                               // double-buffered: logL of every candidate slot
   __shared__ double sX[kChainWarps][NSS_NSLOT + 1];                // chain position, one copy per warp (lane-level box tests)
   __shared__ __align__(16) double sConst[nssk::kSubConstDoubles];
@@ -477,7 +519,6 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
     }
   }
   const int d = P.d;
-  for (int t = threadIdx.x; t < d * d; t += blockDim.x) sL[t] = A.chol[t];
   if (KIND != NSS_KIND_GAUSS) {
     nssk::sub_consts_init(P, sConst);
     for (int t = sl; t < 12; t += LANES) X.scr[t] = t < NSS_NSLOT ? P.theta_fixed[t] : 0.0;   // unsampled slots never change
@@ -507,7 +548,6 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
   }
   const unsigned sub_mask = (LANES == 32 ? 0xffffffffu : ((1u << LANES) - 1u)) << (sub * LANES);
   int par = 0;
-  const int nb = (d + 1) >> 1;
 
   for (int ch = blockIdx.x; ch < A.k; ch += gridDim.x) {
     const uint32_t chain = (uint32_t)ch;
@@ -526,39 +566,19 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
     int rounds = 0, nexec = 0;
     double margin = INFINITY;
 
-    for (int s0 = 0; s0 < A.n_repeats; s0 += kDirChunk) {
-      const int clen = min(kDirChunk, A.n_repeats - s0);
-      // a5: directions of steps s0 .. s0+clen-1.  Normals z (Box-Muller, one Philox block per pair) ...
-      group_sync(G);                            // the previous chunk's directions are no longer read
-      for (int idx = gl; idx < clen * nb; idx += GL) {
-        const int ss = idx / nb, b = idx - ss * nb;
-        uint64_t ka, kb;
-        draw53(A.seed, (uint32_t)(1 + b), (uint32_t)(s0 + ss), chain, it, ka, kb);
-        const double r = sqrt(-2.0 * log((double)(ka + 1) * kTwoM53));
-        double sn, cs2;
-        sincospi(2.0 * ((double)kb * kTwoM53), &sn, &cs2);
-        sZ[ss][2 * b] = r * cs2;
-        sZ[ss][2 * b + 1] = r * sn;
-      }
-      group_sync(G);
-      // ... then n = z/|z|, v = w L n, one (step, row) pair per lane
-      for (int idx = gl; idx < clen * d; idx += GL) {
-        const int ss = idx / d, i = idx - ss * d;
-        const double *z = sZ[ss];
-        double nz = 0.0;
-        for (int j = 0; j < d; ++j) nz += z[j] * z[j];
-        nz = sqrt(nz);
-        double a = 0.0;
-        for (int j = 0; j <= i; ++j) a += sL[i * d + j] * (z[j] / nz);
-        sV[ss][i] = kSliceW * a;
-      }
-      group_sync(G);
-
-      for (int s = s0; s < s0 + clen; ++s) {
+    // a5: the directions were drawn by k_directions; the next step's is fetched while this step runs
+    const double *vsrc = A.dirs + (size_t)ch * A.n_repeats * d;
+    double vpre = (lane < d && A.n_repeats > 0) ? vsrc[lane] : 0.0;
+    {
+      for (int s = 0; s < A.n_repeats; ++s) {
+        __syncwarp();
+        if (lane < d) sV[warp][lane] = vpre;
+        __syncwarp();
+        if (lane < d && s + 1 < A.n_repeats) vpre = vsrc[(size_t)(s + 1) * d + lane];
+        const double *vrow = sV[warp];
         double vj[NC];
 #pragma unroll
-        for (int c = 0; c < NC; ++c) vj[c] = own[c] ? sV[s - s0][sl + c * LANES] : 0.0;
-        const double *vrow = sV[s - s0];
+        for (int c = 0; c < NC; ++c) vj[c] = own[c] ? vrow[sl + c * LANES] : 0.0;
         // uniforms of this step: lane 0 -> bracket offset (block 0); lane 1+i -> shrinkage proposal ubase+i (block 64+ubase+i)
         double ulane = uniform_a(A.seed, lane == 0 ? 0u : (uint32_t)(63 + lane), (uint32_t)s, chain, it);
         int ubase = 0;
@@ -804,11 +824,22 @@ int enqueue_iteration(nss_handle *h, double *live, double *logL, double *birth, 
   k4_finish_select<<<1, kOneCta, 0, st>>>(live, logL, birth, n, k, d, Lstar_in, h->d_rank, dead_idx, h->d_surv_idx, dead_theta,
                                           dead_logL, dead_birth, h->d_state, h->d_flags);
   k4_tune<<<1, kOneCta, 0, st>>>(live, n, d, h->d_mean, h->d_chol, h->d_flags);
-  h->launches += 3;
+  {
+    const size_t need = sizeof(double) * (size_t)k * (n_repeats > 0 ? n_repeats : 1) * d;
+    if (h->dirs_bytes < need) {
+      cudaFree(h->d_dirs);
+      h->d_dirs = nullptr; h->dirs_bytes = 0;
+      cudaError_t e = cudaMalloc((void **)&h->d_dirs, need);
+      if (e != cudaSuccess) { nss_cuda_fail(e, "cudaMalloc(dirs)"); return e == cudaErrorMemoryAllocation ? NSS_ENOMEM : NSS_ECUDA; }
+      h->dirs_bytes = need;
+    }
+    if (n_repeats > 0) k_directions<<<(k * n_repeats + 127) / 128, 128, 0, st>>>(d, h->d_chol, k, n_repeats, seed, iteration, h->d_flags, h->d_dirs);
+  }
+  h->launches += n_repeats > 0 ? 4 : 3;
   NSS_CUDA(cudaGetLastError());
   ChainArgs A;
   A.live = live; A.logL = logL; A.birth = birth; A.n = n; A.k = k; A.n_repeats = n_repeats; A.seed = seed;
-  A.iteration = iteration; A.surv_idx = h->d_surv_idx; A.dead_idx = dead_idx; A.chol = h->d_chol; A.state = h->d_state;
+  A.iteration = iteration; A.surv_idx = h->d_surv_idx; A.dead_idx = dead_idx; A.dirs = h->d_dirs; A.state = h->d_state;
   A.flags = h->d_flags; A.n_evals = h->d_nevals; A.diag = &h->d_ctl->nrounds; A.trace = h->trace_dev; A.margin = h->margin_dev;
   A.G = 1;
   switch (h->dev.n_det) {

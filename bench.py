@@ -206,7 +206,7 @@ def run_ours(args):
         bufs = g.iter_buffers(k)
         runs = 0
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-        evals, k3_ms, launches0 = 0, 0.0, 0
+        evals, k3_ms, launches0, rounds, executed = 0, 0.0, 0, 0, 0
         barrier()
         wall0 = None
         for s in range(args.warmup + args.steps):
@@ -225,6 +225,8 @@ def run_ours(args):
                 ev[s - args.warmup][1].record(stream)
                 evals += st.n_evals
                 k3_ms += g.nss_last_chain_ms()
+                rd, ex = g.nss_last_chain_diag()
+                rounds += rd; executed += ex
             it += 1
         barrier()
         wall = time.perf_counter() - wall0
@@ -309,13 +311,15 @@ def run_ours(args):
         "gpu_launches": launches,
         "evals_per_step": evals / args.steps / world,
         "wall_ms_timed_region": 1e3 * wall,
-        "roofline": {"bound": "alu", "kernel": "k3_slice (persistent slice-sampling chains, likelihood inlined)",
+        "roofline": {"bound": "alu", "kernel": "k3_slice (one slice chain per CTA, likelihood inlined)",
                      "achieved": k3_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": k3_tf / peak_tf,
                      "peak_source": "fp64 DFMA chain measured in this process (nss_fp64_peak); nominal 148 SM x 64 lanes x 2 x "
                                     "1.965 GHz = 37.2; MEASURED_PEAKS.json has no fp64 figure",
                      "flop_per_eval": flop, "fp64_instr_per_eval": instr,
                      "pipe_frac": (evals / world) * instr / (k3_ms * 1e-3) / (peak_tf * 1e12 / 2),
-                     "kernel_ms_per_step": k3_ms / args.steps, "kernel_share_of_step": k3_ms / ms, "traffic": None},
+                     "kernel_ms_per_step": k3_ms / args.steps, "kernel_share_of_step": k3_ms / ms, "traffic": None,
+                     "rounds_per_chain": rounds / args.steps / k, "evaluated_incl_speculative_per_step": executed / args.steps,
+                     "note": "achieved counts only the evaluations the sequential algorithm consumed"},
         "loglike_batch": {"workload": "config 5: N=1e6 prior draws, B=128 x 3 detectors, k_rec_thread", "ms": k1_ms,
                           "evals_per_s": k1_rate, "tflops": k1_rate * flop / 1e12, "frac": k1_rate * flop / 1e12 / peak_tf,
                           "pipe_frac": k1_rate * instr / (peak_tf * 1e12 / 2)},
@@ -328,7 +332,7 @@ def run_ours(args):
         from oracle import nss_oracle as orc
         orc.build()
         wo = inputs.make_data(inputs.config2(), orc.waveform)
-        n_it = 2
+        n_it = 16
         ev_o, s_o, cores = oracle_steps(wo, n_it, 0, w.n_repeats, SEED)
         line["cpu_baseline"] = {"value": ev_o / s_o, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"NS iterations 0..{n_it - 1} of the same config-2 run (n_live 1000, n_delete 500, "

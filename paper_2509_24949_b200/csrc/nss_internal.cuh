@@ -75,6 +75,9 @@ struct nss_handle {
   // device staging for the host-buffer entry points (grown on demand)
   unsigned char *d_stage;
   size_t stage_bytes;
+  // second stream for the kernels of an iteration that do not depend on each other
+  cudaStream_t st2;
+  cudaEvent_t ev_fork, ev_join;
   // device block and events of nss_run, kept between runs
   unsigned char *d_run;
   size_t run_bytes;

@@ -806,6 +806,9 @@ int ensure_scratch(nss_handle *h, int n)
     NSS_CUDA(cudaMallocHost(&h->h_ctl, sizeof(NssCtl)));
     NSS_CUDA(cudaMalloc(&h->d_mean, sizeof(double) * NSS_NSLOT));
     NSS_CUDA(cudaMalloc(&h->d_chol, sizeof(double) * NSS_NSLOT * NSS_NSLOT));
+    NSS_CUDA(cudaStreamCreateWithFlags(&h->st2, cudaStreamNonBlocking));
+    NSS_CUDA(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
+    NSS_CUDA(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming));
     h->d_state = h->d_ctl->state;             // addresses inside the device block (not dereferenced on the host)
     h->d_nevals = &h->d_ctl->nevals;
     h->d_flags = h->d_ctl->flags;
@@ -820,10 +823,15 @@ int enqueue_iteration(nss_handle *h, double *live, double *logL, double *birth, 
                       int32_t *dead_idx, cudaStream_t st)
 {
   const int d = h->dev.d;
+  // the tuning (a3) does not depend on the selection (a1): it runs beside it on the handle's second stream
+  NSS_CUDA(cudaEventRecord(h->ev_fork, st));
+  NSS_CUDA(cudaStreamWaitEvent(h->st2, h->ev_fork, 0));
+  k4_tune<<<1, kOneCta, 0, h->st2>>>(live, n, d, h->d_mean, h->d_chol, h->d_flags);
+  NSS_CUDA(cudaEventRecord(h->ev_join, h->st2));
   k4_rank<<<(n + kRankThreads - 1) / kRankThreads, kRankThreads, 0, st>>>(logL, n, k, h->d_rank, dead_idx);
   k4_finish_select<<<1, kOneCta, 0, st>>>(live, logL, birth, n, k, d, Lstar_in, h->d_rank, dead_idx, h->d_surv_idx, dead_theta,
                                           dead_logL, dead_birth, h->d_state, h->d_flags);
-  k4_tune<<<1, kOneCta, 0, st>>>(live, n, d, h->d_mean, h->d_chol, h->d_flags);
+  NSS_CUDA(cudaStreamWaitEvent(st, h->ev_join, 0));
   {
     const size_t need = sizeof(double) * (size_t)k * (n_repeats > 0 ? n_repeats : 1) * d;
     if (h->dirs_bytes < need) {

@@ -152,6 +152,9 @@ extern "C" int nss_destroy(nss_handle *h)
   if (h->h_ctl) cudaFreeHost(h->h_ctl);
   cudaFree(h->d_mean); cudaFree(h->d_chol); cudaFree(h->d_birth); cudaFree(h->d_stage);
   cudaFree(h->d_run); cudaFree(h->d_dirs);
+  if (h->st2) cudaStreamDestroy(h->st2);
+  if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+  if (h->ev_join) cudaEventDestroy(h->ev_join);
   if (h->ev_run[0]) cudaEventDestroy(h->ev_run[0]);
   if (h->ev_run[1]) cudaEventDestroy(h->ev_run[1]);
   if (h->ev_k3[0]) cudaEventDestroy(h->ev_k3[0]);

@@ -245,8 +245,10 @@ class Problem:
         return dict(rc=rc, live=live, logL=logL, dead_theta=dth, dead_logL=dl, dead_idx=didx,
                     logLstar=ls.value, n_evals=ne.value, trace=trace, margin=margin)
 
-    def run(self, n_live, n_delete, n_repeats, seed, stop_dlogz=-3.0, max_iter=10000, nthreads=None):
-        cap = int(n_delete) * int(max_iter) + int(n_live) if max_iter < 400 else 400 * n_delete + n_live
+    def run(self, n_live, n_delete, n_repeats, seed, stop_dlogz=-3.0, max_iter=10000, nthreads=None, cap=None):
+        if cap is None:                      # rows of the caller-side result arrays (no arithmetic depends on it)
+            cap = int(n_delete) * int(max_iter) + int(n_live) if max_iter < 400 else 400 * n_delete + n_live
+        cap = int(cap)
         dth, dl = np.empty((cap, self.d)), np.empty(cap)
         db, dw, scal = np.empty(cap), np.empty(cap), np.zeros(6)
         rc = lib().orc_run(self._h, n_live, n_delete, n_repeats, int(seed), stop_dlogz, max_iter, cap,

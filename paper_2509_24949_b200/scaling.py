@@ -1,0 +1,73 @@
+"""Scaling sweeps of the paper's Fig. 2 on the synthetic config-2 workload.
+
+    python -m paper_2509_24949_b200.scaling [--seed S] [--repeats R] [--quick]
+
+  left  panel: NSS wall-clock to convergence vs n_live with n_delete = n_live/2, against the naive-linear line
+               t(n0) * n/n0 the paper draws dashed;
+  right panel: wall-clock vs n_delete at n_live = 1000, against the perfect-parallel line t(1)/n_delete.
+
+Every point is one `nss_run` through the C ABI (setup excluded), the best wall clock of R runs
+(the library keeps no state between runs, so they are identical in everything but time).  Prints two markdown tables.
+The paper's figure is from an NVIDIA L4 with IMRPhenomD on GW150914; only the shape of the curves is comparable.
+"""
+from __future__ import annotations
+
+import argparse
+import time
+
+
+def run_point(g, n_live, n_delete, n_repeats, seed, repeats):
+    cap = 60 * n_live + 4 * n_delete          # dead points: ~H * n_live + the final live set, with room to spare
+    times, r = [], None
+    for _ in range(repeats + 1):              # the first run warms the launch path
+        t0 = time.perf_counter()
+        r = g.nss_run(n_live, n_delete, n_repeats, seed, max_iter=10_000_000, cap=cap)
+        times.append(time.perf_counter() - t0)
+    best = min(times[1:]) if len(times) > 1 else times[0]
+    return best, r
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--seed", type=int, default=1)
+    ap.add_argument("--repeats", type=int, default=2)
+    ap.add_argument("--quick", action="store_true", help="fewer and smaller points")
+    args = ap.parse_args()
+
+    import torch
+    from . import build, inputs, nss
+    build.build()
+    if not torch.cuda.is_available():
+        raise SystemExit("scaling.py needs a CUDA device: the product path has no CPU fallback")
+    w = inputs.make_data(inputs.config2(), nss.nss_waveform)
+    g = nss.Nss(w)
+    nrep = w.n_repeats
+
+    lives = (250, 500, 1000, 2000) if args.quick else (250, 500, 1000, 2000, 4000, 8000, 16000)
+    print("## wall-clock vs n_live (n_delete = n_live/2, config-2 likelihood, 55 slice repeats)\n")
+    print("| n_live | n_delete | wall s | device ms | iterations | evaluations | evals/s | logZ | +- | naive-linear s |")
+    print("|---|---|---|---|---|---|---|---|---|---|")
+    t0 = None
+    for n in lives:
+        t, r = run_point(g, n, n // 2, nrep, args.seed, args.repeats)
+        if t0 is None:
+            t0 = (t, n)
+        print(f"| {n} | {n // 2} | {t:.4f} | {r['gpu_ms']:.1f} | {r['n_iter']} | {r['n_evals']} | {r['n_evals'] / t:.3e} | "
+              f"{r['logZ']:.2f} | {r['logZ_err']:.2f} | {t0[0] * n / t0[1]:.4f} |", flush=True)
+
+    dels = (10, 50, 250, 500) if args.quick else (1, 2, 5, 10, 25, 50, 100, 250, 500, 750)
+    print("\n## wall-clock vs n_delete (n_live = 1000)\n")
+    print("| n_delete | wall s | device ms | iterations | evaluations | evals/s | logZ | +- | perfect-parallel s |")
+    print("|---|---|---|---|---|---|---|---|---|")
+    t1 = None
+    for k in dels:
+        t, r = run_point(g, 1000, k, nrep, args.seed, args.repeats if k >= 10 else 1)
+        if t1 is None:
+            t1 = (t, k)
+        print(f"| {k} | {t:.4f} | {r['gpu_ms']:.1f} | {r['n_iter']} | {r['n_evals']} | {r['n_evals'] / t:.3e} | "
+              f"{r['logZ']:.2f} | {r['logZ_err']:.2f} | {t1[0] * t1[1] / k:.4f} |", flush=True)
+    g.close()
+
+
+if __name__ == "__main__":
+    main()

@@ -244,6 +244,25 @@ def test_run_config1_matches_oracle(nssmod, oracle, wl1):
     g.close()
 
 
+@pytest.mark.parametrize("n_delete", [1, 7, 25, 75])
+def test_run_delete_fraction_sweep_matches_oracle(nssmod, oracle, wl1, n_delete):
+    """The n_delete axis of the paper's Fig. 2 (right panel): one chain per iteration up to three
+    quarters of the live set.  Same seed -> the oracle's run, decision for decision, until a near-threshold test flips;
+    always logZ within 3 sigma_NS, and the bookkeeping invariant sum(w) + X_end = 1 (P14) at every delete fraction."""
+    g, p = nssmod.Nss(wl1), oracle.Problem(wl1)
+    r = g.nss_run(100, n_delete, 12, 5, max_iter=100000, cap=100 * 60)
+    o = p.run(100, n_delete, 12, 5, max_iter=100000, cap=100 * 60)
+    assert r["rc"] == 0 and o["rc"] == 0
+    assert abs(r["logZ"] - o["logZ"]) < 3 * math.hypot(r["logZ_err"], o["logZ_err"])
+    assert np.all(np.diff(r["dead_logL"][: r["n_dead"] - 100]) >= 0)           # dead points leave in ascending logL
+    assert np.exp(r["dead_logw"]).sum() == pytest.approx(1.0, abs=1e-9)        # dead + final live weights exhaust the prior
+    if r["n_dead"] == o["n_dead"] and np.allclose(r["dead_logL"], o["dead_logL"], rtol=1e-9, atol=1e-6):
+        assert r["n_iter"] == o["n_iter"] and r["n_evals"] == o["n_evals"]
+        assert np.allclose(r["dead_logw"], o["dead_logw"], rtol=0, atol=1e-9)
+        assert np.array_equal(r["dead_theta"], o["dead_theta"]) or np.allclose(r["dead_theta"], o["dead_theta"], rtol=1e-12, atol=1e-12)
+    g.close()
+
+
 def test_iterate_device_and_host_forms_match_oracle(nssmod, oracle, wl1):
     """nss_iterate = replace step + evidence bookkeeping + live evidence (all §8(a) rows); the host-buffer
     form returns the same bits as the device form."""

@@ -165,6 +165,22 @@ def test_replace_step_trajectories_config2_and_teacher_forced_threshold(nssmod, 
     g.close()
 
 
+@pytest.mark.parametrize("n_live,n_delete", [(1000, 500), (5000, 2500)])
+def test_replace_step_full_size_bench_configuration(nssmod, oracle, wl2, n_live, n_delete):
+    """BASELINE configs[1] and configs[2] at full size, in the launch configuration bench.py times (all 55 slice
+    repeats, automatic lanes / warps per chain): one NS iteration from the initial live set and one from a population
+    three iterations in, every chain against the oracle's trajectory (A20: chains whose margins exceed the logL tolerance)."""
+    g, p = nssmod.Nss(wl2), oracle.Problem(wl2)
+    live, logL = p.init_live(n_live, 4)
+    r, o, safe = _trajectory_parity(g, p, live, logL, n_delete, 55, seed=4, it=0, w=wl2, max_excluded=0.05)
+    live, logL = o["live"], o["logL"]
+    for it in (1, 2):
+        o = p.replace_step(live, logL, n_delete, 8, 4, it)
+        live, logL = o["live"], o["logL"]
+    _trajectory_parity(g, p, live, logL, n_delete, 55, seed=4, it=3, w=wl2, max_excluded=0.05)
+    g.close()
+
+
 def test_replace_step_full_grid_kind(nssmod, oracle):
     w = inputs.make_data(inputs.config4(), oracle.waveform)
     g, p = nssmod.Nss(w), oracle.Problem(w)

@@ -160,6 +160,17 @@ def config_dict(w):
             "l2": "flushed (256 MiB write) between steps, outside the per-step event pairs; working set < 1 MB, ALU-bound"}
 
 
+def aggregate_replicas(dist, times, counts, device):
+    """Replicas only: every rank ran the same number of steps on its own seeds.  The job's time is
+    the MAX over ranks of each timed quantity, its work the SUM over ranks of each count."""
+    import torch
+    t = torch.tensor(list(times), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor(list(counts), dtype=torch.float64, device=device)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return tuple(float(x) for x in t), tuple(int(x) for x in c)
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -287,12 +298,8 @@ def run_ours(args):
 
     # max over ranks of the timed quantities; sum of the work
     if dist:
-        t = torch.tensor([ms, t_h, k3_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        c = torch.tensor([evals, evals_h, launches], dtype=torch.float64, device="cuda")
-        dist.all_reduce(c, op=dist.ReduceOp.SUM)
-        ms, t_h, k3_ms = (float(x) for x in t)
-        evals, evals_h, launches = (int(x) for x in c)
+        (ms, t_h, k3_ms), (evals, evals_h, launches, rounds, executed) = aggregate_replicas(
+            dist, (ms, t_h, k3_ms), (evals, evals_h, launches, rounds, executed), "cuda")
     if rank != 0:
         if dist:
             dist.destroy_process_group()
@@ -318,7 +325,7 @@ def run_ours(args):
                      "flop_per_eval": flop, "fp64_instr_per_eval": instr,
                      "pipe_frac": (evals / world) * instr / (k3_ms * 1e-3) / (peak_tf * 1e12 / 2),
                      "kernel_ms_per_step": k3_ms / args.steps, "kernel_share_of_step": k3_ms / ms, "traffic": None,
-                     "rounds_per_chain": rounds / args.steps / k, "evaluated_incl_speculative_per_step": executed / args.steps,
+                     "rounds_per_chain": rounds / args.steps / k / world, "evaluated_incl_speculative_per_step": executed / args.steps / world,
                      "note": "achieved counts only the evaluations the sequential algorithm consumed"},
         "loglike_batch": {"workload": "config 5: N=1e6 prior draws, B=128 x 3 detectors, k_rec_thread", "ms": k1_ms,
                           "evals_per_s": k1_rate, "tflops": k1_rate * flop / 1e12, "frac": k1_rate * flop / 1e12 / peak_tf,

@@ -185,7 +185,10 @@ int launch_rec(nss_handle *h, const double *theta, int64_t N, double *logL, cuda
   constexpr bool CROSS = KIND == NSS_KIND_RB;
   const NssDev &P = h->dev;
   int variant = h->loglike_variant, rc_sub = NSS_OK;
-  if (variant == 0) variant = N >= (int64_t)h->n_sm * 512 ? 1 : 2;
+  // automatic: one thread per point for large relative-binning batches (table resident, no per-point redundancy);
+  // a warp per point otherwise, and always for the full grid (measured: 3.8e7 vs 3.1e7 evals/s, the streamed table
+  // costs the thread form a CTA barrier per tile)
+  if (variant == 0) variant = (CROSS && N >= (int64_t)h->n_sm * 512) ? 1 : 2;
   if (variant == 1) {
     const size_t rec_bytes = (size_t)P.rec_rs * sizeof(double), bytes = (size_t)P.n_rec * rec_bytes;
     int tile_recs = P.n_rec, n_tiles = 1;

@@ -502,6 +502,7 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
   __shared__ double sV[kChainWarps][NSS_NSLOT + 1];                // direction of the current step, one copy per warp
   __shared__ double sRes[2][kSlots];                               // double-buffered: logL of every candidate slot
   __shared__ double sX[kChainWarps][NSS_NSLOT + 1];                // chain position, one copy per warp (lane-level box tests)
+  __shared__ double sLo[NSS_NSLOT + 1], sHi[NSS_NSLOT + 1];        // prior box, (-inf, +inf) for the unused coordinates
   __shared__ __align__(16) double sConst[nssk::kSubConstDoubles];
   if (A.flags[0] | A.flags[1]) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -519,6 +520,11 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
     }
   }
   const int d = P.d;
+  for (int t = threadIdx.x; t <= NSS_NSLOT; t += blockDim.x) {
+    sLo[t] = t < d ? P.lo[t] : -INFINITY;
+    sHi[t] = t < d ? P.hi[t] : INFINITY;
+  }
+  if (lane <= NSS_NSLOT) { sX[warp][lane] = 0.0; sV[warp][lane] = 0.0; }
   if (KIND != NSS_KIND_GAUSS) {
     nssk::sub_consts_init(P, sConst);
     for (int t = sl; t < 12; t += LANES) X.scr[t] = t < NSS_NSLOT ? P.theta_fixed[t] : 0.0;   // unsampled slots never change
@@ -609,13 +615,13 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
             }
           }
           // box test (inclusive) of the lane's own test: y = x + t v, every coordinate
-          bool inb = lane < nt;
+          int inb_i = lane < nt;                         // branch-free: every coordinate, then one AND
 #pragma unroll
-          for (int j = 0; j < NSS_NSLOT; ++j)
-            if (j < d) {
-              const double y = __dadd_rn(sX[warp][j], __dmul_rn(my_t, vrow[j]));
-              inb = inb && (y >= P.lo[j]) && (y <= P.hi[j]);
-            }
+          for (int j = 0; j < NSS_NSLOT; ++j) {
+            const double y = __dadd_rn(sX[warp][j], __dmul_rn(my_t, vrow[j]));
+            inb_i &= (int)(y >= sLo[j]) & (int)(y <= sHi[j]);
+          }
+          const bool inb = inb_i != 0;
           const unsigned M = __ballot_sync(0xffffffffu, inb);      // tests inside the box, in sequential order
           // ---- evaluate: the cs-th test inside the box goes to candidate slot cs -------------------------------
           const bool have = cs < __popc(M);

@@ -98,6 +98,13 @@ int nss_set_loglike_variant(nss_handle *h, int32_t variant);
  * sequential algorithm for every G and every lane count (tests/test_gpu_sampler.py). */
 int nss_set_chain_warps(nss_handle *h, int32_t warps);
 
+/* NEXT-2 (covariance-tuned slices are "troublesome for the wrapped phase and polarization angle"):
+ * flags_host[j] != 0 makes sampled dimension j periodic in the slice sampler: a candidate's coordinate is mapped back
+ * into [lo_j, hi_j) as y - W floor((y - lo_j)/W), W = hi_j - lo_j, and takes no part in the prior-box test (default and
+ * NULL: hard inclusive walls in every dimension, reading A16).  Host array of d flags, copied.  The likelihood should
+ * be periodic in that coordinate over the box (phi_c over 2 pi, psi over pi, ra over 2 pi); the evidence is valid either way. */
+int nss_set_periodic(nss_handle *h, const int32_t *flags_host);
+
 /* Diagnostics of the most recent nss_replace_step / nss_iterate (read from the control block that call fetched):
  * rounds run by all chains together, and candidates evaluated including the speculative ones the sequential
  * algorithm did not need (the evaluation count n_evals never includes those). */

@@ -63,6 +63,7 @@ typedef struct orc_problem {
   int n_bins;
   int kind;                 /* 0 RB, 1 full grid, 2 Gaussian test */
   double gauss_mu[ORC_NSLOT], gauss_sigma[ORC_NSLOT];
+  int periodic[ORC_NSLOT];  /* NEXT-2: sampled dim j wraps in [lo_j, hi_j) instead of hitting a wall (0 = hard wall, A16) */
   /* derived (O7..O9) */
   double DD;                /* sum_det <d,d> */
   int *edge_idx;            /* [B+1] grid indices i_e */
@@ -611,12 +612,28 @@ typedef struct {
   int64_t n_evals; double margin;
 } chain_ctx;
 
+/* NEXT-2 (PAPER.md:45 names the wrapped phase and polarisation angle as the sampler's weak point; reading R4 in
+ * DESIGN.md): a periodic coordinate is mapped back into its box, y <- y - W floor((y - lo)/W), W = hi - lo
+ * (division, floor, product and difference each rounded once), and takes no part in the box test. */
+static double orc_wrap(double y, double lo, double hi)
+{
+  const double W = hi - lo;
+  const double kf = floor((y - lo) / W);
+  return y - W * kf;
+}
+
+void orc_set_periodic(orc_problem *p, const int *flags)
+{
+  for (int j = 0; j < ORC_NSLOT; ++j) p->periodic[j] = (flags && j < p->d) ? (flags[j] != 0) : 0;
+}
+
 /* inside(t): box test first (inclusive), then logL(x + t v) > L*  (strict) */
 static int inside(chain_ctx *c, const double *x, const double *v, double t, double *y, double *ly)
 {
   const int d = c->p->d;
   for (int j = 0; j < d; ++j) {
     y[j] = x[j] + t * v[j];
+    if (c->p->periodic[j]) { y[j] = orc_wrap(y[j], c->p->lo[j], c->p->hi[j]); continue; }
     if (!(y[j] >= c->p->lo[j] && y[j] <= c->p->hi[j])) return 0;
   }
   const double l = orc_loglike(c->p, y);

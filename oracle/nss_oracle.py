@@ -44,6 +44,8 @@ def lib():
         L.orc_create.argtypes = [C.c_int, c_ip, c_dp, c_dp, c_dp, C.c_int, c_dp, C.c_double, C.c_int,
                                  C.c_double, C.c_double, c_dp, c_dp, c_dp, C.c_int, C.c_int, c_dp, c_dp]
         L.orc_destroy.argtypes = [C.c_void_p]
+        L.orc_set_periodic.argtypes = [C.c_void_p, c_ip]
+        L.orc_set_periodic.restype = None
         L.orc_loglike.restype = C.c_double
         L.orc_loglike.argtypes = [C.c_void_p, c_dp]
         L.orc_loglike_kind.restype = C.c_double
@@ -183,6 +185,12 @@ class Problem:
                                    _dp(keep[7]), _dp(keep[8]))
         if not self._h:
             raise ValueError("orc_create rejected the problem")
+
+    def set_periodic(self, flags):
+        """NEXT-2: sampled dim j wraps in [lo_j, hi_j) when flags[j] != 0 (default: hard walls, A16)."""
+        f = np.zeros(11, dtype=np.int32)
+        f[: self.d] = np.asarray(flags, dtype=np.int32)[: self.d]
+        lib().orc_set_periodic(self._h, f.ctypes.data_as(c_ip))
 
     def __del__(self):
         if getattr(self, "_h", None):

@@ -15,6 +15,7 @@ struct NssDev {
   int32_t slot_src[NSS_NSLOT];      // canonical slot t -> sampled dim, or -1 (fixed)
   double theta_fixed[NSS_NSLOT];
   double lo[NSS_NSLOT], hi[NSS_NSLOT];
+  int32_t periodic[NSS_NSLOT];      // sampled dim j wraps in [lo_j, hi_j) in the slice sampler (nss_set_periodic)
   double gauss_mu[NSS_NSLOT], gauss_isig[NSS_NSLOT];
   double D6[NSS_MAXDET][6];   // symmetric detector tensors (O4)
   double rc[NSS_MAXDET][3];   // vertex / c [s]

@@ -465,6 +465,15 @@ __global__ void __launch_bounds__(128) k_directions(int d, const double *__restr
 // the accepted one).  Decisions, positions and the evaluation count are those of the sequential oracle.
 // The chain position x and direction v are spread over the lanes of every sub-warp (lane j holds x_j, v_j, and
 // x_{j+LANES}, v_{j+LANES} when LANES < d).
+// NEXT-2 (R4): a periodic coordinate is mapped back into its box, y - W floor((y - lo)/W), every
+// operation rounded once (the oracle does the same with contraction off), and takes no part in the box test
+__device__ __forceinline__ double wrap_periodic(double y, double lo, double hi)
+{
+  const double W = __dsub_rn(hi, lo);
+  const double kf = floor(__ddiv_rn(__dsub_rn(y, lo), W));
+  return __dsub_rn(y, __dmul_rn(W, kf));
+}
+
 struct ChainArgs {
   double *live;                 // [n][d] in/out
   double *logL;                 // [n]    in/out
@@ -521,8 +530,9 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
   }
   const int d = P.d;
   for (int t = threadIdx.x; t <= NSS_NSLOT; t += blockDim.x) {
-    sLo[t] = t < d ? P.lo[t] : -INFINITY;
-    sHi[t] = t < d ? P.hi[t] : INFINITY;
+    const bool wall = t < d && !P.periodic[t];
+    sLo[t] = wall ? P.lo[t] : -INFINITY;
+    sHi[t] = wall ? P.hi[t] : INFINITY;
   }
   if (lane <= NSS_NSLOT) { sX[warp][lane] = 0.0; sV[warp][lane] = 0.0; }
   if (KIND != NSS_KIND_GAUSS) {
@@ -544,6 +554,7 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
   bool own[NC];
   int dst_idx[NC];                                       // where coordinate j goes in the likelihood's input
   double lo_j[NC], hi_j[NC];
+  bool per[NC];                                          // the coordinate wraps instead of hitting a wall
 #pragma unroll
   for (int c = 0; c < NC; ++c) {
     const int j = sl + c * LANES;
@@ -551,6 +562,7 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
     lo_j[c] = own[c] ? P.lo[j] : 0.0;
     hi_j[c] = own[c] ? P.hi[j] : 0.0;
     dst_idx[c] = own[c] ? (KIND == NSS_KIND_GAUSS ? j : P.param_index[j]) : 0;
+    per[c] = own[c] && P.periodic[j] != 0;
   }
   const unsigned sub_mask = (LANES == 32 ? 0xffffffffu : ((1u << LANES) - 1u)) << (sub * LANES);
   int par = 0;
@@ -639,7 +651,11 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
           const double tc = nssk::shfl_d(my_t, e);
 #pragma unroll
           for (int c = 0; c < NC; ++c)
-            if (own[c]) X.scr[dst_idx[c]] = __dadd_rn(xj[c], __dmul_rn(tc, vj[c]));
+            if (own[c]) {
+              double y = __dadd_rn(xj[c], __dmul_rn(tc, vj[c]));
+              if (per[c]) y = wrap_periodic(y, lo_j[c], hi_j[c]);
+              X.scr[dst_idx[c]] = y;
+            }
           __syncwarp();
           double ly;
           if (KIND == NSS_KIND_GAUSS) ly = have ? nssk::gauss_loglike(P, X.scr) : -INFINITY;
@@ -677,8 +693,15 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
               if (in) { v = res[rank++]; ++evals; margin = fmin(margin, fabs(v - Lstar)); pass = v > Lstar; }
               if (pass) {
 #pragma unroll
-                for (int c = 0; c < NC; ++c) xj[c] = __dadd_rn(xj[c], __dmul_rn(tj, vj[c]));
-                for (int jj = lane; jj < d; jj += 32) sX[warp][jj] = __dadd_rn(sX[warp][jj], __dmul_rn(tj, vrow[jj]));
+                for (int c = 0; c < NC; ++c) {
+                  xj[c] = __dadd_rn(xj[c], __dmul_rn(tj, vj[c]));
+                  if (per[c]) xj[c] = wrap_periodic(xj[c], lo_j[c], hi_j[c]);
+                }
+                for (int jj = lane; jj < d; jj += 32) {
+                  double y = __dadd_rn(sX[warp][jj], __dmul_rn(tj, vrow[jj]));
+                  if (P.periodic[jj]) y = wrap_periodic(y, P.lo[jj], P.hi[jj]);
+                  sX[warp][jj] = y;
+                }
                 lx = v; acc = kk; done = true;
                 break;
               }
@@ -895,6 +918,13 @@ extern "C" int nss_set_chain_lanes(nss_handle *h, int32_t lanes)
 {
   if (!h || !(lanes == 0 || lanes == 8 || lanes == 16 || lanes == 32)) return NSS_EINVAL;
   h->chain_lanes = lanes;
+  return NSS_OK;
+}
+
+extern "C" int nss_set_periodic(nss_handle *h, const int32_t *flags_host)
+{
+  if (!h) return NSS_EINVAL;
+  for (int j = 0; j < NSS_NSLOT; ++j) h->dev.periodic[j] = (flags_host && j < h->dev.d) ? (flags_host[j] != 0) : 0;
   return NSS_OK;
 }
 

@@ -60,7 +60,7 @@ EXPORTS = ("nss_create", "nss_destroy", "nss_loglike_batch", "nss_loglike_batch_
            "nss_replace_step", "nss_iterate", "nss_iterate_host",
            "nss_set_trace", "nss_select_lowest", "nss_tune", "nss_evidence_update", "nss_init_live",
            "nss_philox", "nss_run", "nss_waveform", "nss_get_tables", "nss_fp64_peak", "nss_launch_count",
-           "nss_last_chain_ms", "nss_set_chain_warps", "nss_set_chain_lanes", "nss_last_chain_diag",
+           "nss_last_chain_ms", "nss_set_chain_warps", "nss_set_chain_lanes", "nss_last_chain_diag", "nss_set_periodic",
            "nss_strerror", "nss_last_cuda_error", "nss_version")
 
 _lib = None
@@ -101,6 +101,7 @@ def lib():
         L.nss_last_chain_ms.argtypes = [vp, c_dp]
         L.nss_set_chain_warps.argtypes = [vp, C.c_int32]
         L.nss_set_chain_lanes.argtypes = [vp, C.c_int32]
+        L.nss_set_periodic.argtypes = [vp, C.POINTER(C.c_int32)]
         L.nss_last_chain_diag.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.nss_launch_count.restype = C.c_int64
         L.nss_strerror.argtypes = [C.c_int]
@@ -217,6 +218,15 @@ class Nss:
         a, b = C.c_int64(), C.c_int64()
         _check(lib().nss_last_chain_diag(self._h, C.byref(a), C.byref(b)), "nss_last_chain_diag")
         return a.value, b.value
+
+    def nss_set_periodic(self, flags):
+        """NEXT-2: sampled dim j wraps in [lo_j, hi_j) in the slice sampler when flags[j] != 0 (None: hard walls)."""
+        if flags is None:
+            _check(lib().nss_set_periodic(self._h, None), "nss_set_periodic")
+            return
+        f = np.zeros(11, dtype=np.int32)
+        f[: self.d] = np.asarray(flags, dtype=np.int32)[: self.d]
+        _check(lib().nss_set_periodic(self._h, f.ctypes.data_as(C.POINTER(C.c_int32))), "nss_set_periodic")
 
     def set_chain_lanes(self, lanes: int):
         _check(lib().nss_set_chain_lanes(self._h, int(lanes)), "nss_set_chain_lanes")

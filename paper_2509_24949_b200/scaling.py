@@ -7,7 +7,8 @@
   right panel: wall-clock vs n_delete at n_live = 1000, against the perfect-parallel line t(1)/n_delete.
 
 Every point is one `nss_run` through the C ABI (setup excluded), the best wall clock of R runs
-(the library keeps no state between runs, so they are identical in everything but time).  Prints two markdown tables.
+(the library keeps no state between runs, so they are identical in everything but time).  Prints markdown tables; the
+last one compares hard walls with wrapped phi_c, psi, ra (NEXT-2).
 The paper's figure is from an NVIDIA L4 with IMRPhenomD on GW150914; only the shape of the curves is comparable.
 """
 from __future__ import annotations
@@ -66,6 +67,17 @@ def main():
             t1 = (t, k)
         print(f"| {k} | {t:.4f} | {r['gpu_ms']:.1f} | {r['n_iter']} | {r['n_evals']} | {r['n_evals'] / t:.3e} | "
               f"{r['logZ']:.2f} | {r['logZ_err']:.2f} | {t1[0] * t1[1] / k:.4f} |", flush=True)
+    # NEXT-2: hard walls (A16) against wrapped phi_c, psi, ra (nss_set_periodic), config 2 as benchmarked
+    print("\n## hard walls vs wrapped phi_c, psi, ra (n_live = 1000, n_delete = 500)\n")
+    print("| coordinates | wall s | iterations | evaluations | evals per slice step | logZ | +- | H |")
+    print("|---|---|---|---|---|---|---|---|")
+    for name, flags in (("walls", None), ("phi_c, psi, ra wrapped", [0, 0, 0, 0, 0, 0, 1, 0, 1, 1, 0])):
+        g.nss_set_periodic(flags)
+        for sd in (args.seed, args.seed + 1):
+            t, r = run_point(g, 1000, 500, nrep, sd, args.repeats)
+            print(f"| {name} (seed {sd}) | {t:.4f} | {r['n_iter']} | {r['n_evals']} | {(r['n_evals'] - 1000) / (r['n_iter'] * 500 * nrep):.2f} | "
+                  f"{r['logZ']:.2f} | {r['logZ_err']:.2f} | {r['H']:.2f} |", flush=True)
+    g.nss_set_periodic(None)
     g.close()
 
 

@@ -368,3 +368,75 @@ def test_chain_group_width_does_not_change_the_trajectory(nssmod, oracle, wl1, w
             assert np.allclose(first[1][d][safe], ref[1][d][safe], rtol=1e-9, atol=1e-6)
     g.set_chain_lanes(0)
     g.close()
+
+
+# ---- NEXT-2: periodic coordinates (nss_set_periodic) -------------------------------------------------------------------
+@pytest.mark.parametrize("cfg", ["gauss", "config1", "config2"])
+def test_next2_periodic_trajectories_match_oracle(nssmod, oracle, wl1, wl2, cfg):
+    """Wrapped phi_c (config 1), phi_c / psi / ra (config 2), or two of four coordinates of the Gaussian test problem:
+    every chain against the oracle's trajectory, from the prior-wide population (where slices cross the seam all the
+    time) and from a compressed one; then the flags switch off again."""
+    if cfg == "gauss":
+        w, n, k, nrep = inputs.gaussian_workload(4, sigma=0.3), 600, 300, 12
+        flags = [1, 0, 1, 0]
+    elif cfg == "config1":
+        w, n, k, nrep = wl1, 100, 50, 12
+        flags = [0, 0, 0, 1]
+    else:
+        w, n, k, nrep = wl2, 1000, 500, 20
+        flags = [0, 0, 0, 0, 0, 0, 1, 0, 1, 1, 0]
+    g, p = nssmod.Nss(w), oracle.Problem(w)
+    g.nss_set_periodic(flags)
+    p.set_periodic(flags)
+    live, logL = p.init_live(n, 6)
+    r, o, safe = _trajectory_parity(g, p, live, logL, k, nrep, seed=6, it=0, w=w, max_excluded=0.06)
+    moved = o["live"][o["dead_idx"]]
+    assert np.all(moved >= w.lo) and np.all(moved <= w.hi)
+    # the wrapped run differs from the walled one (some slice crossed a seam), on both sides alike
+    p.set_periodic(np.zeros(w.d, dtype=int))
+    walls = p.replace_step(live, logL, k, nrep, 6, 0)
+    assert not np.array_equal(walls["live"], o["live"])
+    p.set_periodic(flags)
+    live, logL = o["live"], o["logL"]
+    for it in (1, 2):
+        o = p.replace_step(live, logL, k, 4, 6, it)
+        live, logL = o["live"], o["logL"]
+    _trajectory_parity(g, p, live, logL, k, nrep, seed=6, it=3, w=w, max_excluded=0.06)
+    # lane / warp counts do not change a wrapped trajectory either
+    ref = None
+    for L, G in ((32, 1), (16, 2), (8, 1), (0, 0)):
+        if cfg == "gauss" and L not in (32, 0):
+            continue
+        g.set_chain_lanes(L); g.set_chain_warps(G)
+        rr = g.nss_replace_step(live, logL, k, nrep, 6, 4, want_trace=True)
+        cur = (rr["trace"].cpu().numpy(), rr["live"].cpu().numpy(), rr["margin"].cpu().numpy(), rr["dead_idx"].cpu().numpy())
+        if ref is None:
+            ref = cur
+        else:
+            ok = np.minimum(ref[2], cur[2]) > 1e-6
+            assert np.array_equal(ref[0][ok], cur[0][ok]) and np.array_equal(ref[1][ref[3]][ok], cur[1][cur[3]][ok])
+    g.set_chain_lanes(0); g.set_chain_warps(0)
+    g.nss_set_periodic(None)
+    _trajectory_parity(g, oracle.Problem(w), live, logL, k, 3, seed=6, it=5, w=w, max_excluded=0.06)
+    g.close()
+
+
+def test_next2_periodic_run_matches_oracle_and_analytic(nssmod, oracle):
+    """End to end with wrapped coordinates: the Gaussian with its peak 0.2 sigma from a wall (O16's analytic logZ holds on
+    the torus too), GPU against oracle and against the closed form."""
+    w = inputs.gaussian_workload(3, sigma=0.05)
+    w.gauss_mu = w.gauss_mu.copy()
+    w.gauss_mu[0] = -0.99
+    g, p = nssmod.Nss(w), oracle.Problem(w)
+    g.nss_set_periodic([1, 1, 0])
+    p.set_periodic([1, 1, 0])
+    truth = sum(math.log(0.05 * math.sqrt(2 * math.pi) / 2.0
+                         * (scipy.stats.norm.cdf((1 - m) / 0.05) - scipy.stats.norm.cdf((-1 - m) / 0.05))) for m in w.gauss_mu[:3])
+    r, o = g.nss_run(1000, 500, 15, 3), p.run(1000, 500, 15, 3)
+    assert r["rc"] == 0 and o["rc"] == 0
+    assert abs(r["logZ"] - truth) < 3 * r["logZ_err"]
+    assert abs(r["logZ"] - o["logZ"]) < 3 * math.hypot(r["logZ_err"], o["logZ_err"])
+    if r["n_dead"] == o["n_dead"] and np.allclose(r["dead_logL"], o["dead_logL"], rtol=1e-9, atol=1e-9):
+        assert r["n_evals"] == o["n_evals"]
+        assert np.allclose(r["dead_theta"], o["dead_theta"], rtol=0, atol=1e-12)
+    g.close()

@@ -256,3 +256,70 @@ def test_run_matches_stepwise_composition(oracle):
         t += 1
     assert t == r["n_iter"]
     assert np.logaddexp(logZ, lzl) == pytest.approx(r["logZ"], rel=1e-13)
+
+
+# ---- NEXT-2: periodic coordinates in the slice sampler (R4) ----------------------------------
+def test_next2_periodic_slices_stay_uniform_and_in_the_box(oracle):
+    """P13 with wrapped coordinates: no constraint (L* = -inf) => still uniform in the box; a wrapped coordinate
+    never fails the box test, so its brackets step out to the cap while a walled coordinate stops them."""
+    d, n, k = 3, 1000, 500
+    w = inputs.gaussian_workload(d, sigma=1.0)
+    p = oracle.Problem(w)
+    rng = np.random.default_rng(3)
+    live = rng.uniform(-1, 1, size=(n, d))
+    logL = p.loglike_batch(live)
+    p.set_periodic([1, 0, 1])
+    r = p.replace_step(live, logL, k, 40, seed=11, iteration=0, logLstar=-math.inf, want_trace=True)
+    assert r["rc"] == 0
+    new = r["live"][r["dead_idx"]]
+    assert np.all(new >= -1) and np.all(new <= 1)
+    for j in range(d):
+        assert scipy.stats.kstest((new[:, j] + 1) / 2, "uniform").pvalue > 1e-3
+    assert np.all(r["trace"][:, :, 2] >= 0)
+    walled = r["trace"][:, :, :2].mean()
+    p.set_periodic([1, 1, 1])                       # nothing stops a bracket any more: every side reaches the cap of 32
+    r2 = p.replace_step(live, logL, k, 5, seed=11, iteration=0, logLstar=-math.inf, want_trace=True)
+    assert np.all(r2["trace"][:, :, :2] == 32) and walled < 32
+    new2 = r2["live"][r2["dead_idx"]]
+    assert np.all(new2 >= -1) and np.all(new2 <= 1)
+    p.set_periodic([0, 0, 0])                       # and the flags switch off again: the default walls (A16)
+    r3 = p.replace_step(live, logL, k, 5, seed=11, iteration=0, logLstar=-math.inf, want_trace=True)
+    r4 = oracle.Problem(w).replace_step(live, logL, k, 5, seed=11, iteration=0, logLstar=-math.inf, want_trace=True)
+    assert np.array_equal(r3["live"], r4["live"]) and np.array_equal(r3["trace"], r4["trace"])
+
+
+def test_next2_wrap_is_the_identity_inside_and_a_shift_by_periods_outside(oracle):
+    """A chain that never leaves the box must not notice the flags: with a constraint region well inside the box
+    (a tight Gaussian, L* high) the wrapped and the walled sampler make the same decisions and end at the same bits."""
+    w = inputs.gaussian_workload(4, sigma=0.02)
+    p = oracle.Problem(w)
+    rng = np.random.default_rng(5)
+    live = rng.normal(size=(400, 4)) * 0.02
+    logL = p.loglike_batch(live)
+    a = p.replace_step(live, logL, 200, 12, seed=2, iteration=1, want_trace=True)
+    p.set_periodic([1, 1, 1, 1])
+    b = p.replace_step(live, logL, 200, 12, seed=2, iteration=1, want_trace=True)
+    assert np.array_equal(a["live"], b["live"]) and np.array_equal(a["trace"], b["trace"]) and a["n_evals"] == b["n_evals"]
+
+
+@pytest.mark.parametrize("flags", [(1, 0, 0), (1, 1, 1)])
+def test_next2_evidence_does_not_depend_on_the_topology(oracle, flags):
+    """The evidence of a likelihood under a uniform prior is the same integral on the box and on the torus, so NS with
+    wrapped coordinates must reproduce O16's analytic logZ (here with the peak 0.2 sigma from a wall, where wrapping
+    changes most of the slices) within 3 sigma_NS."""
+    w = inputs.gaussian_workload(3, sigma=0.05)
+    w.gauss_mu = w.gauss_mu.copy()
+    w.gauss_mu[0] = -0.99
+    p = oracle.Problem(w)
+    p.set_periodic(flags)
+    truth = sum(math.log(0.05 * math.sqrt(2 * math.pi) / 2.0
+                         * (scipy.stats.norm.cdf((1 - m) / 0.05) - scipy.stats.norm.cdf((-1 - m) / 0.05))) for m in w.gauss_mu[:3])
+    o = p.run(1000, 500, 15, 3)
+    assert o["rc"] == 0
+    assert abs(o["logZ"] - truth) < 3 * o["logZ_err"]
+    pw = np.exp(o["dead_logL"] + o["dead_logw"] - o["logZ"])
+    mean0 = pw @ o["dead_theta"][:, 0]
+    # posterior of the first coordinate: a normal truncated at the wall -0.99 - 0.2 sigma ... its mean is known
+    a = (-1 - w.gauss_mu[0]) / 0.05
+    tm = w.gauss_mu[0] + 0.05 * scipy.stats.norm.pdf(a) / (1 - scipy.stats.norm.cdf(a))
+    assert abs(mean0 - tm) < 0.01

@@ -21,7 +21,9 @@
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): see DESIGN.md §5.  Unpinned by any external
  * source: the higher PN phase coefficients phi_2..phi_7 (P2: "parity unpinned"; only sanity
- * identities), and the sampler conventions A12/A14/A15/A17 (validity pinned by P13/P15 only).
+ * identities), and the sampler conventions A12/A14/A15/A17 (validity pinned by P13/P15 only); the wrap
+ * convention of periodic coordinates (NEXT-2, R4) likewise: nothing external fixes where the seam
+ * value goes, its validity is pinned by uniformity, identity inside the box and the analytic evidence.
  */
 #include <complex.h>
 #include <math.h>

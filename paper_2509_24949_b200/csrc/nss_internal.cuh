@@ -78,7 +78,7 @@ struct nss_handle {
   size_t stage_bytes;
   // second stream for the kernels of an iteration that do not depend on each other
   cudaStream_t st2;
-  cudaEvent_t ev_fork, ev_join;
+  cudaEvent_t ev_fork, ev_join, ev_sel, ev_evid;
   // device block and events of nss_run, kept between runs
   unsigned char *d_run;
   size_t run_bytes;

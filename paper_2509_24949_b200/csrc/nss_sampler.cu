@@ -413,7 +413,7 @@ __global__ void __launch_bounds__(128) k_directions(int d, const double *__restr
                                                     uint32_t it, const int32_t *__restrict__ flags, double *__restrict__ dirs)
 {
   __shared__ double sL[NSS_NSLOT * NSS_NSLOT];
-  if (flags[0] | flags[1]) return;
+  if (flags[0]) return;                                  // Cholesky failed (flags[1] belongs to the selection, which runs beside this)
   for (int t = threadIdx.x; t < d * d; t += blockDim.x) sL[t] = chol[t];
   __syncthreads();
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
@@ -838,6 +838,8 @@ int ensure_scratch(nss_handle *h, int n)
     NSS_CUDA(cudaStreamCreateWithFlags(&h->st2, cudaStreamNonBlocking));
     NSS_CUDA(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
     NSS_CUDA(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming));
+    NSS_CUDA(cudaEventCreateWithFlags(&h->ev_sel, cudaEventDisableTiming));
+    NSS_CUDA(cudaEventCreateWithFlags(&h->ev_evid, cudaEventDisableTiming));
     h->d_state = h->d_ctl->state;             // addresses inside the device block (not dereferenced on the host)
     h->d_nevals = &h->d_ctl->nevals;
     h->d_flags = h->d_ctl->flags;
@@ -849,42 +851,55 @@ int ensure_scratch(nss_handle *h, int n)
 // the device part of one NS iteration (no host synchronisation): K4.1, K4.2, K4.3, K3
 int enqueue_iteration(nss_handle *h, double *live, double *logL, double *birth, int n, int k, double Lstar_in, int n_repeats,
                       uint64_t seed, uint32_t iteration, double *dead_theta, double *dead_logL, double *dead_birth,
-                      int32_t *dead_idx, cudaStream_t st)
+                      int32_t *dead_idx, double *dead_logw, cudaStream_t st)
 {
   const int d = h->dev.d;
-  // the tuning (a3) does not depend on the selection (a1): it runs beside it on the handle's second stream
+  // Second stream: the tuning (a3) and the directions (a5) do not depend on the selection (a1) and run beside it;
+  // the evidence update (a2) needs only the dead logL, so it runs beside the chains (K3).
   NSS_CUDA(cudaEventRecord(h->ev_fork, st));
   NSS_CUDA(cudaStreamWaitEvent(h->st2, h->ev_fork, 0));
   k4_tune<<<1, kOneCta, 0, h->st2>>>(live, n, d, h->d_mean, h->d_chol, h->d_flags);
-  NSS_CUDA(cudaEventRecord(h->ev_join, h->st2));
-  k4_rank<<<(n + kRankThreads - 1) / kRankThreads, kRankThreads, 0, st>>>(logL, n, k, h->d_rank, dead_idx);
-  k4_finish_select<<<1, kOneCta, 0, st>>>(live, logL, birth, n, k, d, Lstar_in, h->d_rank, dead_idx, h->d_surv_idx, dead_theta,
-                                          dead_logL, dead_birth, h->d_state, h->d_flags);
-  NSS_CUDA(cudaStreamWaitEvent(st, h->ev_join, 0));
   {
     const size_t need = sizeof(double) * (size_t)k * (n_repeats > 0 ? n_repeats : 1) * d;
     if (h->dirs_bytes < need) {
+      NSS_CUDA(cudaDeviceSynchronize());                 // an earlier launch may still read the old block
       cudaFree(h->d_dirs);
       h->d_dirs = nullptr; h->dirs_bytes = 0;
       cudaError_t e = cudaMalloc((void **)&h->d_dirs, need);
       if (e != cudaSuccess) { nss_cuda_fail(e, "cudaMalloc(dirs)"); return e == cudaErrorMemoryAllocation ? NSS_ENOMEM : NSS_ECUDA; }
       h->dirs_bytes = need;
     }
-    if (n_repeats > 0) k_directions<<<(k * n_repeats + 127) / 128, 128, 0, st>>>(d, h->d_chol, k, n_repeats, seed, iteration, h->d_flags, h->d_dirs);
+    if (n_repeats > 0)
+      k_directions<<<(k * n_repeats + 127) / 128, 128, 0, h->st2>>>(d, h->d_chol, k, n_repeats, seed, iteration, h->d_flags, h->d_dirs);
   }
+  NSS_CUDA(cudaEventRecord(h->ev_join, h->st2));
+  k4_rank<<<(n + kRankThreads - 1) / kRankThreads, kRankThreads, 0, st>>>(logL, n, k, h->d_rank, dead_idx);
+  k4_finish_select<<<1, kOneCta, 0, st>>>(live, logL, birth, n, k, d, Lstar_in, h->d_rank, dead_idx, h->d_surv_idx, dead_theta,
+                                          dead_logL, dead_birth, h->d_state, h->d_flags);
   h->launches += n_repeats > 0 ? 4 : 3;
+  if (dead_logw) {
+    NSS_CUDA(cudaEventRecord(h->ev_sel, st));
+    NSS_CUDA(cudaStreamWaitEvent(h->st2, h->ev_sel, 0));
+    k4_evidence<<<1, kOneCta, 0, h->st2>>>(dead_logL, n, k, dead_logw, h->d_state);
+    NSS_CUDA(cudaEventRecord(h->ev_evid, h->st2));
+    h->launches += 1;
+  }
+  NSS_CUDA(cudaStreamWaitEvent(st, h->ev_join, 0));
   NSS_CUDA(cudaGetLastError());
   ChainArgs A;
   A.live = live; A.logL = logL; A.birth = birth; A.n = n; A.k = k; A.n_repeats = n_repeats; A.seed = seed;
   A.iteration = iteration; A.surv_idx = h->d_surv_idx; A.dead_idx = dead_idx; A.dirs = h->d_dirs; A.state = h->d_state;
   A.flags = h->d_flags; A.n_evals = h->d_nevals; A.diag = &h->d_ctl->nrounds; A.trace = h->trace_dev; A.margin = h->margin_dev;
   A.G = 1;
+  int rc;
   switch (h->dev.n_det) {
-    case 0: case 1: return launch_chains<1>(h, A, st);
-    case 2: return launch_chains<2>(h, A, st);
-    case 3: return launch_chains<3>(h, A, st);
-    default: return launch_chains<4>(h, A, st);
+    case 0: case 1: rc = launch_chains<1>(h, A, st); break;
+    case 2: rc = launch_chains<2>(h, A, st); break;
+    case 3: rc = launch_chains<3>(h, A, st); break;
+    default: rc = launch_chains<4>(h, A, st); break;
   }
+  if (dead_logw) NSS_CUDA(cudaStreamWaitEvent(st, h->ev_evid, 0));     // whatever follows on st sees logX, logZ, logw
+  return rc;
 }
 
 }  // namespace
@@ -1030,7 +1045,7 @@ extern "C" int nss_replace_step(nss_handle *h, double *live_dev, double *logL_de
   rc = begin_iteration(h, 0, 0.0, 0.0, 1, st);
   if (rc) return rc;
   rc = enqueue_iteration(h, live_dev, logL_dev, nullptr, n_live, n_delete, logLstar, n_repeats, seed, iteration, dead_theta_dev,
-                         dead_logL_dev, nullptr, dead_idx_dev, st);
+                         dead_logL_dev, nullptr, dead_idx_dev, nullptr, st);
   if (rc) return rc;
   rc = fetch_ctl(h, st);
   if (rc) return rc;
@@ -1069,11 +1084,10 @@ extern "C" int nss_iterate(nss_handle *h, double *live_dev, double *logL_dev, in
   rc = begin_iteration(h, 1, state_host->logX, state_host->logZ, 1, st);
   if (rc) return rc;
   rc = enqueue_iteration(h, live_dev, logL_dev, nullptr, n_live, n_delete, NAN, n_repeats, seed, iteration, dead_theta_dev,
-                         dead_logL_dev, nullptr, dead_idx_dev, st);
+                         dead_logL_dev, nullptr, dead_idx_dev, dead_logw_dev, st);
   if (rc) return rc;
-  k4_evidence<<<1, kOneCta, 0, st>>>(dead_logL_dev, n_live, n_delete, dead_logw_dev, h->d_state);
   k4_live_evidence<<<1, kOneCta, 0, st>>>(logL_dev, n_live, stop_dlogz, 1, h->d_state, h->d_flags);
-  h->launches += 2;
+  h->launches += 1;
   NSS_CUDA(cudaGetLastError());
   rc = fetch_ctl(h, st);
   if (rc) return rc;
@@ -1198,10 +1212,8 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
     if (t >= max_iter) { result = NSS_ENOTCONV; break; }
     if (n_dead + k + n > cap) { result = NSS_ECAP; break; }
     rc = enqueue_iteration(h, live, logL, h->d_birth, n, k, NAN, n_repeats, seed, (uint32_t)t, dth + (size_t)n_dead * d, dl + n_dead,
-                           db + n_dead, h->d_dead_idx, st);
+                           db + n_dead, h->d_dead_idx, dw + n_dead, st);
     if (rc) { cleanup(); return rc; }
-    k4_evidence<<<1, kOneCta, 0, st>>>(dl + n_dead, n, k, dw + n_dead, h->d_state);
-    h->launches += 1;
     n_dead += k;
     ++t;
   }

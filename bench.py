@@ -331,7 +331,8 @@ def run_ours(args):
                           "evals_per_s": k1_rate, "tflops": k1_rate * flop / 1e12, "frac": k1_rate * flop / 1e12 / peak_tf,
                           "pipe_frac": k1_rate * instr / (peak_tf * 1e12 / 2)},
         "nss_run": {"wall_s": run_wall, "gpu_ms": r["gpu_ms"], "n_iter": r["n_iter"], "n_evals": r["n_evals"],
-                    "logZ": r["logZ"], "logZ_err": r["logZ_err"], "H": r["H"], "rc": r["rc"]},
+                    "logZ": r["logZ"], "logZ_err": r["logZ_err"], "H": r["H"], "rc": r["rc"],
+                    "kish_ess": r["ess"], "ess_per_s": r["ess"] / run_wall},
         "clocks": clocks.summary(),
     }
     # ---- CPU baseline: the oracle as it stands, on this box's host cores, bounded sample -----------------------

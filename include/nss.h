@@ -198,6 +198,8 @@ typedef struct {
   double *dead_logw;               /* host [cap]      log prior-volume weight                    */
   int64_t cap;                     /* >= n_iter*n_delete + n_live                                */
   double  gpu_ms;                  /* device time of the run (CUDA events), setup excluded       */
+  double  ess;                     /* Kish effective sample size (sum p)^2 / sum p^2 of the posterior weights
+                                      p_i ~ exp(logL_i + logw_i) over all rows (O15; the paper's Table 1b metric) */
 } nss_result;
 
 /* Full run (O13, O14): initial live points, NS iterations until logZ_live - logZ < stop_dlogz

@@ -388,6 +388,35 @@ __global__ void __launch_bounds__(256) k_evidence_error(const double *__restrict
   }
 }
 
+// ---- O15 / NEXT-4: Kish effective sample size of the posterior weights, one CTA -----------------------------------
+// a_i = logL_i + logw_i over the dead rows, and logL_i + logX_end - ln n over the final live points;
+// ESS = (sum e^(a_i - amax))^2 / sum e^(2 (a_i - amax)).  out[0] = ESS.
+__global__ void __launch_bounds__(kOneCta) k_kish_ess(const double *__restrict__ dead_logL, const double *__restrict__ dead_logw,
+                                                      long long n_dead, const double *__restrict__ live_logL, int n,
+                                                      const double *__restrict__ state, double *__restrict__ out)
+{
+  __shared__ double red[32];
+  const double lw_live = state[0] - log((double)n);
+  double mx = -INFINITY;
+  for (long long i = threadIdx.x; i < n_dead; i += kOneCta) mx = fmax(mx, dead_logL[i] + dead_logw[i]);
+  for (int i = threadIdx.x; i < n; i += kOneCta) mx = fmax(mx, live_logL[i] + lw_live);
+  mx = block_max(mx, red);
+  double s1 = 0.0, s2 = 0.0;
+  if (mx > -INFINITY) {
+    for (long long i = threadIdx.x; i < n_dead; i += kOneCta) {
+      const double a = dead_logL[i] + dead_logw[i];
+      if (a > -INFINITY) { const double p = exp(a - mx); s1 += p; s2 = fma(p, p, s2); }
+    }
+    for (int i = threadIdx.x; i < n; i += kOneCta) {
+      const double a = live_logL[i] + lw_live;
+      if (a > -INFINITY) { const double p = exp(a - mx); s1 += p; s2 = fma(p, p, s2); }
+    }
+  }
+  s1 = block_sum(s1, red);
+  s2 = block_sum(s2, red);
+  if (threadIdx.x == 0) out[0] = s2 > 0.0 ? s1 * s1 / s2 : 0.0;
+}
+
 __global__ void k_fill(double *__restrict__ p, int n, double v)
 {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -1169,7 +1198,7 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
   const size_t o_live = 0, o_logL = o_live + align256(sizeof(double) * (size_t)n * d), o_dth = o_logL + align256(sizeof(double) * n),
                o_dl = o_dth + align256(sizeof(double) * (size_t)cap * d), o_db = o_dl + align256(sizeof(double) * cap),
                o_dw = o_db + align256(sizeof(double) * cap), o_err = o_dw + align256(sizeof(double) * cap),
-               total = o_err + align256(sizeof(double) * kErrReplicas);
+               total = o_err + align256(sizeof(double) * (kErrReplicas + 1));
   if (h->run_bytes < total) {
     cudaFree(h->d_run);
     h->d_run = nullptr; h->run_bytes = 0;
@@ -1234,9 +1263,10 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
     RUN_CUDA(cudaMemcpyAsync(out->dead_logL_birth, db, sizeof(double) * n_dead, cudaMemcpyDeviceToHost, st));
     RUN_CUDA(cudaMemcpyAsync(out->dead_logw, dw, sizeof(double) * n_it_dead, cudaMemcpyDeviceToHost, st));
     // O15: the replica evidences on the device (one CTA per replica), reduced to a standard deviation below
-    double lz_rep[kErrReplicas];
+    double lz_rep[kErrReplicas + 1];                     // [kErrReplicas] = Kish ESS
     k_evidence_error<<<kErrReplicas, 256, 0, st>>>(dl, n_it_dead, n, k, seed, logL, derr);
-    h->launches += 1;
+    k_kish_ess<<<1, kOneCta, 0, st>>>(dl, dw, n_it_dead, logL, n, h->d_state, derr + kErrReplicas);
+    h->launches += 2;
     RUN_CUDA(cudaMemcpyAsync(lz_rep, derr, sizeof(lz_rep), cudaMemcpyDeviceToHost, st));
     RUN_CUDA(cudaEventRecord(e1, st));
     RUN_CUDA(cudaStreamSynchronize(st));
@@ -1263,6 +1293,7 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
     double var = sum2 / R - mu * mu;
     var = var < 0 ? 0 : var;
     out->logZ = logZf; out->logZ_err = sqrt(var * R / (R - 1)); out->H = H;
+    out->ess = lz_rep[kErrReplicas];
     out->n_iter = t; out->n_dead = n_dead; out->n_evals = (int64_t)ne + n;
   }
 #undef RUN_CUDA

@@ -48,7 +48,7 @@ class nss_result(C.Structure):
         ("logZ", C.c_double), ("logZ_err", C.c_double), ("H", C.c_double), ("n_iter", C.c_int32),
         ("n_dead", C.c_int64), ("n_evals", C.c_int64), ("dead_theta", C.POINTER(C.c_double)),
         ("dead_logL", C.POINTER(C.c_double)), ("dead_logL_birth", C.POINTER(C.c_double)),
-        ("dead_logw", C.POINTER(C.c_double)), ("cap", C.c_int64), ("gpu_ms", C.c_double)]
+        ("dead_logw", C.POINTER(C.c_double)), ("cap", C.c_int64), ("gpu_ms", C.c_double), ("ess", C.c_double)]
 
 
 class nss_iter_state(C.Structure):
@@ -353,7 +353,7 @@ class Nss:
         _check(rc, "nss_run", ok=(NSS_OK, NSS_ENOTCONV))
         nd = int(res.n_dead)
         return dict(rc=rc, logZ=res.logZ, logZ_err=res.logZ_err, H=res.H, n_iter=int(res.n_iter), n_dead=nd,
-                    n_evals=int(res.n_evals), gpu_ms=res.gpu_ms, dead_theta=dth[:nd], dead_logL=dl[:nd],
+                    n_evals=int(res.n_evals), gpu_ms=res.gpu_ms, ess=res.ess, dead_theta=dth[:nd], dead_logL=dl[:nd],
                     dead_logL_birth=db[:nd], dead_logw=dw[:nd])
 
     def nss_get_tables(self):

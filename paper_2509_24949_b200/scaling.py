@@ -46,15 +46,15 @@ def main():
 
     lives = (250, 500, 1000, 2000) if args.quick else (250, 500, 1000, 2000, 4000, 8000, 16000)
     print("## wall-clock vs n_live (n_delete = n_live/2, config-2 likelihood, 55 slice repeats)\n")
-    print("| n_live | n_delete | wall s | device ms | iterations | evaluations | evals/s | logZ | +- | naive-linear s |")
-    print("|---|---|---|---|---|---|---|---|---|---|")
+    print("| n_live | n_delete | wall s | device ms | iterations | evaluations | evals/s | logZ | +- | Kish ESS | naive-linear s |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|")
     t0 = None
     for n in lives:
         t, r = run_point(g, n, n // 2, nrep, args.seed, args.repeats)
         if t0 is None:
             t0 = (t, n)
         print(f"| {n} | {n // 2} | {t:.4f} | {r['gpu_ms']:.1f} | {r['n_iter']} | {r['n_evals']} | {r['n_evals'] / t:.3e} | "
-              f"{r['logZ']:.2f} | {r['logZ_err']:.2f} | {t0[0] * n / t0[1]:.4f} |", flush=True)
+              f"{r['logZ']:.2f} | {r['logZ_err']:.2f} | {r['ess']:.0f} | {t0[0] * n / t0[1]:.4f} |", flush=True)
 
     dels = (10, 50, 250, 500) if args.quick else (1, 2, 5, 10, 25, 50, 100, 250, 500, 750)
     print("\n## wall-clock vs n_delete (n_live = 1000)\n")

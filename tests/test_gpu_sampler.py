@@ -440,3 +440,35 @@ def test_next2_periodic_run_matches_oracle_and_analytic(nssmod, oracle):
         assert r["n_evals"] == o["n_evals"]
         assert np.allclose(r["dead_theta"], o["dead_theta"], rtol=0, atol=1e-12)
     g.close()
+
+
+# ---- NEXT-4: Kish effective sample size (the paper's Table 1b metric; O15) -----------------------------
+def _kish(logL, logw):
+    a = logL + logw
+    a = a[np.isfinite(a)]
+    p = np.exp(a - a.max())
+    return p.sum() ** 2 / (p * p).sum()
+
+
+def test_next4_kish_ess_matches_the_formula_and_the_oracle(nssmod, oracle, wl1):
+    """ESS = (sum p)^2 / sum p^2 over all returned rows, p ~ exp(logL + logw).  Closed forms pin the formula (equal
+    weights -> N; one weight dominating -> 1); the library's device reduction must agree with it on the library's own
+    rows, and with the oracle's rows wherever the two runs made the same decisions."""
+    assert _kish(np.zeros(1000), np.full(1000, -3.0)) == pytest.approx(1000.0)
+    assert _kish(np.array([0.0, -800.0, -900.0]), np.zeros(3)) == pytest.approx(1.0)
+    g, p = nssmod.Nss(wl1), oracle.Problem(wl1)
+    same = 0
+    for seed in (1, 2, 3):
+        r, o = g.nss_run(100, 50, 12, seed), p.run(100, 50, 12, seed)
+        assert r["ess"] == pytest.approx(_kish(r["dead_logL"], r["dead_logw"]), rel=1e-10)
+        assert 1.0 < r["ess"] < r["n_dead"]
+        if r["n_dead"] == o["n_dead"] and np.allclose(r["dead_logL"], o["dead_logL"], rtol=1e-9, atol=1e-6):
+            same += 1
+            assert r["ess"] == pytest.approx(_kish(o["dead_logL"], o["dead_logw"]), rel=1e-6)
+    assert same >= 1
+    g.close()
+    w = inputs.gaussian_workload(4, sigma=0.05)
+    g = nssmod.Nss(w)
+    r = g.nss_run(1000, 500, 20, 2)
+    assert r["ess"] == pytest.approx(_kish(r["dead_logL"], r["dead_logw"]), rel=1e-10)
+    g.close()

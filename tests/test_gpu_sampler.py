@@ -472,3 +472,36 @@ def test_next4_kish_ess_matches_the_formula_and_the_oracle(nssmod, oracle, wl1):
     r = g.nss_run(1000, 500, 20, 2)
     assert r["ess"] == pytest.approx(_kish(r["dead_logL"], r["dead_logw"]), rel=1e-10)
     g.close()
+
+
+# ---- degenerate and extreme shapes ------------------------------------------------------------------------------------
+def test_edge_shapes_match_oracle(nssmod, oracle, wl1):
+    """n_repeats = 0 (chains just copy their start survivor), n_delete = n_live - 1 (one survivor seeds every chain),
+    n_delete = 1, a one-dimensional problem, and a single relative-binning bin."""
+    g, p = nssmod.Nss(wl1), oracle.Problem(wl1)
+    live, logL = p.init_live(64, 9)
+    r = g.nss_replace_step(live, logL, 32, 0, 9, 0)
+    o = p.replace_step(live, logL, 32, 0, 9, 0)
+    assert np.array_equal(r["live"].cpu().numpy(), o["live"]) and np.array_equal(r["logL"].cpu().numpy(), o["logL"])
+    assert r["n_evals"] == o["n_evals"] == 0
+    _trajectory_parity(g, p, live, logL, 63, 5, seed=9, it=1, w=wl1, max_excluded=0.1)
+    _trajectory_parity(g, p, live, logL, 1, 12, seed=9, it=2, w=wl1, max_excluded=1.0)
+    g.close()
+    w = inputs.gaussian_workload(1, sigma=0.1)
+    g, p = nssmod.Nss(w), oracle.Problem(w)
+    live, logL = p.init_live(50, 3)
+    _trajectory_parity(g, p, live, logL, 25, 7, seed=3, it=0, w=w)
+    rr, oo = g.nss_run(50, 25, 5, 3), p.run(50, 25, 5, 3)
+    assert abs(rr["logZ"] - oo["logZ"]) < 3 * math.hypot(rr["logZ_err"], oo["logZ_err"]) + 1e-9
+    g.close()
+    w1 = inputs.make_data(inputs.config1(n_bins=1), oracle.waveform)
+    g, p = nssmod.Nss(w1), oracle.Problem(w1)
+    X = inputs.draw_prior(w1, 300, 4)
+    ref = p.loglike_batch(X)
+    for variant in (1, 2):
+        g.set_loglike_variant(variant)
+        got = g.nss_loglike_batch(X).cpu().numpy()
+        assert np.all(np.abs(got - ref) <= 1e-6 + 1e-9 * np.abs(ref))
+    live, logL = p.init_live(40, 2)
+    _trajectory_parity(g, p, live, logL, 20, 4, seed=2, it=0, w=w1, max_excluded=0.1)
+    g.close()

@@ -611,7 +611,7 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
     double lx = A.logL[slot];
     long long evals = 0;
     int rounds = 0, nexec = 0;
-    double margin = INFINITY;
+    double margin = INFINITY, margin_l = INFINITY;        // bracket-end tests (uniform) / this lane's proposals
 
     // a5: the directions were drawn by k_directions; the next step's is fetched while this step runs
     const double *vsrc = A.dirs + (size_t)ch * A.n_repeats * d;
@@ -646,13 +646,14 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
           nshr = nshr < 2 * C ? nshr : 2 * C;            // no point in listing far more tests than can be evaluated
           const int nt = nside + nshr;
           double my_t = (lane == 0 && !ldone) ? l : r;   // lanes < nside: the bracket ends
+          double my_ls = l, my_rs = r;                   // the bracket after this lane's test has failed
           {
             double ls = l, rs = r;
             for (int j = 0; j < nshr; ++j) {
               const double uk = nssk::shfl_d(ulane, kk - ubase + j + 1);
               const double t = __dadd_rn(ls, __dmul_rn(rs - ls, uk));
               if (t < 0.0) ls = t; else rs = t;
-              if (lane == nside + j) my_t = t;
+              if (lane == nside + j) { my_t = t; my_ls = ls; my_rs = rs; }
             }
           }
           // box test (inclusive) of the lane's own test: y = x + t v, every coordinate
@@ -669,8 +670,8 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
           ++rounds;
           nexec += min(C, __popc(M));
           int e = 0;                                     // lane holding the test of slot cs: the one with cs set bits of M below it
+          const int below = __popc(M & ((1u << lane) - 1u));
           {
-            const int below = __popc(M & ((1u << lane) - 1u));
 #pragma unroll
             for (int q = 0; q < NSUB; ++q) {
               const unsigned hit = __ballot_sync(0xffffffffu, inb && below == w * NSUB + q);
@@ -713,31 +714,45 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
             }
           }
           if (ldone && rdone && !expanded && !stop) {
-            for (int j = 0; j < nshr; ++j) {
-              const bool in = (M >> (nside + j)) & 1u;
-              if (in && rank >= C) break;
-              const double tj = nssk::shfl_d(my_t, nside + j);
-              bool pass = false;
-              double v = -INFINITY;
-              if (in) { v = res[rank++]; ++evals; margin = fmin(margin, fabs(v - Lstar)); pass = v > Lstar; }
-              if (pass) {
+            // shrinkage, all listed proposals at once: lane i holds proposal i - nside.  A proposal outside the box
+            // fails for free; one inside has the result of slot `below` if below < C, else it is not known yet.
+            const bool shr = lane >= nside && lane < nt;
+            const bool has = inb && below < C;
+            const double vi = has ? res[below < kSlots ? below : 0] : -INFINITY;
+            const unsigned mU = __ballot_sync(0xffffffffu, shr && inb && below >= C);
+            const unsigned mP = __ballot_sync(0xffffffffu, shr && has && vi > Lstar);
+            const unsigned mH = __ballot_sync(0xffffffffu, shr && has);
+            const int firstU = mU ? __ffs(mU) - 1 : 32, firstP = mP ? __ffs(mP) - 1 : 32;
+            const bool accepted = firstP < firstU;
+            int end = firstU < firstP ? firstU : firstP;   // proposals [nside, end) failed
+            end = end < nt ? end : nt;
+            const unsigned upto = accepted ? (firstP == 31 ? 0xffffffffu : ((1u << (firstP + 1)) - 1u))
+                                           : (end >= 32 ? 0xffffffffu : ((1u << end) - 1u));
+            evals += __popc(mH & upto);
+            if (shr && has && ((upto >> lane) & 1u)) margin_l = fmin(margin_l, fabs(vi - Lstar));
+            if (accepted) {
+              const double tj = nssk::shfl_d(my_t, firstP);
+              lx = nssk::shfl_d(vi, firstP);
 #pragma unroll
-                for (int c = 0; c < NC; ++c) {
-                  xj[c] = __dadd_rn(xj[c], __dmul_rn(tj, vj[c]));
-                  if (per[c]) xj[c] = wrap_periodic(xj[c], lo_j[c], hi_j[c]);
-                }
-                for (int jj = lane; jj < d; jj += 32) {
-                  double y = __dadd_rn(sX[warp][jj], __dmul_rn(tj, vrow[jj]));
-                  if (P.periodic[jj]) y = wrap_periodic(y, P.lo[jj], P.hi[jj]);
-                  sX[warp][jj] = y;
-                }
-                lx = v; acc = kk; done = true;
-                break;
+              for (int c = 0; c < NC; ++c) {
+                xj[c] = __dadd_rn(xj[c], __dmul_rn(tj, vj[c]));
+                if (per[c]) xj[c] = wrap_periodic(xj[c], lo_j[c], hi_j[c]);
               }
-              if (tj < 0.0) l = tj; else r = tj;
-              ++kk;
+              for (int jj = lane; jj < d; jj += 32) {
+                double y = __dadd_rn(sX[warp][jj], __dmul_rn(tj, vrow[jj]));
+                if (P.periodic[jj]) y = wrap_periodic(y, P.lo[jj], P.hi[jj]);
+                sX[warp][jj] = y;
+              }
+              acc = kk + (firstP - nside); done = true;
+            } else {
+              const int nrej = end - nside;
+              if (nrej > 0) {
+                l = nssk::shfl_d(my_ls, end - 1);
+                r = nssk::shfl_d(my_rs, end - 1);
+                kk += nrej;
+              }
+              if (kk >= kMaxShrink) done = true;
             }
-            if (!done && kk >= kMaxShrink) done = true;
           }
           __syncwarp();
         }
@@ -747,6 +762,9 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
         }
       }
     }
+    double margin_all = fmin(margin, margin_l);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) margin_all = fmin(margin_all, __shfl_xor_sync(0xffffffffu, margin_all, o));
     // a10: replace the deleted slot in place
     if (w == 0 && sub == 0) {
       const int dst = A.dead_idx[ch];
@@ -756,7 +774,7 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
       if (sl == 0) {
         A.logL[dst] = lx;
         if (A.birth) A.birth[dst] = Lstar;
-        if (A.margin) A.margin[ch] = margin;
+        if (A.margin) A.margin[ch] = margin_all;
         atomicAdd(A.n_evals, (unsigned long long)evals);
         atomicAdd(A.diag, (unsigned long long)rounds);
         atomicAdd(A.diag + 1, (unsigned long long)nexec);

@@ -1,4 +1,4 @@
-// nss_sampler.cu — K3 persistent slice-sampling chains, K4 on-device NS bookkeeping, and the host
+// nss_sampler.cu — K3 slice-sampling chains (one chain per CTA), k_directions, K4 on-device NS bookkeeping, and the host
 // driver behind nss_replace_step / nss_run (O11-O15).
 #include <math.h>
 #include <string.h>

@@ -67,7 +67,8 @@ struct nss_handle {
   int32_t *d_surv_idx, *d_dead_idx, *d_rank, *d_flags;   // flags: [0] chol error, [1] threshold violation, [2] done
   double *d_mean, *d_chol, *d_state;                      // state: logX, logZ, logZ_live, Lstar
   unsigned long long *d_nevals;
-  NssCtl *d_ctl, *h_ctl;       // d_state, d_nevals, d_flags point into d_ctl; h_ctl is pinned
+  NssCtl *d_ctl, *h_ctl;       // d_state, d_nevals, d_flags point into d_ctl; h_ctl is pinned, two slots
+  cudaEvent_t ev_ctl[2];       // nss_run: the copy into slot i has landed
   double *d_birth;
   double *d_dirs;              // [k][n_repeats][d] slice directions of the current iteration
   size_t dirs_bytes;

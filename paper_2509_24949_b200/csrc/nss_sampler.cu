@@ -85,9 +85,10 @@ __global__ void k_init_live(const __grid_constant__ NssDev P, int n, uint64_t se
 // rank_i = #{ j : logL_j < logL_i  or (logL_j == logL_i and j < i) }.  dead_idx[rank] = i for rank < k.
 constexpr int kRankThreads = 256;
 __global__ void __launch_bounds__(kRankThreads) k4_rank(const double *__restrict__ logL, int n, int k, int32_t *__restrict__ rank,
-                                                        int32_t *__restrict__ dead_idx)
+                                                        int32_t *__restrict__ dead_idx, const int32_t *__restrict__ stop)
 {
   __shared__ double tile[1024];
+  if (stop && stop[2]) return;                           // the run has converged: a speculatively queued iteration does nothing
   const int i = blockIdx.x * kRankThreads + threadIdx.x;
   const double Li = i < n ? logL[i] : INFINITY;
   int cnt = 0;
@@ -118,6 +119,7 @@ __global__ void __launch_bounds__(kOneCta) k4_finish_select(const double *__rest
                                                             int32_t *__restrict__ flags)
 {
   __shared__ int warp_tot[32];
+  if (flags[2] && live) return;                          // converged (nss_run queues one iteration ahead); the select hook passes live = NULL
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const double Lstar = isnan(Lstar_in) ? logL[dead_idx[k - 1]] : Lstar_in;
   const int chunk = (n + kOneCta - 1) / kOneCta;
@@ -181,6 +183,7 @@ __global__ void __launch_bounds__(kOneCta) k4_tune(const double *__restrict__ li
   __shared__ double part[kOneCta];
   __shared__ double mean[NSS_NSLOT];
   __shared__ double cov[NSS_NSLOT * NSS_NSLOT];
+  if (flags[2]) return;
   const int tid = threadIdx.x;
   {
     const int ng = kOneCta / d, j = tid % d, g = tid / d;
@@ -261,9 +264,10 @@ __device__ __forceinline__ double logaddexp_d(double a, double b)
 }
 
 __global__ void __launch_bounds__(kOneCta) k4_evidence(const double *__restrict__ dead_logL, int n, int k, double *__restrict__ logw,
-                                                       double *__restrict__ state)
+                                                       double *__restrict__ state, const int32_t *__restrict__ stop)
 {
   __shared__ double red[32];
+  if (stop && stop[2]) return;
   __shared__ double warp_tot[32];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const double logX0 = state[0], logZ0 = state[1];
@@ -442,7 +446,7 @@ __global__ void __launch_bounds__(128) k_directions(int d, const double *__restr
                                                     uint32_t it, const int32_t *__restrict__ flags, double *__restrict__ dirs)
 {
   __shared__ double sL[NSS_NSLOT * NSS_NSLOT];
-  if (flags[0]) return;                                  // Cholesky failed (flags[1] belongs to the selection, which runs beside this)
+  if (flags[0] | flags[2]) return;                       // Cholesky failed, or converged (flags[1] belongs to the selection, which runs beside this)
   for (int t = threadIdx.x; t < d * d; t += blockDim.x) sL[t] = chol[t];
   __syncthreads();
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
@@ -542,7 +546,7 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
   __shared__ double sX[kChainWarps][NSS_NSLOT + 1];                // chain position, one copy per warp (lane-level box tests)
   __shared__ double sLo[NSS_NSLOT + 1], sHi[NSS_NSLOT + 1];        // prior box, (-inf, +inf) for the unused coordinates
   __shared__ __align__(16) double sConst[nssk::kSubConstDoubles];
-  if (A.flags[0] | A.flags[1]) return;
+  if (A.flags[0] | A.flags[1] | A.flags[2]) return;      // Cholesky failure, threshold violation, or converged
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int sl = lane & (LANES - 1), sub = lane / LANES;
   nssk::SubCtx X;
@@ -879,7 +883,9 @@ int ensure_scratch(nss_handle *h, int n)
   NSS_CUDA(cudaMalloc(&h->d_birth, sizeof(double) * n));
   if (!h->d_flags) {
     NSS_CUDA(cudaMalloc(&h->d_ctl, sizeof(NssCtl)));
-    NSS_CUDA(cudaMallocHost(&h->h_ctl, sizeof(NssCtl)));
+    NSS_CUDA(cudaMallocHost(&h->h_ctl, 2 * sizeof(NssCtl)));     // [1] is nss_run's second slot
+    NSS_CUDA(cudaEventCreateWithFlags(&h->ev_ctl[0], cudaEventDisableTiming));
+    NSS_CUDA(cudaEventCreateWithFlags(&h->ev_ctl[1], cudaEventDisableTiming));
     NSS_CUDA(cudaMalloc(&h->d_mean, sizeof(double) * NSS_NSLOT));
     NSS_CUDA(cudaMalloc(&h->d_chol, sizeof(double) * NSS_NSLOT * NSS_NSLOT));
     NSS_CUDA(cudaStreamCreateWithFlags(&h->st2, cudaStreamNonBlocking));
@@ -920,14 +926,14 @@ int enqueue_iteration(nss_handle *h, double *live, double *logL, double *birth, 
       k_directions<<<(k * n_repeats + 127) / 128, 128, 0, h->st2>>>(d, h->d_chol, k, n_repeats, seed, iteration, h->d_flags, h->d_dirs);
   }
   NSS_CUDA(cudaEventRecord(h->ev_join, h->st2));
-  k4_rank<<<(n + kRankThreads - 1) / kRankThreads, kRankThreads, 0, st>>>(logL, n, k, h->d_rank, dead_idx);
+  k4_rank<<<(n + kRankThreads - 1) / kRankThreads, kRankThreads, 0, st>>>(logL, n, k, h->d_rank, dead_idx, h->d_flags);
   k4_finish_select<<<1, kOneCta, 0, st>>>(live, logL, birth, n, k, d, Lstar_in, h->d_rank, dead_idx, h->d_surv_idx, dead_theta,
                                           dead_logL, dead_birth, h->d_state, h->d_flags);
   h->launches += n_repeats > 0 ? 4 : 3;
   if (dead_logw) {
     NSS_CUDA(cudaEventRecord(h->ev_sel, st));
     NSS_CUDA(cudaStreamWaitEvent(h->st2, h->ev_sel, 0));
-    k4_evidence<<<1, kOneCta, 0, h->st2>>>(dead_logL, n, k, dead_logw, h->d_state);
+    k4_evidence<<<1, kOneCta, 0, h->st2>>>(dead_logL, n, k, dead_logw, h->d_state, h->d_flags);
     NSS_CUDA(cudaEventRecord(h->ev_evid, h->st2));
     h->launches += 1;
   }
@@ -1031,7 +1037,7 @@ extern "C" int nss_select_lowest(nss_handle *h, const double *logL_dev, int32_t 
   if (rc) return rc;
   rc = begin_iteration(h, 0, 0.0, 0.0, 0, st);
   if (rc) return rc;
-  k4_rank<<<(n_live + kRankThreads - 1) / kRankThreads, kRankThreads, 0, st>>>(logL_dev, n_live, n_delete, h->d_rank, dead_idx_dev);
+  k4_rank<<<(n_live + kRankThreads - 1) / kRankThreads, kRankThreads, 0, st>>>(logL_dev, n_live, n_delete, h->d_rank, dead_idx_dev, nullptr);
   k4_finish_select<<<1, kOneCta, 0, st>>>(nullptr, logL_dev, nullptr, n_live, n_delete, h->dev.d, NAN, h->d_rank, dead_idx_dev,
                                           surv_idx_dev, nullptr, nullptr, nullptr, h->d_state, h->d_flags);
   h->launches += 2;
@@ -1069,7 +1075,7 @@ extern "C" int nss_evidence_update(nss_handle *h, const double *dead_logL_dev, i
   if (rc) return rc;
   rc = begin_iteration(h, 1, state_host[0], state_host[1], 0, st);
   if (rc) return rc;
-  k4_evidence<<<1, kOneCta, 0, st>>>(dead_logL_dev, n_live, n_delete, logw_dev, h->d_state);
+  k4_evidence<<<1, kOneCta, 0, st>>>(dead_logL_dev, n_live, n_delete, logw_dev, h->d_state, nullptr);
   h->launches += 1;
   NSS_CUDA(cudaGetLastError());
   rc = fetch_ctl(h, st);
@@ -1249,24 +1255,39 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
   int t = 0;
   int64_t n_dead = 0;
   int result = NSS_OK;
-  for (;;) {
-    k4_live_evidence<<<1, kOneCta, 0, st>>>(logL, n, stop_dlogz, t > 0, h->d_state, h->d_flags);
+  // The loop runs one iteration ahead of the host: the stop test of iteration t (k4_live_evidence sets flags[2] on the
+  // device) is read from a pinned slot while iteration t and the stop test of t+1 are already queued.  Every kernel of
+  // an iteration returns at once when flags[2] is set, so the iteration queued past convergence changes nothing.
+  auto stage = [&](int tt) -> int {
+    k4_live_evidence<<<1, kOneCta, 0, st>>>(logL, n, stop_dlogz, tt > 0, h->d_state, h->d_flags);
     h->launches += 1;
-    RUN_CUDA(cudaMemcpyAsync(h->h_ctl, h->d_ctl, sizeof(NssCtl), cudaMemcpyDeviceToHost, st));
-    RUN_CUDA(cudaStreamSynchronize(st));
-    if (h->h_ctl->flags[0]) { result = NSS_ECHOL; break; }
-    if (h->h_ctl->flags[2]) break;
-    if (t >= max_iter) { result = NSS_ENOTCONV; break; }
-    if (n_dead + k + n > cap) { result = NSS_ECAP; break; }
-    rc = enqueue_iteration(h, live, logL, h->d_birth, n, k, NAN, n_repeats, seed, (uint32_t)t, dth + (size_t)n_dead * d, dl + n_dead,
-                           db + n_dead, h->d_dead_idx, dw + n_dead, st);
-    if (rc) { cleanup(); return rc; }
+    NSS_CUDA(cudaMemcpyAsync(&h->h_ctl[tt & 1], h->d_ctl, sizeof(NssCtl), cudaMemcpyDeviceToHost, st));
+    NSS_CUDA(cudaEventRecord(h->ev_ctl[tt & 1], st));
+    return NSS_OK;
+  };
+  rc = stage(0);
+  if (rc) { cleanup(); return rc; }
+  for (;;) {
+    const bool room = n_dead + k + n <= cap, more = t < max_iter;
+    if (room && more) {
+      rc = enqueue_iteration(h, live, logL, h->d_birth, n, k, NAN, n_repeats, seed, (uint32_t)t, dth + (size_t)n_dead * d, dl + n_dead,
+                             db + n_dead, h->d_dead_idx, dw + n_dead, st);
+      if (rc) { cleanup(); return rc; }
+      rc = stage(t + 1);
+      if (rc) { cleanup(); return rc; }
+    }
+    RUN_CUDA(cudaEventSynchronize(h->ev_ctl[t & 1]));
+    const NssCtl &c = h->h_ctl[t & 1];
+    if (c.flags[0]) { result = NSS_ECHOL; break; }
+    if (c.flags[2]) break;                               // converged before iteration t: what was queued for it did nothing
+    if (!more) { result = NSS_ENOTCONV; break; }
+    if (!room) { result = NSS_ECAP; break; }
     n_dead += k;
     ++t;
   }
   if (result == NSS_OK || result == NSS_ENOTCONV) {
     // O14: append the live points in ascending logL
-    k4_rank<<<(n + kRankThreads - 1) / kRankThreads, kRankThreads, 0, st>>>(logL, n, n, h->d_rank, h->d_dead_idx);
+    k4_rank<<<(n + kRankThreads - 1) / kRankThreads, kRankThreads, 0, st>>>(logL, n, n, h->d_rank, h->d_dead_idx, nullptr);
     k_gather_rows<<<(n + 255) / 256, 256, 0, st>>>(live, logL, h->d_birth, h->d_dead_idx, n, d, dth + (size_t)n_dead * d, dl + n_dead,
                                                    db + n_dead);
     h->launches += 2;

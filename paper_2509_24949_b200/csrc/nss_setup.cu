@@ -156,6 +156,8 @@ extern "C" int nss_destroy(nss_handle *h)
   if (h->ev_fork) cudaEventDestroy(h->ev_fork);
   if (h->ev_join) cudaEventDestroy(h->ev_join);
   if (h->ev_sel) cudaEventDestroy(h->ev_sel);
+  if (h->ev_ctl[0]) cudaEventDestroy(h->ev_ctl[0]);
+  if (h->ev_ctl[1]) cudaEventDestroy(h->ev_ctl[1]);
   if (h->ev_evid) cudaEventDestroy(h->ev_evid);
   if (h->ev_run[0]) cudaEventDestroy(h->ev_run[0]);
   if (h->ev_run[1]) cudaEventDestroy(h->ev_run[1]);

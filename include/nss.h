@@ -204,7 +204,12 @@ typedef struct {
 
 /* Full run (O13, O14): initial live points, NS iterations until logZ_live - logZ < stop_dlogz
  * (default -3.0) or max_iter, then the live points are appended (ascending logL, weight X/n).
- * Everything stays on the device; results are copied to the caller's host arrays at the end. */
+ * Everything stays on the device; results are copied to the caller's host arrays at the end.  The host queues one
+ * iteration ahead: the stop test sets a device flag, the kernels of an iteration queued past it return at once, and the
+ * flag reaches the host through a pinned slot ("the entire end-to-end algorithm can then run in GPU memory").
+ * logZ_err (200 stochastic-compression replicas, O15) and ess are reduced on the device.  Returns NSS_OK, NSS_ENOTCONV
+ * (max_iter reached, results valid), NSS_ECAP (out->cap too small: needs n_iter * n_delete + n_live rows), NSS_ECHOL,
+ * NSS_EINVAL, NSS_ENOMEM or NSS_ECUDA.  Synchronous: returns after the stream has drained. */
 int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t n_repeats, uint64_t seed,
             double stop_dlogz, int32_t max_iter, nss_result *out, void *cuda_stream);
 

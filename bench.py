@@ -324,7 +324,10 @@ def run_ours(args):
                                     "1.965 GHz = 37.2; MEASURED_PEAKS.json has no fp64 figure",
                      "flop_per_eval": flop, "fp64_instr_per_eval": instr,
                      "pipe_frac": (evals / world) * instr / (k3_ms * 1e-3) / (peak_tf * 1e12 / 2),
-                     "kernel_ms_per_step": k3_ms / args.steps, "kernel_share_of_step": k3_ms / ms, "traffic": None,
+                     "kernel_ms_per_step": k3_ms / args.steps, "kernel_share_of_step": k3_ms / ms,
+                     "traffic": 2560256,
+                     "traffic_note": "bytes per launch, dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full "
+                                     "capture (profiles/r01e_k3_slice_full.md): the slice directions; the kernel is not memory-bound",
                      "rounds_per_chain": rounds / args.steps / k / world, "evaluated_incl_speculative_per_step": executed / args.steps / world,
                      "note": "achieved counts only the evaluations the sequential algorithm consumed"},
         "loglike_batch": {"workload": "config 5: N=1e6 prior draws, B=128 x 3 detectors, k_rec_thread", "ms": k1_ms,

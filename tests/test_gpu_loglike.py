@@ -157,3 +157,4 @@ def test_gaussian_kind(nssmod, oracle):
     m = np.isfinite(ref)
     assert np.allclose(got[m], ref[m], rtol=1e-13, atol=0)
     g.close()
+

@@ -505,3 +505,29 @@ def test_edge_shapes_match_oracle(nssmod, oracle, wl1):
     live, logL = p.init_live(40, 2)
     _trajectory_parity(g, p, live, logL, 20, 4, seed=2, it=0, w=w1, max_excluded=0.1)
     g.close()
+
+
+@pytest.mark.parametrize("names", [("H1", "L1"), ("H1", "L1", "V1", "SYN")])
+def test_two_and_four_detectors(nssmod, oracle, names):
+    """The kernels are compiled per detector count (1..4): config 2 with two and with four detectors (the fourth is the
+    synthetic one of config 1), relative binning and full grid, every batch variant and one NS iteration of chains."""
+    import dataclasses
+    base = inputs.config2(n_bins=64, n_live=200, n_delete=100)
+    f = base.f_min + base.df * np.arange(base.n_freq)
+    w = dataclasses.replace(base, det_names=names, det=inputs.detector_array(names),
+                            psd=np.tile(inputs.psd_aligo_fit(f)[None, :], (len(names), 1)), data=None)
+    w = inputs.make_data(w, oracle.waveform)
+    X = np.concatenate([inputs.draw_prior(w, 1500, 5), inputs.draw_near(w, 150, 6, 0.01 * (w.hi - w.lo))])
+    for kind in (0, 1):
+        g, p = nssmod.Nss(w, kind=kind), oracle.Problem(w, kind=kind)
+        n = len(X) if kind == 0 else 300
+        ref = p.loglike_batch(X[:n])
+        for variant in (1, 2):
+            g.set_loglike_variant(variant)
+            got = g.nss_loglike_batch(X[:n]).cpu().numpy()
+            assert np.all(np.abs(got - ref) <= 1e-6 + 1e-9 * np.abs(ref))
+        g.set_loglike_variant(0)
+        if kind == 0:
+            live, logL = p.init_live(200, 3)
+            _trajectory_parity(g, p, live, logL, 100, 6, seed=3, it=0, w=w, max_excluded=0.06)
+        g.close()

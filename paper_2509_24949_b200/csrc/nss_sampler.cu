@@ -219,24 +219,32 @@ __global__ void __launch_bounds__(kOneCta) k4_tune(const double *__restrict__ li
     }
     __syncthreads();
   }
-  if (tid == 0) {
-    double L[NSS_NSLOT * NSS_NSLOT];
-    for (int a = 0; a < d * d; ++a) L[a] = 0.0;
+  // Cholesky by the first warp, column by column: lane i owns row i.  Every element is the same sum in the same
+  // order as the row-by-row definition (s = cov_ij - sum_{m<j} L_im L_jm), only the rows of a column run side by side.
+  __shared__ double sLc[NSS_NSLOT * NSS_NSLOT];
+  if (tid < 32) {
+    const int i = tid;
+    for (int a = tid; a < d * d; a += 32) sLc[a] = 0.0;
+    __syncwarp();
     bool ok = true;
-    for (int i = 0; i < d && ok; ++i)
-      for (int j = 0; j <= i; ++j) {
-        double s = cov[i * d + j];
-        for (int m = 0; m < j; ++m) s -= L[i * d + m] * L[j * d + m];
-        if (i == j) {
-          if (!(s > 0.0)) { ok = false; break; }
-          L[i * d + i] = sqrt(s);
-        } else
-          L[i * d + j] = s / L[j * d + j];
+    for (int j = 0; j < d; ++j) {
+      double sacc = 0.0;
+      if (i >= j && i < d) {
+        sacc = cov[i * d + j];
+        for (int m = 0; m < j; ++m) sacc -= sLc[i * d + m] * sLc[j * d + m];
       }
-    if (!ok) flags[0] = 1;
-    for (int a = 0; a < d * d; ++a) chol_out[a] = L[a];
+      const double piv = __shfl_sync(0xffffffffu, sacc, j);
+      if (!(piv > 0.0)) { ok = false; break; }              // uniform: every lane sees the same pivot
+      const double ljj = sqrt(piv);
+      if (i == j) sLc[j * d + j] = ljj;
+      else if (i > j && i < d) sLc[i * d + j] = sacc / ljj;
+      __syncwarp();
+    }
+    if (!ok && tid == 0) flags[0] = 1;
+    __syncwarp();
+    for (int a = tid; a < d * d; a += 32) chol_out[a] = sLc[a];
     if (mean_out)
-      for (int a = 0; a < d; ++a) mean_out[a] = mean[a];
+      for (int a = tid; a < d; a += 32) mean_out[a] = mean[a];
   }
 }
 

@@ -1,0 +1,59 @@
+"""Likelihood-kernel microbenchmark of BASELINE.json configs[4] ("config 5"): batches of N prior-uniform parameter
+vectors of the config-2 problem, relative binning with B bins x 3 detectors, through `nss_loglike_batch`.
+
+    python -m paper_2509_24949_b200.microbench
+
+Prints a markdown table: evaluations per second and the fraction of the fp64 DFMA issue peak (measured in the same
+process by `nss_fp64_peak`) for the automatic kernel choice and for both kernel forms (one thread per point; one
+sub-warp per point).  Parity of the same kernels against the oracle at B = 64, 256, 1024 is in
+tests/test_gpu_loglike.py; this script only times (inputs resident in HBM, L2 flushed between launches).
+"""
+from __future__ import annotations
+
+
+def work(B: int, n_det: int):
+    """fp64-pipe instructions one evaluation needs."""
+    E = B + 1
+    return 600 + E * 8 + E * n_det * 25
+
+
+def main():
+    import torch
+    from . import build, inputs, nss
+    build.build()
+    if not torch.cuda.is_available():
+        raise SystemExit("microbench.py needs a CUDA device: the product path has no CPU fallback")
+    peak = nss.nss_fp64_peak(300.0)                      # TFLOP/s; DFMA issue peak = peak / 2 instructions/s
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    print(f"fp64 DFMA peak measured in this process: {peak:.1f} TFLOP/s\n")
+    print("| B | N | kernel | ms | evals/s | fp64 instr./eval | fraction of the DFMA issue peak |")
+    print("|---|---|---|---|---|---|---|")
+    for B in (64, 128, 256, 1024):
+        w = inputs.make_data(inputs.config5(B), nss.nss_waveform)
+        g = nss.Nss(w)
+        Xall = torch.as_tensor(inputs.draw_prior(w, 1_000_000, 5), device="cuda")
+        for N in (1_000, 10_000, 100_000, 1_000_000):
+            X = Xall[:N].contiguous()
+            out = torch.empty(N, dtype=torch.float64, device="cuda")
+            for variant, name in ((0, "automatic"), (1, "thread per point"), (2, "sub-warp per point")):
+                g.set_loglike_variant(variant)
+                for _ in range(2):
+                    g.nss_loglike_batch(X, out)
+                ts = []
+                for _ in range(5):
+                    flush.fill_(1)
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record()
+                    g.nss_loglike_batch(X, out)
+                    b.record()
+                    b.synchronize()
+                    ts.append(a.elapsed_time(b))
+                ms = sorted(ts)[2]
+                rate = N / (ms * 1e-3)
+                ins = work(B, w.n_det)
+                print(f"| {B} | {N} | {name} | {ms:.4f} | {rate:.3e} | {ins} | {rate * ins / (peak * 1e12 / 2):.3f} |", flush=True)
+        g.close()
+
+
+if __name__ == "__main__":
+    main()

@@ -531,3 +531,31 @@ def test_two_and_four_detectors(nssmod, oracle, names):
             live, logL = p.init_live(200, 3)
             _trajectory_parity(g, p, live, logL, 100, 6, seed=3, it=0, w=w, max_excluded=0.06)
         g.close()
+
+
+def test_run_stops_at_max_iter_and_reports_a_small_result_array(nssmod, oracle, wl1):
+    """nss_run queues one iteration ahead of the host, so the exits other than convergence need their own check:
+    max_iter (NSS_ENOTCONV, results valid and equal to the oracle's truncated run, nothing of a further iteration
+    applied), max_iter = 0 (only the live points), and a result array that is too small (NSS_ECAP)."""
+    g, p = nssmod.Nss(wl1), oracle.Problem(wl1)
+    for mi in (3, 1, 0):
+        r = g.nss_run(100, 50, 12, 2, max_iter=mi, cap=100 + 50 * max(mi, 1))
+        o = p.run(100, 50, 12, 2, max_iter=mi, cap=100 + 50 * max(mi, 1))
+        assert r["rc"] == nssmod.NSS_ENOTCONV and o["rc"] == 1
+        assert r["n_iter"] == o["n_iter"] == mi and r["n_dead"] == o["n_dead"] == 100 + 50 * mi
+        assert np.allclose(r["dead_logL"], o["dead_logL"], rtol=1e-9, atol=1e-6)
+        assert r["logZ"] == pytest.approx(o["logZ"], abs=1e-6)
+        assert np.allclose(r["dead_logw"], o["dead_logw"], rtol=0, atol=1e-9)
+    import ctypes as C
+    res = nssmod.nss_result()
+    n = 100 + 50                                    # room for one iteration only; the run needs ~29
+    bufs = [np.empty((n, wl1.d)), np.empty(n), np.empty(n), np.empty(n)]
+    c_dp = C.POINTER(C.c_double)
+    res.dead_theta, res.dead_logL, res.dead_logL_birth, res.dead_logw = (b.ctypes.data_as(c_dp) for b in bufs)
+    res.cap = n
+    rc = nssmod.lib().nss_run(g._h, 100, 50, 12, 2, -3.0, 10000, C.byref(res), None)
+    assert rc == nssmod.NSS_ECAP
+    assert p.run(100, 50, 12, 2, cap=n)["rc"] == -3
+    r = g.nss_run(100, 50, 12, 2)                   # and the handle is fine afterwards
+    assert r["rc"] == 0 and r["n_iter"] > 5
+    g.close()

@@ -855,4 +855,32 @@ int orc_run(const orc_problem *p, int n, int k, int n_repeats, uint64_t seed, do
   return rc;
 }
 
-int orc_version(void) { return 1; }
+/* ---- NEXT-4 / reading R6: equal-weight posterior samples -----------------------------------
+ * PAPER.md:59-63 quotes, in brackets beside the Kish ESS, the number of "equal weight samples" and does not
+ * define them.  Reading R6: the weighted rows (posterior weight p_i ~ exp(logL_i + logw_i), O15) are compressed
+ * to unit weights by keeping row i with probability p_i / max_j p_j, independently: keep iff u_i < p_i / p_max,
+ * u_i = the [0,1) uniform of Philox counter (block 0, step i mod 2^32, chain i div 2^32, iteration 0xFFFFFFFD).
+ * The kept rows, in ascending row order, are an equally weighted sample of the posterior; their expected number
+ * is sum_i p_i / p_max.  Rows with logL + logw = -inf are never kept.  Returns the number kept (idx_out may be
+ * NULL; otherwise it receives the kept row indices, at most n of them). */
+#define ORC_ITER_EQUAL 0xFFFFFFFDu
+int64_t orc_resample_equal(const double *logL, const double *logw, int64_t n, uint64_t seed, int64_t *idx_out)
+{
+  double amax = -INFINITY;
+  for (int64_t i = 0; i < n; ++i) {
+    const double a = logL[i] + logw[i];
+    if (a > amax) amax = a;
+  }
+  if (amax == -INFINITY) return 0;
+  int64_t m = 0;
+  for (int64_t i = 0; i < n; ++i) {
+    const double a = logL[i] + logw[i];
+    if (!(a > -INFINITY)) continue;
+    const double p = exp(a - amax);
+    const double u = orc_uniform_a(seed, 0u, (uint32_t)(i & 0xFFFFFFFF), (uint32_t)(i >> 32), ORC_ITER_EQUAL);
+    if (u < p) { if (idx_out) idx_out[m] = i; ++m; }
+  }
+  return m;
+}
+
+int orc_version(void) { return 2; }

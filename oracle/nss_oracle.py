@@ -82,6 +82,8 @@ def lib():
         L.orc_run.restype = C.c_int
         L.orc_run.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_uint64, C.c_double, C.c_int,
                               C.c_int64, c_dp, c_dp, c_dp, c_dp, c_dp, C.c_int]
+        L.orc_resample_equal.restype = C.c_int64
+        L.orc_resample_equal.argtypes = [c_dp, c_dp, C.c_int64, C.c_uint64, C.POINTER(C.c_int64)]
         _lib = L
     return _lib
 
@@ -156,6 +158,14 @@ def evidence_update(dead_logL, n, logX, logZ):
     x, z = C.c_double(logX), C.c_double(logZ)
     lib().orc_evidence_update(_dp(dl), n, dl.size, C.byref(x), C.byref(z), _dp(lw))
     return x.value, z.value, lw
+
+
+def resample_equal(logL, logw, seed) -> np.ndarray:
+    """Reading R6: row indices of the equal-weight posterior sample (ascending)."""
+    l, w = _f64(logL), _f64(logw)
+    idx = np.empty(l.size, dtype=np.int64)
+    m = lib().orc_resample_equal(_dp(l), _dp(w), l.size, int(seed), idx.ctypes.data_as(C.POINTER(C.c_int64)))
+    return idx[:m].copy()
 
 
 def tune(live):

@@ -75,6 +75,31 @@ def test_tune_matches_oracle(nssmod, oracle):
         g.close()
 
 
+def test_tune_near_singular_covariance_reading_r5(nssmod, oracle):
+    """Reading R5: ECHOL if and only if a pivot as computed is <= 0.  A nearly singular live-point covariance
+    (chi_1 ~ chi_2 to 1e-5 of their spread: pivot ~1e-10 of the variance) factors on both sides; the well-conditioned
+    columns agree to 1e-8, the tiny pivot to 1e-4 (it is a difference of nearly equal sums, taken in a different but
+    fixed order), and the GPU factor reproduces the covariance.  With exactly collinear columns the pivot is rounding
+    noise of either sign: each side may report ECHOL or return a factor, and a returned factor reproduces the covariance."""
+    from test_oracle_sampler import near_singular_population
+    g = nssmod.Nss(inputs.gaussian_workload(11))
+    x = near_singular_population(np.random.default_rng(5))
+    rc, mean, chol = g.nss_tune(x)
+    orc, omean, ocov, ochol = oracle.tune(x)
+    assert rc == 0 and orc == 0
+    L = chol.cpu().numpy()
+    assert np.allclose(L[:, :3], ochol[:, :3], rtol=1e-8, atol=1e-300)
+    assert np.allclose(L[:, 4:], ochol[:, 4:], rtol=1e-4, atol=1e-12 * np.abs(ochol).max())
+    assert L[3, 3] == pytest.approx(ochol[3, 3], rel=1e-4)
+    assert np.allclose(L @ L.T, ocov, rtol=1e-9, atol=1e-22)
+    x[:, 3] = x[:, 2]
+    rc, mean, chol = g.nss_tune(x)
+    L = chol.cpu().numpy()
+    cov = np.cov(x.T)
+    assert rc == nssmod.NSS_ECHOL or np.allclose(L @ L.T, cov, rtol=1e-9, atol=1e-16 * cov[2, 2])
+    g.close()
+
+
 @pytest.mark.parametrize("n,k", [(1000, 500), (5000, 2500), (100, 1), (3000, 2999)])
 def test_evidence_update_matches_oracle(ggauss, oracle, n, k):
     rng = np.random.default_rng(2)
@@ -112,6 +137,8 @@ def _trajectory_parity(g, p, live, logL, k, n_repeats, seed, it, logLstar=math.n
     gtr, otr = r["trace"].cpu().numpy(), o["trace"]
     margin = np.minimum(r["margin"].cpu().numpy(), o["margin"])
     safe = margin > 1e-6                          # A20: chains whose bracket tests all clear L* by > 1e-6
+    print(f"[trajectory parity] n={live.shape[0]} k={k} repeats={n_repeats} it={it}: {(~safe).sum()} of {k} chains excluded "
+          f"by the 1e-6 margin rule ({100 * (~safe).mean():.2f} %, limit {100 * max_excluded:.0f} %)")
     assert safe.mean() >= 1 - max_excluded, f"{(~safe).sum()} of {k} chains excluded"
     assert np.array_equal(gtr[safe], otr[safe])                       # identical decisions
     didx = o["dead_idx"]
@@ -189,6 +216,21 @@ def test_replace_step_full_grid_kind(nssmod, oracle):
     g.close()
 
 
+def test_replace_step_full_grid_at_the_bench_launch_shape(nssmod, oracle):
+    """BASELINE configs[3] (full frequency grid, 4017 bins x 3 detectors) at n_live 1000 / n_delete 500: K3's
+    NSS_KIND_FULL instantiation in its real launch shape (500 one-chain CTAs), 11 slice repeats instead of 55 so that
+    the oracle's 12 051-term sums stay affordable; every chain against the oracle's trajectory, from the prior-wide
+    population and from a compressed one."""
+    w = inputs.make_data(inputs.config4(), oracle.waveform)
+    g, p = nssmod.Nss(w), oracle.Problem(w)
+    live, logL = p.init_live(1000, 6)
+    r, o, safe = _trajectory_parity(g, p, live, logL, 500, 11, seed=6, it=0, w=w, max_excluded=0.05)
+    live, logL = o["live"], o["logL"]
+    o = p.replace_step(live, logL, 500, 2, 6, 1)
+    _trajectory_parity(g, p, o["live"], o["logL"], 500, 3, seed=6, it=2, w=w, max_excluded=0.05)
+    g.close()
+
+
 def test_replace_step_degenerate_population_reports_cholesky(nssmod, oracle):
     w = inputs.gaussian_workload(3)
     g = nssmod.Nss(w)
@@ -233,30 +275,183 @@ def test_run_gaussian_matches_oracle_and_analytic(nssmod, oracle, d, n, k, seed)
     g.close()
 
 
+def _replays(r, o):
+    """True when the GPU run made the oracle's decisions: same dead rows (logL within the logL tolerance)."""
+    return r["n_dead"] == o["n_dead"] and bool(np.allclose(r["dead_logL"], o["dead_logL"], rtol=1e-9, atol=1e-6))
+
+
+def _assert_replay(r, o, w):
+    """What a replayed run must satisfy beyond _replays: same iterations, same sequential evaluation count, same rows
+    (positions within 1e-9 of the prior width, A20)."""
+    assert r["n_iter"] == o["n_iter"] and r["n_evals"] == o["n_evals"]
+    assert np.allclose(r["dead_logw"], o["dead_logw"], rtol=0, atol=1e-9)
+    assert r["logZ"] == pytest.approx(o["logZ"], abs=1e-6)
+    assert np.allclose(r["dead_logL_birth"], o["dead_logL_birth"], rtol=1e-9, atol=1e-6)
+    assert np.all(np.abs(r["dead_theta"] - o["dead_theta"]) <= 1e-9 * (w.hi - w.lo))
+
+
+def _weights(res):
+    a = res["dead_logL"] + res["dead_logw"]
+    pw = np.exp(a - a.max())
+    return pw / pw.sum()
+
+
 def test_run_config1_matches_oracle(nssmod, oracle, wl1):
-    """End-to-end: logZ within 3 sigma_NS, posterior means within 0.1 sigma of the posterior width,
-    over the seed ensemble of config 1 (trajectories are identical until a near-threshold test flips)."""
+    """End to end on config 1 over its seed ensemble: logZ within 3 sigma_NS and posterior means within 0.1 sigma of the
+    oracle's posterior width, asserted for every seed whether or not the run replayed (north_star); and every seed is
+    expected to replay the oracle decision for decision (|logL_GPU - logL_oracle| ~ 1e-11 against ~1e5 bracket tests)."""
     g, p = nssmod.Nss(wl1), oracle.Problem(wl1)
-    dz, exact = [], 0
+    exact = 0
     for seed in (1, 2, 3, 4):
         r = g.nss_run(100, 50, 12, seed)
         o = p.run(100, 50, 12, seed)
         assert r["rc"] == 0 and o["rc"] == 0
-        sig = math.hypot(r["logZ_err"], o["logZ_err"])
-        assert abs(r["logZ"] - o["logZ"]) < 3 * sig
-        dz.append(r["logZ"] - o["logZ"])
-        if r["n_dead"] == o["n_dead"] and np.allclose(r["dead_logL"], o["dead_logL"], rtol=1e-9, atol=1e-6):
+        assert abs(r["logZ"] - o["logZ"]) < 3 * math.hypot(r["logZ_err"], o["logZ_err"])
+        pg, po = _weights(r), _weights(o)
+        mg, mo = pg @ r["dead_theta"], po @ o["dead_theta"]
+        so = np.sqrt(po @ (o["dead_theta"] - mo) ** 2)
+        assert np.all(np.abs(mg - mo) < 0.1 * so)
+        if _replays(r, o):
             exact += 1
-            assert np.allclose(r["dead_logw"], o["dead_logw"], rtol=0, atol=1e-9)
-            assert r["logZ"] == pytest.approx(o["logZ"], abs=1e-6)
-            assert r["n_evals"] == o["n_evals"]
-        pw_g = np.exp(r["dead_logL"] + r["dead_logw"] - r["logZ"])
-        pw_o = np.exp(o["dead_logL"] + o["dead_logw"] - o["logZ"])
-        mg, mo = pw_g @ r["dead_theta"], pw_o @ o["dead_theta"]
-        so = np.sqrt(pw_o @ (o["dead_theta"] - mo) ** 2)
-        if exact:
-            assert np.all(np.abs(mg - mo) < 0.1 * so)
-    assert exact >= 2, "at least half the seeds should replay bit-for-bit identical decision sequences"
+            _assert_replay(r, o, wl1)
+    print(f"[config 1] {exact} of 4 seeds replayed the oracle's run decision for decision")
+    assert exact >= 3
+    g.close()
+
+
+def test_run_seed_ensemble_replays_the_oracle(nssmod, oracle, wl1):
+    """The seed-ensemble check behind DESIGN.md §5's replay claim: 16 seeds of config 1 and 8 seeds of a 5-dimensional
+    Gaussian, each a whole run to the stop rule on both sides.  Every run must agree in logZ within 3 sigma_NS, and at
+    least 7 in 8 must be the oracle's run decision for decision (a flip needs a bracket test within ~1e-11 of L*)."""
+    g, p = nssmod.Nss(wl1), oracle.Problem(wl1)
+    exact, worst = 0, 0.0
+    for seed in range(100, 116):
+        r, o = g.nss_run(100, 50, 12, seed), p.run(100, 50, 12, seed)
+        worst = max(worst, abs(r["logZ"] - o["logZ"]) / math.hypot(r["logZ_err"], o["logZ_err"]))
+        if _replays(r, o):
+            exact += 1
+            _assert_replay(r, o, wl1)
+    g.close()
+    print(f"[ensemble] config 1: {exact} of 16 seeds replayed; worst |dlogZ| / sigma = {worst:.3f}")
+    assert worst < 3.0 and exact >= 14
+    w = inputs.gaussian_workload(5, sigma=0.07)
+    g, p = nssmod.Nss(w), oracle.Problem(w)
+    exact, worst = 0, 0.0
+    for seed in range(200, 208):
+        r, o = g.nss_run(500, 250, 15, seed), p.run(500, 250, 15, seed)
+        worst = max(worst, abs(r["logZ"] - o["logZ"]) / math.hypot(r["logZ_err"], o["logZ_err"]))
+        if _replays(r, o):
+            exact += 1
+            _assert_replay(r, o, w)
+    g.close()
+    print(f"[ensemble] 5-d Gaussian: {exact} of 8 seeds replayed; worst |dlogZ| / sigma = {worst:.3f}")
+    assert worst < 3.0 and exact >= 7
+
+
+def test_run_statistical_parity_on_independent_seeds(nssmod, oracle):
+    """north_star's statistical criteria on runs that do NOT share a trajectory: the GPU run uses seed 11, the oracle
+    seeds 12 and 13 (different Philox streams from the first draw on).  4-d Gaussian, n_live 4000 so that the Monte-Carlo
+    error of a posterior mean (sigma / sqrt(ESS), ESS ~ 1e4) is ~ 0.01 sigma and 0.1 sigma is a real bar: logZ within
+    3 sigma_NS of each other and of the analytic value, means within 0.1 sigma, widths within 5 %."""
+    w = inputs.gaussian_workload(4, sigma=0.05)
+    g, p = nssmod.Nss(w), oracle.Problem(w)
+    r = g.nss_run(4000, 2000, 20, 11)
+    truth = _analytic_logz(4, 0.05, 1.0)
+    assert abs(r["logZ"] - truth) < 3 * r["logZ_err"]
+    pg = _weights(r)
+    mg = pg @ r["dead_theta"]
+    sg = np.sqrt(pg @ (r["dead_theta"] - mg) ** 2)
+    for seed in (12, 13):
+        o = p.run(4000, 2000, 20, seed)
+        assert not _replays(r, o)
+        assert abs(r["logZ"] - o["logZ"]) < 3 * math.hypot(r["logZ_err"], o["logZ_err"])
+        po = _weights(o)
+        mo = po @ o["dead_theta"]
+        so = np.sqrt(po @ (o["dead_theta"] - mo) ** 2)
+        assert np.all(np.abs(mg - mo) < 0.1 * so)
+        assert np.all(np.abs(sg / so - 1) < 0.05)
+    g.close()
+
+
+def _config2_summary(res):
+    """Posterior means / widths of the quantities SURVEY.md §8(d) says to compare on config 2: Mc, q, the spin
+    combination beta that enters the phase (chi_1, chi_2 are individually unconstrained), d_L, t_c, iota, ra, dec as
+    plain means; phi_c (period 2 pi) and psi (period pi) as circular means.  Returns (values, widths, is_circular, period)."""
+    th, pw = res["dead_theta"], _weights(res)
+    q = th[:, 1]
+    eta = q / (1 + q) ** 2
+    m1, m2 = 1 / (1 + q), q / (1 + q)
+    beta = (113 / 12 * m1 ** 2 + 25 / 4 * eta) * th[:, 2] + (113 / 12 * m2 ** 2 + 25 / 4 * eta) * th[:, 3]
+    cols = [th[:, 0], q, beta, th[:, 4], th[:, 5], th[:, 7], th[:, 9], th[:, 10]]
+    mean = np.array([pw @ c for c in cols])
+    sd = np.array([math.sqrt(pw @ (c - m) ** 2) for c, m in zip(cols, mean)])
+    circ = []
+    for col, period in ((th[:, 6], 2 * math.pi), (th[:, 8], math.pi)):
+        z = pw @ np.exp(2j * math.pi * col / period)
+        circ.append((np.angle(z) * period / (2 * math.pi), math.sqrt(max(-2 * math.log(abs(z)), 0.0)) * period / (2 * math.pi), period))
+    return mean, sd, circ
+
+
+@pytest.mark.parametrize("seed", [1, 2])
+def test_run_config2_matches_oracle(nssmod, oracle, wl2, seed):
+    """north_star's Target: a whole NSS run on the 11-parameter, 3-detector heterodyned workload (BASELINE configs[1]:
+    n_live 1000, n_delete 500, 55 repeats) to the stop rule on both sides.  Unconditionally: |dlogZ| < 3 hypot(sigma_GPU,
+    sigma_oracle); posterior means of Mc, q, beta, d_L, t_c, iota, ra, dec within 0.1 of the oracle's posterior width;
+    phi_c and psi compared as wrapped angles.  And the run is expected to replay: same iterations, same sequential
+    evaluation count, same dead rows."""
+    g, p = nssmod.Nss(wl2), oracle.Problem(wl2)
+    import time
+    t0 = time.perf_counter()
+    r = g.nss_run(1000, 500, 55, seed)
+    t1 = time.perf_counter()
+    o = p.run(1000, 500, 55, seed)
+    t2 = time.perf_counter()
+    print(f"[config 2, seed {seed}] GPU {t1 - t0:.3f} s, oracle {t2 - t1:.1f} s on {oracle.n_cores()} cores; n_iter {r['n_iter']} / {o['n_iter']}, "
+          f"n_evals {r['n_evals']} / {o['n_evals']}, logZ {r['logZ']:.4f} +- {r['logZ_err']:.3f} / {o['logZ']:.4f} +- {o['logZ_err']:.3f}")
+    assert r["rc"] == 0 and o["rc"] == 0
+    assert abs(r["logZ"] - o["logZ"]) < 3 * math.hypot(r["logZ_err"], o["logZ_err"])
+    assert r["H"] == pytest.approx(o["H"], abs=0.5)
+    mg, sg, cg = _config2_summary(r)
+    mo, so, co = _config2_summary(o)
+    assert np.all(np.abs(mg - mo) < 0.1 * so), (mg, mo, so)
+    for (ag, wg, per), (ao, wo, _) in zip(cg, co):
+        dist = abs((ag - ao + per / 2) % per - per / 2)
+        assert dist < 0.1 * wo
+    replay = _replays(r, o)
+    print(f"[config 2, seed {seed}] replayed decision for decision: {replay}")
+    assert replay, "config 2 is expected to replay (a flip needs a bracket test within ~1e-10 of L*)"
+    _assert_replay(r, o, wl2)
+    g.close()
+
+
+def test_run_config3_bounded_matches_oracle(nssmod, oracle, wl2):
+    """BASELINE configs[2] (n_live 5000, n_delete 2500, 55 repeats: 2500 concurrent chains) through nss_run for two NS
+    iterations (NSS_ENOTCONV: results valid) against the oracle's truncated run: same rows, weights and evidence."""
+    g, p = nssmod.Nss(wl2), oracle.Problem(wl2)
+    cap = 5000 + 2 * 2500
+    r = g.nss_run(5000, 2500, 55, 3, max_iter=2, cap=cap)
+    o = p.run(5000, 2500, 55, 3, max_iter=2, cap=cap)
+    assert r["rc"] == nssmod.NSS_ENOTCONV and o["rc"] == 1
+    assert r["n_iter"] == o["n_iter"] == 2 and r["n_dead"] == o["n_dead"] == cap
+    assert abs(r["logZ"] - o["logZ"]) < 3 * math.hypot(r["logZ_err"], o["logZ_err"]) + 1e-6
+    assert _replays(r, o)
+    _assert_replay(r, o, wl2)
+    g.close()
+
+
+def test_run_config4_bounded_matches_oracle(nssmod, oracle):
+    """BASELINE configs[3] (full-grid likelihood, n_live 1000, n_delete 500) through nss_run: two NS iterations with 11
+    slice repeats against the oracle's truncated run."""
+    w = inputs.make_data(inputs.config4(), oracle.waveform)
+    g, p = nssmod.Nss(w), oracle.Problem(w)
+    cap = 1000 + 2 * 500
+    r = g.nss_run(1000, 500, 11, 4, max_iter=2, cap=cap)
+    o = p.run(1000, 500, 11, 4, max_iter=2, cap=cap)
+    assert r["rc"] == nssmod.NSS_ENOTCONV and o["rc"] == 1
+    assert r["n_iter"] == o["n_iter"] == 2 and r["n_dead"] == o["n_dead"] == cap
+    assert abs(r["logZ"] - o["logZ"]) < 3 * math.hypot(r["logZ_err"], o["logZ_err"]) + 1e-6
+    assert _replays(r, o)
+    _assert_replay(r, o, w)
     g.close()
 
 
@@ -272,10 +467,10 @@ def test_run_delete_fraction_sweep_matches_oracle(nssmod, oracle, wl1, n_delete)
     assert abs(r["logZ"] - o["logZ"]) < 3 * math.hypot(r["logZ_err"], o["logZ_err"])
     assert np.all(np.diff(r["dead_logL"][: r["n_dead"] - 100]) >= 0)           # dead points leave in ascending logL
     assert np.exp(r["dead_logw"]).sum() == pytest.approx(1.0, abs=1e-9)        # dead + final live weights exhaust the prior
-    if r["n_dead"] == o["n_dead"] and np.allclose(r["dead_logL"], o["dead_logL"], rtol=1e-9, atol=1e-6):
-        assert r["n_iter"] == o["n_iter"] and r["n_evals"] == o["n_evals"]
-        assert np.allclose(r["dead_logw"], o["dead_logw"], rtol=0, atol=1e-9)
-        assert np.array_equal(r["dead_theta"], o["dead_theta"]) or np.allclose(r["dead_theta"], o["dead_theta"], rtol=1e-12, atol=1e-12)
+    replay = _replays(r, o)
+    print(f"[delete-fraction sweep] n_delete={n_delete}: replayed {replay}")
+    assert replay, "every point of the sweep replayed the oracle on B200 when this test was written"
+    _assert_replay(r, o, wl1)
     g.close()
 
 
@@ -436,9 +631,10 @@ def test_next2_periodic_run_matches_oracle_and_analytic(nssmod, oracle):
     assert r["rc"] == 0 and o["rc"] == 0
     assert abs(r["logZ"] - truth) < 3 * r["logZ_err"]
     assert abs(r["logZ"] - o["logZ"]) < 3 * math.hypot(r["logZ_err"], o["logZ_err"])
-    if r["n_dead"] == o["n_dead"] and np.allclose(r["dead_logL"], o["dead_logL"], rtol=1e-9, atol=1e-9):
-        assert r["n_evals"] == o["n_evals"]
-        assert np.allclose(r["dead_theta"], o["dead_theta"], rtol=0, atol=1e-12)
+    replay = _replays(r, o)
+    print(f"[periodic run] replayed {replay}")
+    assert replay, "the wrapped Gaussian run replayed the oracle on B200 when this test was written"
+    _assert_replay(r, o, w)
     g.close()
 
 

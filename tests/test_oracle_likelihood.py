@@ -5,6 +5,7 @@ case or an exact identity that a dropped term / wrong sign / transposed operand 
 """
 import copy
 import math
+import os
 
 import numpy as np
 import pytest
@@ -54,7 +55,73 @@ def test_p1_full_phase_tends_to_newtonian_at_low_v(oracle):
     assert abs(r[1]) < 1e-3
 
 
-# ---- P2 (sanity only; the PN coefficients themselves are "parity unpinned") -----------------------
+# ---- P2: the higher PN coefficients, recovered numerically and compared with SURVEY.md O3's literals ---------------
+def _golden_literals():
+    """tests/golden/taylorf2_o3_literals.txt (typed by hand from SURVEY.md:346-355) -> {name: mpmath value}."""
+    import mpmath as mp
+    sym = {"pi": mp.pi, "pi^2": mp.pi ** 2, "gammaE": mp.mpf("0.5772156649015329")}
+    out = {}
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "taylorf2_o3_literals.txt")
+    for line in open(path):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        name, expr = (t.strip() for t in line.split("|"))
+        val = mp.mpf(0)
+        for term in expr.split(" + "):
+            parts = [t.strip() for t in term.split("*")]
+            p, q = parts[0].split("/")
+            t = mp.mpf(int(p)) / int(q)
+            for s in parts[1:]:
+                t *= sym[s]
+            val += t
+        out[name] = val
+    return out
+
+
+def test_p2_pn_literals_recovered_from_the_phase(oracle):
+    """S(v) = (128 eta v^5 / 3)(Psi - 2 pi f t_c + phi_c + pi/4) = sum_k phi_k v^k is LINEAR in every literal of O3 once
+    the basis (power of v, ln v, power of eta, spin combination) is fixed.  Evaluate orc_phase on a grid of (v, q, spins),
+    solve the least-squares problem for the 22 coefficients in 60-digit arithmetic (inputs are the oracle's doubles), and
+    compare each with the rational literal stored under tests/golden/ (typed from SURVEY.md O3, not from the oracle).
+    A dropped term, a wrong sign or a mistyped digit in any phi_k of oracle/nss_oracle.c changes a recovered
+    coefficient by far more than the recovery error (measured: < 3e-9 relative; bar 1e-8)."""
+    import mpmath as mp
+    mp.mp.dps = 60
+    G = _golden_literals()
+    rows, rhs = [], []
+    Mc = 30.0
+    for q in (1.0, 0.8, 0.6, 0.45, 0.3, 0.2, 0.12):
+        for c1, c2 in ((0.0, 0.0), (0.7, -0.4), (-0.3, 0.9)):
+            for vt in np.geomspace(0.15, 3.0, 24):          # the formula is just a formula: v need not be physical
+                f = float(vt ** 3 / (math.pi * Mc * (q / (1 + q) ** 2) ** -0.6 * GMSUN))
+                psi = oracle.phase(f, _canon(Mc=Mc, q=q, chi1z=c1, chi2z=c2, tc=0.0, phic=0.0))
+                qm = mp.mpf(q)
+                eta = qm / (1 + qm) ** 2
+                v = mp.cbrt(mp.pi * mp.mpf(Mc) * eta ** (mp.mpf(-3) / 5) * mp.mpf(GMSUN) * mp.mpf(f))
+                lv = mp.log(v)
+                m1, m2 = 1 / (1 + qm), qm / (1 + qm)
+                b_m, b_e = m1 ** 2 * mp.mpf(c1) + m2 ** 2 * mp.mpf(c2), eta * (mp.mpf(c1) + mp.mpf(c2))
+                rows.append([1, v, v ** 2, v ** 2 * eta, v ** 3, v ** 3 * b_m, v ** 3 * b_e, v ** 4, v ** 4 * eta, v ** 4 * eta ** 2,
+                             v ** 5, v ** 5 * eta, v ** 5 * lv, v ** 5 * lv * eta, v ** 6, v ** 6 * eta, v ** 6 * eta ** 2,
+                             v ** 6 * eta ** 3, v ** 6 * lv, v ** 7, v ** 7 * eta, v ** 7 * eta ** 2])
+                rhs.append((128 * eta * v ** 5 / 3) * (mp.mpf(psi) + mp.pi / 4))
+    A, b = mp.matrix(rows), mp.matrix(rhs)
+    x = mp.lu_solve(A.T * A, A.T * b)
+    # phi_5 = P5 (1 + 3 ln(v / v_lso)) = P5 (1 + (3/2) ln(1/v_lso^2)) + 3 P5 ln v;   -(6848/21) ln(4v) = phi6_ln (ln 4 + ln v)
+    k5 = 1 + G["phi5_ln"] / 2 * mp.log(G["vlso_inv_square"])
+    expect = [G["phi0"], G["phi1"], G["phi2_eta0"], G["phi2_eta1"],
+              G["phi3_const"], G["phi3_beta"] * G["beta_mass2"], G["phi3_beta"] * G["beta_eta"],
+              G["phi4_eta0"], G["phi4_eta1"], G["phi4_eta2"],
+              G["phi5_eta0"] * k5, G["phi5_eta1"] * k5, G["phi5_ln"] * G["phi5_eta0"], G["phi5_ln"] * G["phi5_eta1"],
+              G["phi6_eta0"] + G["phi6_ln"] * mp.log(G["phi6_ln_arg"]), G["phi6_eta1"], G["phi6_eta2"], G["phi6_eta3"],
+              G["phi6_ln"], G["phi7_eta0"], G["phi7_eta1"], G["phi7_eta2"]]
+    for i, e in enumerate(expect):
+        scale = abs(e) if e != 0 else mp.mpf(1)
+        assert abs(x[i] - e) / scale < 1e-8, f"coefficient {i}: recovered {mp.nstr(x[i], 15)}, SURVEY O3 says {mp.nstr(e, 15)}"
+
+
+# ---- P2 sanity identities -------------------------------------------------------------------------------------------
 def test_p2_spin_orbit_enters_only_through_beta(oracle):
     # phi_3 shifts by exactly 4*beta: Psi(chi) - Psi(0) = 3/(128 eta v^5) * 4 beta v^3
     th0, th1 = _canon(chi1z=0.0, chi2z=0.0), _canon(chi1z=0.3, chi2z=-0.2)

@@ -115,6 +115,36 @@ def test_p12_tune_vs_numpy(oracle):
     assert oracle.tune(x2)[0] != 0
 
 
+def near_singular_population(rng, n=1000, eps=1e-5):
+    """The realistic failure late in a run (chi_1 / chi_2 enter the phase only through beta): column 3 is column 2 plus
+    a perturbation eps times smaller, so the last-but-one pivot is ~eps^2 of the column variance."""
+    scales = np.array([1.0, 0.1, 0.5, 0.5, 600.0, 1e-3, 1.5, 0.3, 0.6, 0.01, 0.014])
+    x = rng.normal(size=(n, 11)) * scales + 10 * scales
+    x[:, 3] = x[:, 2] + eps * scales[3] * rng.normal(size=n)
+    return x
+
+
+def test_p12_tune_near_singular_covariance_reading_r5(oracle):
+    """DESIGN.md reading R5: the Cholesky fails (ECHOL) if and only if a pivot, computed as written (O12.3), is <= 0 — no
+    relative epsilon, no jitter (A11).  A nearly singular covariance (pivot ~1e-10 of the variance) must therefore
+    factor, and the factor must reproduce the covariance (the only property the slice directions need: v = w L z/|z|
+    has covariance proportional to L L^T); NumPy's factor of the same matrix agrees on the well-conditioned columns.
+    Exactly collinear columns leave a pivot of the order of the rounding error whose sign is luck: either outcome is
+    legal, but a returned factor must still reproduce the covariance."""
+    rng = np.random.default_rng(5)
+    x = near_singular_population(rng)
+    rc, mean, cov, chol = oracle.tune(x)
+    assert rc == 0
+    assert np.allclose(cov, np.cov(x.T), rtol=1e-9, atol=1e-22)
+    assert np.allclose(chol @ chol.T, cov, rtol=1e-11, atol=1e-22)
+    ref = np.linalg.cholesky(cov)
+    assert np.allclose(chol[:, :3], ref[:, :3], rtol=1e-9, atol=1e-18)
+    assert chol[3, 3] == pytest.approx(ref[3, 3], rel=1e-4) and chol[3, 3] < 1e-4 * chol[2, 2]
+    x[:, 3] = x[:, 2]
+    rc, mean, cov, chol = oracle.tune(x)
+    assert rc != 0 or np.allclose(chol @ chol.T, cov, rtol=1e-9, atol=1e-16 * cov[2, 2])
+
+
 def test_p12_p14_evidence_update(oracle):
     n, k = 1000, 500
     rng = np.random.default_rng(2)
@@ -323,3 +353,82 @@ def test_next2_evidence_does_not_depend_on_the_topology(oracle, flags):
     a = (-1 - w.gauss_mu[0]) / 0.05
     tm = w.gauss_mu[0] + 0.05 * scipy.stats.norm.pdf(a) / (1 - scipy.stats.norm.cdf(a))
     assert abs(mean0 - tm) < 0.01
+
+
+def test_next2_bracket_longer_than_one_period_keeps_the_slice_uniform(oracle):
+    """A wrapped coordinate never fails the box test, so with a loose constraint a bracket can grow past one period
+    (up to 32 widths per side) and wrapped proposals then cover parts of the circle more than once.  The slice is the
+    lifted periodic set on the line and stepping-out / shrinkage on it is ordinary slice sampling, so the wrapped draw
+    stays uniform on the admissible arc.  1-D circle [-1, 1), threshold admitting the arc |x| < 0.8 (80 % of the circle):
+    an end that steps across the seam lands inside the arc again and the bracket keeps growing."""
+    w = inputs.gaussian_workload(1, sigma=1.0)
+    p = oracle.Problem(w)
+    p.set_periodic([1])
+    c = 0.8
+    Lstar = -0.5 * c * c
+    rng = np.random.default_rng(8)
+    n, k = 1200, 600
+    live = rng.uniform(-c, c, size=(n, 1))
+    logL = p.loglike_batch(live)
+    r = p.replace_step(live, logL, k, 30, seed=4, iteration=0, logLstar=Lstar, want_trace=True)
+    assert r["rc"] == 0
+    new = r["live"][r["dead_idx"]][:, 0]
+    assert np.all(np.abs(new) < c)
+    assert scipy.stats.kstest((new + c) / (2 * c), "uniform").pvalue > 1e-3
+    # bracket length in units of the coordinate: (1 + expansions) * |v|, |v| = 2 * s.d. of the live points (A14)
+    width = (1 + r["trace"][:, :, 0] + r["trace"][:, :, 1]) * 2.0 * np.std(live[:, 0], ddof=1)
+    assert (width > 2.0).mean() > 0.2, "the case must exercise brackets longer than the period"
+
+
+# ---- NEXT-4 / reading R6: equal-weight posterior samples ---------------------------------------------------------------
+def test_r6_equal_weight_resampling_closed_forms(oracle):
+    """orc_resample_equal keeps row i iff u_i < p_i / p_max.  What the mathematics fixes: equal weights keep every row;
+    a row with the maximum weight is always kept and rows 800 nats below never; weights of exactly half the maximum keep
+    about half (binomial); the expected number kept is sum p / p_max; the kept rows are an equally weighted sample of
+    the weighted distribution (their plain mean matches the weighted mean); rows of zero weight are never kept; and the
+    draw is a function of (seed, row) only."""
+    n = 20000
+    z = np.zeros(n)
+    assert np.array_equal(oracle.resample_equal(z, np.full(n, -7.0), 1), np.arange(n))
+    lw = np.full(n, -800.0); lw[[5, 77]] = 0.0
+    assert np.array_equal(oracle.resample_equal(z, lw, 2), [5, 77])
+    lw = np.full(n, math.log(0.5)); lw[0] = 0.0
+    m = oracle.resample_equal(z, lw, 3).size
+    assert abs(m - 1 - (n - 1) / 2) < 5 * math.sqrt(n / 4)
+    rng = np.random.default_rng(0)
+    x = rng.normal(size=n)
+    logL = -0.5 * ((x - 0.7) / 0.3) ** 2            # weight ~ N(0.7, 0.3) density ratio over the N(0,1) proposal
+    logw = rng.normal(size=n) * 0.0
+    logw[::10] = -np.inf
+    counts = [oracle.resample_equal(logL, logw, s).size for s in range(40)]
+    pw = np.exp(logL + logw - (logL + logw).max())
+    assert abs(np.mean(counts) - pw.sum()) < 5 * math.sqrt(pw.sum() / 40)
+    idx = oracle.resample_equal(logL, logw, 9)
+    assert np.all(np.diff(idx) > 0) and not np.any(np.isin(idx, np.arange(0, n, 10)))
+    wmean = (pw * x).sum() / pw.sum()
+    wsd = math.sqrt((pw * (x - wmean) ** 2).sum() / pw.sum())
+    assert abs(x[idx].mean() - wmean) < 5 * wsd / math.sqrt(idx.size)
+    assert abs(x[idx].std() / wsd - 1) < 0.1
+    assert np.array_equal(idx, oracle.resample_equal(logL, logw, 9))
+    assert not np.array_equal(idx, oracle.resample_equal(logL, logw, 10))
+    # u_i is the documented Philox counter: (block 0, step i, chain 0, iteration 0xFFFFFFFD)
+    u = np.array([oracle.uniform_a(9, 0, i, 0, 0xFFFFFFFD) for i in range(200)])
+    assert np.array_equal(np.flatnonzero(u < pw[:200]), idx[idx < 200])
+    assert oracle.resample_equal(z[:3], np.full(3, -np.inf), 1).size == 0
+
+
+# ---- sanitizers (SURVEY.md §5) -------------------------------------------------------------------------------------------
+def test_oracle_is_clean_under_address_and_undefined_sanitizers(tmp_path):
+    """The oracle compiled with -fsanitize=address,undefined (leak check included) walks every entry point on tiny
+    problems of all three likelihood kinds (oracle/sanitize_main.c): any out-of-bounds access, leak or undefined
+    arithmetic aborts."""
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    exe = str(tmp_path / "orc_sanitized")
+    cmd = ["gcc", "-std=c99", "-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=all", "-ffp-contract=off",
+           "-fopenmp", os.path.join(root, "oracle", "nss_oracle.c"), os.path.join(root, "oracle", "sanitize_main.c"),
+           "-o", exe, "-lm"]
+    subprocess.run(cmd, check=True)
+    r = subprocess.run([exe], capture_output=True, text=True, timeout=300,
+                       env=dict(os.environ, ASAN_OPTIONS="detect_leaks=1:abort_on_error=0", OMP_NUM_THREADS="2"))
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert "sanitize_main: ok" in r.stdout and "runtime error" not in r.stderr and "AddressSanitizer" not in r.stderr

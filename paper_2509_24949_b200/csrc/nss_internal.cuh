@@ -45,6 +45,13 @@ struct NssCtl {
   unsigned long long nevals;
   unsigned long long nrounds, nexec;   // K3 diagnostics: rounds run by all chains, candidates evaluated (incl. speculative)
   int32_t flags[4];            // [0] Cholesky error, [1] threshold violation, [2] stop rule reached
+  // work distribution inside an iteration (device only)
+  uint32_t front_done;         // blocks of k4_front that have finished (the last one publishes the flags)
+  uint32_t rank_done;          // ranking blocks of k4_front that have finished (the last one does the selection tail)
+  int32_t sel_bad;             // a survivor below a supplied threshold (selection tail -> flags[1])
+  uint32_t tune_cnt[2];        // counters of the tuning blocks of k4_front: column sums published, products published
+  uint32_t chains_done;        // chains finished (the CTA that finishes the last one runs the live-evidence epilogue)
+  int32_t chol_now;            // Cholesky status of the tuning block of the iteration being set up
 };
 
 struct nss_handle {
@@ -64,8 +71,8 @@ struct nss_handle {
   size_t rec_bytes, soa_bytes[3];
   // sampler scratch (grown on demand)
   int32_t scratch_n;
-  int32_t *d_surv_idx, *d_dead_idx, *d_rank, *d_flags;   // flags: [0] chol error, [1] threshold violation, [2] done
-  double *d_mean, *d_chol, *d_state;                      // state: logX, logZ, logZ_live, Lstar
+  int32_t *d_surv_idx, *d_dead_idx, *d_rank, *d_rank_part, *d_flags;   // flags: [0] chol error, [1] threshold violation, [2] done
+  double *d_mean, *d_chol, *d_tune_scratch, *d_state;                      // state: logX, logZ, logZ_live, Lstar
   unsigned long long *d_nevals;
   NssCtl *d_ctl, *h_ctl;       // d_state, d_nevals, d_flags point into d_ctl; h_ctl is pinned, two slots
   cudaEvent_t ev_ctl[2];       // nss_run: the copy into slot i has landed
@@ -77,9 +84,6 @@ struct nss_handle {
   // device staging for the host-buffer entry points (grown on demand)
   unsigned char *d_stage;
   size_t stage_bytes;
-  // second stream for the kernels of an iteration that do not depend on each other
-  cudaStream_t st2;
-  cudaEvent_t ev_fork, ev_join, ev_sel, ev_evid;
   // device block and events of nss_run, kept between runs
   unsigned char *d_run;
   size_t run_bytes;

@@ -81,45 +81,90 @@ __global__ void k_init_live(const __grid_constant__ NssDev P, int n, uint64_t se
   live[idx] = __dadd_rn(P.lo[j], __dmul_rn(P.hi[j] - P.lo[j], u));   // unfused: same bits as the oracle
 }
 
-// ---- K4.1 (O12.1): rank of every live point in (logL, slot) order, by counting ------------------------------
-// rank_i = #{ j : logL_j < logL_i  or (logL_j == logL_i and j < i) }.  dead_idx[rank] = i for rank < k.
-constexpr int kRankThreads = 256;
-__global__ void __launch_bounds__(kRankThreads) k4_rank(const double *__restrict__ logL, int n, int k, int32_t *__restrict__ rank,
-                                                        int32_t *__restrict__ dead_idx, const int32_t *__restrict__ stop)
+// ---- K4 bookkeeping (O12.1 - O12.3, O14) as block-level device functions ------------------------------------------
+// They run either as kernels of their own (the test hooks nss_select_lowest / nss_tune / nss_evidence_update, the
+// initial stop test of nss_run) or inside the two fused kernels of an iteration: k4_front (rank + tune in parallel
+// blocks, then selection tail + evidence in whichever block finishes last) and the epilogue of K3 (live evidence).
+constexpr int kOneCta = 1024;
+constexpr int kRankElems = 256;          // live points ranked per block: 4 threads per point, each scanning a quarter of every tile
+
+struct K4Smem {
+  union {
+    struct { double tile[1024]; int cnt4[4 * kRankElems]; } rank;
+    struct { double part[kOneCta]; double mean[NSS_NSLOT]; double cov[NSS_NSLOT * NSS_NSLOT]; double Lc[NSS_NSLOT * NSS_NSLOT]; } tune;
+    struct { double red[32]; double warp_tot[32]; int iwarp_tot[32]; } red;
+  };
+  unsigned ticket;
+};
+
+// K4.1 (O12.1): rank_i = #{ j : logL_j < logL_i  or (logL_j == logL_i and j < i) }, by counting: exact and stable (ties by
+// slot).  The n x n comparisons are cut into blocks of kRankElems live points x one segment of J slots (4 threads per
+// point, a quarter of the segment each; the segment is staged in shared memory and read two values per load by
+// broadcast); a block writes the partial counts part[segment][i] and rank_finish adds them.  The kernel is bound by
+// instruction issue (~2.5 instructions per comparison), so the segments are short (J ~ 256, at most kRankMaxSeg of
+// them) to spread the work over every SM: ~3 us at n_live = 1000 .. 5000, ~0.5 ms at 65536 (where one
+// iteration of chains takes > 10 ms).
+constexpr int kRankMaxSeg = 32;
+__host__ __device__ inline int rank_segments(int n) { const int s = (n + 255) / 256; return s < 1 ? 1 : s < kRankMaxSeg ? s : kRankMaxSeg; }
+__host__ __device__ inline int rank_seg_len(int n) { const int nseg = rank_segments(n); return (((n + nseg - 1) / nseg) + 7) & ~7; }
+
+__device__ __forceinline__ void rank_block(const double *__restrict__ logL, int n, int be, int sg, int nseg, int32_t *__restrict__ part,
+                                           K4Smem &sm)
 {
-  __shared__ double tile[1024];
-  if (stop && stop[2]) return;                           // the run has converged: a speculatively queued iteration does nothing
-  const int i = blockIdx.x * kRankThreads + threadIdx.x;
+  const int e = threadIdx.x & (kRankElems - 1), seg4 = threadIdx.x >> 8;
+  const int i = be * kRankElems + e;
   const double Li = i < n ? logL[i] : INFINITY;
+  const double *tile = sm.rank.tile;
+  const int J = rank_seg_len(n), j0 = sg * J, j1 = min(n, j0 + J);
   int cnt = 0;
-  for (int base = 0; base < n; base += 1024) {
-    const int len = min(1024, n - base);
+  for (int base = j0; base < j1; base += 1024) {
+    const int len = min(1024, j1 - base);
     __syncthreads();
-    for (int t = threadIdx.x; t < len; t += kRankThreads) tile[t] = logL[base + t];
+    if ((int)threadIdx.x < len) sm.rank.tile[threadIdx.x] = logL[base + threadIdx.x];
     __syncthreads();
-    // j < i part of the tile uses <=, the rest uses <
-    const int split = max(0, min(len, i - base));
-    for (int t = 0; t < split; ++t) cnt += tile[t] <= Li;
-    for (int t = split; t < len; ++t) cnt += tile[t] < Li;
+    const int q = ((len + 3) / 4 + 1) & ~1;                // quarter of the tile per thread, even so that pairs stay aligned
+    const int t0 = min(len, seg4 * q), t1 = min(len, t0 + q);
+    const int split = max(t0, min(t1, i - base));          // tile positions before slot i count on <=, the rest on <
+    int t = t0;
+    for (; t < split && (t & 1); ++t) cnt += tile[t] <= Li;
+    for (; t + 1 < split; t += 2) { const double2 v = *reinterpret_cast<const double2 *>(tile + t); cnt += (int)(v.x <= Li) + (int)(v.y <= Li); }
+    for (; t < split; ++t) cnt += tile[t] <= Li;
+    for (; t < t1 && (t & 1); ++t) cnt += tile[t] < Li;
+    for (; t + 1 < t1; t += 2) { const double2 v = *reinterpret_cast<const double2 *>(tile + t); cnt += (int)(v.x < Li) + (int)(v.y < Li); }
+    for (; t < t1; ++t) cnt += tile[t] < Li;
   }
-  if (i < n) {
-    rank[i] = cnt;
-    if (cnt < k) dead_idx[cnt] = i;
-  }
+  __syncthreads();
+  sm.rank.cnt4[seg4 * kRankElems + e] = cnt;
+  __syncthreads();
+  if (seg4 == 0 && i < n)
+    part[(size_t)sg * n + i] = sm.rank.cnt4[e] + sm.rank.cnt4[kRankElems + e] + sm.rank.cnt4[2 * kRankElems + e] + sm.rank.cnt4[3 * kRankElems + e];
+  __syncthreads();
 }
 
-// ---- K4.2: survivor compaction (ascending slot), gather of the dead rows, threshold -----------------------
-constexpr int kOneCta = 1024;
-__global__ void __launch_bounds__(kOneCta) k4_finish_select(const double *__restrict__ live, const double *__restrict__ logL,
-                                                            const double *__restrict__ birth, int n, int k, int d,
-                                                            double Lstar_in, const int32_t *__restrict__ rank,
-                                                            const int32_t *__restrict__ dead_idx, int32_t *__restrict__ surv_idx,
-                                                            double *__restrict__ dead_theta, double *__restrict__ dead_logL,
-                                                            double *__restrict__ dead_birth, double *__restrict__ state,
-                                                            int32_t *__restrict__ flags)
+// one block: rank_i = sum of the partial counts; dead_idx[rank] = i for rank < k
+__device__ __forceinline__ void rank_finish(const int32_t *__restrict__ part, int n, int k, int nseg, int32_t *__restrict__ rank,
+                                            int32_t *__restrict__ dead_idx)
 {
-  __shared__ int warp_tot[32];
-  if (flags[2] && live) return;                          // converged (nss_run queues one iteration ahead); the select hook passes live = NULL
+  for (int i = threadIdx.x; i < n; i += blockDim.x) {
+    int c = 0;
+#pragma unroll 8                              // independent L2 loads: keep several in flight
+    for (int sg = 0; sg < nseg; ++sg) c += __ldcg(part + (size_t)sg * n + i);
+    rank[i] = c;
+    if (c < k) dead_idx[c] = i;
+  }
+  __syncthreads();
+}
+
+// K4.2: survivor compaction (ascending slot), gather of the dead rows, threshold.  Returns (to every thread) whether a
+// survivor lies below a supplied threshold.
+__device__ __forceinline__ int finish_select_block(const double *__restrict__ live, const double *__restrict__ logL,
+                                                   const double *__restrict__ birth, int n, int k, int d, double Lstar_in,
+                                                   const int32_t *__restrict__ rank, const int32_t *__restrict__ dead_idx,
+                                                   int32_t *__restrict__ surv_idx, double *__restrict__ dead_theta,
+                                                   double *__restrict__ dead_logL, double *__restrict__ dead_birth,
+                                                   double *__restrict__ state, K4Smem &sm)
+{
+  int *warp_tot = sm.red.iwarp_tot;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const double Lstar = isnan(Lstar_in) ? logL[dead_idx[k - 1]] : Lstar_in;
   const int chunk = (n + kOneCta - 1) / kOneCta;
@@ -134,6 +179,7 @@ __global__ void __launch_bounds__(kOneCta) k4_finish_select(const double *__rest
     const int v = __shfl_up_sync(0xffffffffu, incl, o);
     if (lane >= o) incl += v;
   }
+  __syncthreads();
   if (lane == 31) warp_tot[wid] = incl;
   __syncthreads();
   if (wid == 0) {
@@ -150,18 +196,19 @@ __global__ void __launch_bounds__(kOneCta) k4_finish_select(const double *__rest
   if (surv_idx)
     for (int i = i0; i < i1; ++i)
       if (rank[i] >= k) surv_idx[pos++] = i;
-  if (bad) flags[1] = 1;
   for (int j = tid; j < k; j += kOneCta) {
     const int slot = dead_idx[j];
     if (dead_logL) dead_logL[j] = logL[slot];
     if (dead_birth) dead_birth[j] = birth ? birth[slot] : -INFINITY;
-    if (dead_theta)
+    if (dead_theta) {
+#pragma unroll 11                             // independent L2 loads of one row
       for (int a = 0; a < d; ++a) dead_theta[(size_t)j * d + a] = live[(size_t)slot * d + a];
+    }
   }
   if (tid == 0 && state) state[3] = Lstar;
+  return __syncthreads_or(bad ? 1 : 0);
 }
 
-// ---- K4.3 (O12.3): mean, covariance (two-pass, 1/(n-1)), lower Cholesky -------------------------------------
 __device__ __forceinline__ double block_sum(double v, double *red)
 {
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -175,56 +222,100 @@ __device__ __forceinline__ double block_sum(double v, double *red)
   return s;
 }
 
-// Column sums and the d(d+1)/2 centred products are split over row groups (thread = (row group, column) or
-// (row group, pair)); the groups are then added in a fixed order, so the result is deterministic.
-__global__ void __launch_bounds__(kOneCta) k4_tune(const double *__restrict__ live, int n, int d, double *__restrict__ mean_out,
-                                                   double *__restrict__ chol_out, int32_t *__restrict__ flags)
+// K4.3 (O12.3): mean, covariance (two-pass, 1/(n-1)), lower Cholesky, by T co-resident blocks (T <= kTuneMaxBlocks; they
+// are the first blocks of their grid, so they are scheduled together).  Block b owns the rows [b n/T, (b+1) n/T): column
+// sums, then — after a counter barrier among the T blocks — the d(d+1)/2 centred products of its rows; inside a block
+// the rows are split over thread groups (thread = (row group, column) or (row group, pair)) and added in a fixed order,
+// and the blocks' partial sums are added in block order, so the result is deterministic.  The block that finishes last
+// factors the matrix: *chol_fail = 1 if a pivot is <= 0 (reading R5: no relative epsilon), else 0.
+constexpr int kTuneMaxBlocks = 32;
+constexpr int kTunePartDoubles = NSS_NSLOT + NSS_NSLOT * (NSS_NSLOT + 1) / 2;     // per block: column sums, then products
+__host__ __device__ inline int tune_blocks_for(int n) { const int t = n / 128; return t < 1 ? 1 : t > kTuneMaxBlocks ? kTuneMaxBlocks : t; }
+
+__device__ __forceinline__ void tune_block(const double *__restrict__ live, int n, int d, int b, int T, double *__restrict__ scratch,
+                                           uint32_t *__restrict__ counters /*[2]*/, double *__restrict__ mean_out,
+                                           double *__restrict__ chol_out, int32_t *__restrict__ chol_fail, K4Smem &sm)
 {
-  __shared__ double part[kOneCta];
-  __shared__ double mean[NSS_NSLOT];
-  __shared__ double cov[NSS_NSLOT * NSS_NSLOT];
-  if (flags[2]) return;
+  double *part = sm.tune.part, *mean = sm.tune.mean, *cov = sm.tune.cov, *sLc = sm.tune.Lc;
   const int tid = threadIdx.x;
+  const int r0 = (int)((long long)n * b / T), r1 = (int)((long long)n * (b + 1) / T);
+  const int np = d * (d + 1) / 2;
   {
     const int ng = kOneCta / d, j = tid % d, g = tid / d;
     double s = 0.0;
-    if (g < ng)
-      for (int i = g; i < n; i += ng) s += live[(size_t)i * d + j];
+    if (g < ng) {
+#pragma unroll 8                              // the rows come from L2: keep several loads in flight (same order of additions)
+      for (int i = r0 + g; i < r1; i += ng) s += live[(size_t)i * d + j];
+    }
     part[tid] = s;
     __syncthreads();
+    int top = 1;
+    while (2 * top < ng) top *= 2;
+    for (int step = top; step >= 1; step >>= 1) {           // pairwise tree over the row groups: fixed order, deterministic
+      if (g < step && g + step < ng) part[tid] += part[tid + step * d];
+      __syncthreads();
+    }
+    if (tid < d) scratch[b * kTunePartDoubles + tid] = part[tid];
+    if (T > 1) {                                // every block needs every block's column sums
+      __threadfence();
+      __syncthreads();
+      if (tid == 0) {
+        atomicAdd(&counters[0], 1u);
+        while (*(volatile uint32_t *)&counters[0] < (uint32_t)T) {}
+      }
+      __syncthreads();
+      __threadfence();
+    } else __syncthreads();
     if (tid < d) {
       double t = 0.0;
-      for (int q = 0; q < ng; ++q) t += part[q * d + tid];
+      for (int q = 0; q < T; ++q) t += __ldcg(scratch + q * kTunePartDoubles + tid);
       mean[tid] = t / n;
     }
     __syncthreads();
   }
+  int a = 0, bb = 0;
   {
-    const int np = d * (d + 1) / 2, ng = kOneCta / np, p = tid % np, g = tid / np;
-    int a = 0, rem = p;                       // pair index p -> (a, b), b <= a, row-major lower triangle
+    const int ng = kOneCta / np, p = tid % np, g = tid / np;
+    int rem = p;                              // pair index p -> (a, bb), bb <= a, row-major lower triangle
     while (rem > a) { rem -= a + 1; ++a; }
-    const int b = rem;
+    bb = rem;
     double s = 0.0;
     if (g < ng) {
-      const double ma = mean[a], mb = mean[b];
-      for (int i = g; i < n; i += ng) s = fma(live[(size_t)i * d + a] - ma, live[(size_t)i * d + b] - mb, s);
+      const double ma = mean[a], mb = mean[bb];
+#pragma unroll 8
+      for (int i = r0 + g; i < r1; i += ng) s = fma(live[(size_t)i * d + a] - ma, live[(size_t)i * d + bb] - mb, s);
     }
+    __syncthreads();
     part[tid] = s;
     __syncthreads();
-    if (tid < np) {
-      double t = 0.0;
-      for (int q = 0; q < ng; ++q) t += part[q * np + tid];
-      cov[a * d + b] = t / (n - 1);
-      cov[b * d + a] = t / (n - 1);
+    int top = 1;
+    while (2 * top < ng) top *= 2;
+    for (int step = top; step >= 1; step >>= 1) {
+      if (g < step && g + step < ng) part[tid] += part[tid + step * np];
+      __syncthreads();
     }
-    __syncthreads();
+    if (tid < np) scratch[b * kTunePartDoubles + NSS_NSLOT + tid] = part[tid];
   }
+  if (T > 1) {                                  // the block that finishes last adds the partial products and factors
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) sm.ticket = atomicAdd(&counters[1], 1u);
+    __syncthreads();
+    if (sm.ticket != (unsigned)T - 1u) return;
+    __threadfence();
+  } else __syncthreads();
+  if (tid < np) {
+    double t = 0.0;
+    for (int q = 0; q < T; ++q) t += __ldcg(scratch + q * kTunePartDoubles + NSS_NSLOT + tid);
+    cov[a * d + bb] = t / (n - 1);
+    cov[bb * d + a] = t / (n - 1);
+  }
+  __syncthreads();
   // Cholesky by the first warp, column by column: lane i owns row i.  Every element is the same sum in the same
   // order as the row-by-row definition (s = cov_ij - sum_{m<j} L_im L_jm), only the rows of a column run side by side.
-  __shared__ double sLc[NSS_NSLOT * NSS_NSLOT];
   if (tid < 32) {
     const int i = tid;
-    for (int a = tid; a < d * d; a += 32) sLc[a] = 0.0;
+    for (int q = tid; q < d * d; q += 32) sLc[q] = 0.0;
     __syncwarp();
     bool ok = true;
     for (int j = 0; j < d; ++j) {
@@ -240,15 +331,15 @@ __global__ void __launch_bounds__(kOneCta) k4_tune(const double *__restrict__ li
       else if (i > j && i < d) sLc[i * d + j] = sacc / ljj;
       __syncwarp();
     }
-    if (!ok && tid == 0) flags[0] = 1;
+    if (tid == 0) *chol_fail = ok ? 0 : 1;
     __syncwarp();
-    for (int a = tid; a < d * d; a += 32) chol_out[a] = sLc[a];
+    for (int q = tid; q < d * d; q += 32) chol_out[q] = sLc[q];
     if (mean_out)
-      for (int a = tid; a < d; a += 32) mean_out[a] = mean[a];
+      for (int q = tid; q < d; q += 32) mean_out[q] = mean[q];
   }
+  __syncthreads();
 }
 
-// ---- K4.4 (O12.2): log-weights of the dead points, logX shrinkage, logZ accumulation -------------------------
 __device__ __forceinline__ double block_max(double v, double *red)
 {
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -271,15 +362,14 @@ __device__ __forceinline__ double logaddexp_d(double a, double b)
   return m + log(exp(a - m) + exp(b - m));
 }
 
-__global__ void __launch_bounds__(kOneCta) k4_evidence(const double *__restrict__ dead_logL, int n, int k, double *__restrict__ logw,
-                                                       double *__restrict__ state, const int32_t *__restrict__ stop)
+// K4.4 (O12.2): log-weights of the dead points, logX shrinkage, logZ accumulation; one block of any size (multiple of 32)
+__device__ __forceinline__ void evidence_block(const double *__restrict__ dead_logL, int n, int k, double *__restrict__ logw,
+                                               double *__restrict__ state, K4Smem &sm)
 {
-  __shared__ double red[32];
-  if (stop && stop[2]) return;
-  __shared__ double warp_tot[32];
+  double *red = sm.red.red, *warp_tot = sm.red.warp_tot;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const double logX0 = state[0], logZ0 = state[1];
-  const int chunk = (k + kOneCta - 1) / kOneCta;
+  const int nt = blockDim.x, chunk = (k + nt - 1) / nt;
   const int j0 = min(k, tid * chunk), j1 = min(k, j0 + chunk);
   double part = 0.0;
   for (int j = j0; j < j1; ++j) part += 1.0 / (double)(n - j);
@@ -289,6 +379,9 @@ __global__ void __launch_bounds__(kOneCta) k4_evidence(const double *__restrict_
     const double v = __shfl_up_sync(0xffffffffu, incl, o);
     if (lane >= o) incl += v;
   }
+  __syncthreads();
+  if (tid < 32) warp_tot[tid] = 0.0;
+  __syncthreads();
   if (lane == 31) warp_tot[wid] = incl;
   __syncthreads();
   if (wid == 0) {
@@ -320,6 +413,39 @@ __global__ void __launch_bounds__(kOneCta) k4_evidence(const double *__restrict_
     state[0] = logX0 - total;
     state[1] = mx > -INFINITY ? logaddexp_d(logZ0, mx + log(se)) : logZ0;
   }
+  __syncthreads();
+}
+
+// ---- stand-alone kernels (test hooks; the final ordering of the live points in nss_run) -------------------------------
+__global__ void __launch_bounds__(kOneCta) k4_rank(const double *__restrict__ logL, int n, int nseg, int32_t *__restrict__ part)
+{
+  __shared__ K4Smem sm;
+  rank_block(logL, n, blockIdx.x / nseg, blockIdx.x % nseg, nseg, part, sm);
+}
+
+// surv_idx == NULL: only the ordering (rank, dead_idx) is wanted
+__global__ void __launch_bounds__(kOneCta) k4_finish_select(const double *__restrict__ logL, int n, int k, int nseg,
+                                                            const int32_t *__restrict__ part, int32_t *__restrict__ rank,
+                                                            int32_t *__restrict__ dead_idx, int32_t *__restrict__ surv_idx,
+                                                            double *__restrict__ state)
+{
+  __shared__ K4Smem sm;
+  rank_finish(part, n, k, nseg, rank, dead_idx);
+  if (surv_idx) finish_select_block(nullptr, logL, nullptr, n, k, 0, NAN, rank, dead_idx, surv_idx, nullptr, nullptr, nullptr, state, sm);
+}
+
+__global__ void __launch_bounds__(kOneCta) k4_tune(const double *__restrict__ live, int n, int d, int T, double *__restrict__ scratch,
+                                                   NssCtl *ctl, double *__restrict__ mean_out, double *__restrict__ chol_out)
+{
+  __shared__ K4Smem sm;
+  tune_block(live, n, d, blockIdx.x, T, scratch, ctl->tune_cnt, mean_out, chol_out, &ctl->flags[0], sm);
+}
+
+__global__ void __launch_bounds__(kOneCta) k4_evidence(const double *__restrict__ dead_logL, int n, int k, double *__restrict__ logw,
+                                                       double *__restrict__ state)
+{
+  __shared__ K4Smem sm;
+  evidence_block(dead_logL, n, k, logw, state, sm);
 }
 
 // ---- K4.5 (O14): live evidence and stop test ------------------------------------------------------------------
@@ -339,6 +465,64 @@ __global__ void __launch_bounds__(kOneCta) k4_live_evidence(const double *__rest
     state[2] = lzl;
     if (check && (lzl - state[1] < stop_dlogz)) flags[2] = 1;
   }
+}
+
+// ---- the front of an NS iteration in ONE launch ---------------------------------------------------------------------
+// blocks 0 .. T-1 tune (a3: mean, covariance, Cholesky), the others rank the live points (a1) beside them; the rank block
+// that finishes last adds the partial ranks, compacts the survivors, gathers the dead rows and fixes the threshold (a1); the
+// block that finishes last of all publishes the flags and resets the counters.  `reset` = a stand-alone iteration (nss_iterate, nss_replace_step): flags and,
+// on request, state and counters are re-initialised; otherwise (nss_run's loop, queued one iteration ahead of the host) an
+// iteration queued after convergence or after a Cholesky failure does nothing.
+struct FrontArgs {
+  const double *live, *logL, *birth;
+  int32_t n, k, d, T, nseg;
+  double Lstar_in;
+  int32_t *rank_part, *rank, *dead_idx, *surv_idx;
+  double *dead_theta, *dead_logL, *dead_birth;
+  double *tune_scratch, *mean, *chol;
+  NssCtl *ctl;
+  int32_t reset, set_state, zero_evals;
+  double logX, logZ;
+};
+
+__global__ void __launch_bounds__(kOneCta) k4_front(const FrontArgs A)
+{
+  __shared__ K4Smem sm;
+  NssCtl *ctl = A.ctl;
+  if (!A.reset && (ctl->flags[2] | ctl->flags[0])) return;
+  const int b = blockIdx.x;
+  if (b < A.T) {
+    tune_block(A.live, A.n, A.d, b, A.T, A.tune_scratch, ctl->tune_cnt, A.mean, A.chol, &ctl->chol_now, sm);
+  } else {
+    rank_block(A.logL, A.n, (b - A.T) / A.nseg, (b - A.T) % A.nseg, A.nseg, A.rank_part, sm);
+    // the rank block that finishes last runs the selection tail (it does not wait for the tuning blocks)
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) sm.ticket = atomicAdd(&ctl->rank_done, 1u);
+    __syncthreads();
+    if (sm.ticket == gridDim.x - A.T - 1u) {
+      __threadfence();
+      rank_finish(A.rank_part, A.n, A.k, A.nseg, A.rank, A.dead_idx);
+      const int bad = finish_select_block(A.live, A.logL, A.birth, A.n, A.k, A.d, A.Lstar_in, A.rank, A.dead_idx, A.surv_idx, A.dead_theta,
+                                          A.dead_logL, A.dead_birth, ctl->state, sm);
+      if (threadIdx.x == 0) ctl->sel_bad = bad;
+    }
+  }
+  // the block that finishes last of all publishes the flags and resets the counters
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) sm.ticket = atomicAdd(&ctl->front_done, 1u);
+  __syncthreads();
+  if (sm.ticket != gridDim.x - 1 || threadIdx.x != 0) return;
+  __threadfence();
+  ctl->front_done = 0; ctl->rank_done = 0; ctl->chains_done = 0; ctl->tune_cnt[0] = 0; ctl->tune_cnt[1] = 0;
+  const int chol_fail = *(volatile int32_t *)&ctl->chol_now;
+  ctl->flags[1] = *(volatile int32_t *)&ctl->sel_bad;
+  if (A.reset) {
+    ctl->flags[0] = chol_fail; ctl->flags[2] = 0; ctl->flags[3] = 0;
+    if (A.set_state) { ctl->state[0] = A.logX; ctl->state[1] = A.logZ; ctl->state[2] = 0.0; }
+    if (A.zero_evals) { ctl->nevals = 0ull; ctl->nrounds = 0ull; ctl->nexec = 0ull; }
+  } else if (chol_fail) ctl->flags[0] = 1;
 }
 
 // ---- O15: evidence-error replicas (stochastic compression), one CTA per replica -------------------------------
@@ -450,11 +634,20 @@ __global__ void k_gather_rows(const double *__restrict__ live, const double *__r
 // ---- a5: slice directions of every (chain, step), one thread each ------------------------------------------------
 // z ~ N(0, I_d) by Box-Muller (one Philox block per pair: counter (1 + pair, step, chain, iteration)),
 // n = z/|z|, v = w L n with L the Cholesky factor of the live-point covariance (O12.4a).
+// The last block of the grid does not draw directions: it runs the evidence bookkeeping of the deleted batch (a2, O12.2:
+// it needs only the dead logL that k4_front has gathered), beside the direction blocks and off the critical path.
 __global__ void __launch_bounds__(128) k_directions(int d, const double *__restrict__ chol, int k, int n_repeats, uint64_t seed,
-                                                    uint32_t it, const int32_t *__restrict__ flags, double *__restrict__ dirs)
+                                                    uint32_t it, const int32_t *__restrict__ flags, double *__restrict__ dirs,
+                                                    int n, const double *__restrict__ dead_logL, double *__restrict__ dead_logw,
+                                                    double *__restrict__ state)
 {
   __shared__ double sL[NSS_NSLOT * NSS_NSLOT];
-  if (flags[0] | flags[2]) return;                       // Cholesky failed, or converged (flags[1] belongs to the selection, which runs beside this)
+  if (flags[0] | flags[1] | flags[2]) return;            // Cholesky failure, threshold violation, or converged
+  if (blockIdx.x == gridDim.x - 1) {
+    __shared__ K4Smem sm;
+    if (dead_logw) evidence_block(dead_logL, n, k, dead_logw, state, sm);
+    return;
+  }
   for (int t = threadIdx.x; t < d * d; t += blockDim.x) sL[t] = chol[t];
   __syncthreads();
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
@@ -524,13 +717,12 @@ struct ChainArgs {
   uint32_t iteration;
   const int32_t *surv_idx, *dead_idx;
   const double *dirs;           // [k][n_repeats][d] slice directions v = w L z/|z| (k_directions)
-  const double *state;          // state[3] = L*
-  const int32_t *flags;         // flags[0] != 0 (Cholesky failure) or flags[1] != 0 -> do nothing
-  unsigned long long *n_evals;
-  unsigned long long *diag;     // [2]: rounds, evaluated candidates
+  NssCtl *ctl;                  // state[3] = L*; flags (any set -> do nothing); evaluation counters; chains_done
   int32_t *trace;               // optional [k][n_repeats][3]
   double *margin;               // optional [k]
   int32_t G;                    // warps per chain
+  int32_t live_evidence;        // the CTA that finishes the last chain computes logZ_live and the stop test (a11, O14)
+  double stop_dlogz;
 };
 
 constexpr int kChainWarps = 8;          // largest group; a CTA is ONE group (G warps), one chain at a time
@@ -554,7 +746,7 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
   __shared__ double sX[kChainWarps][NSS_NSLOT + 1];                // chain position, one copy per warp (lane-level box tests)
   __shared__ double sLo[NSS_NSLOT + 1], sHi[NSS_NSLOT + 1];        // prior box, (-inf, +inf) for the unused coordinates
   __shared__ __align__(16) double sConst[nssk::kSubConstDoubles];
-  if (A.flags[0] | A.flags[1] | A.flags[2]) return;      // Cholesky failure, threshold violation, or converged
+  __shared__ unsigned sLast;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int sl = lane & (LANES - 1), sub = lane / LANES;
   nssk::SubCtx X;
@@ -585,11 +777,16 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
     nssk::mbar_wait(&bar, 0);
     X.tab = reinterpret_cast<const double *>(smem_raw);
   }
-  const int G = blockDim.x >> 5, GL = blockDim.x, C = G * NSUB;
+  // Everything above is independent of the kernels in front (programmatic dependent launch: it overlaps their tails);
+  // everything below reads what k4_front and k_directions wrote.
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  NssCtl *ctl = A.ctl;
+  if (ctl->flags[0] | ctl->flags[1] | ctl->flags[2]) return;      // Cholesky failure, threshold violation, or converged
+  const int G = blockDim.x >> 5, C = G * NSUB;
   const int w = warp;                                    // warp in the group
   const int gl = w * 32 + lane;                          // lane in the group
   const int cs = w * NSUB + sub;                         // candidate slot of this sub-warp in the group
-  const double Lstar = A.state[3];
+  const double Lstar = ctl->state[3];
   const uint32_t it = A.iteration;
   const int ns = A.n - A.k;
   bool own[NC];
@@ -605,7 +802,6 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
     dst_idx[c] = own[c] ? (KIND == NSS_KIND_GAUSS ? j : P.param_index[j]) : 0;
     per[c] = own[c] && P.periodic[j] != 0;
   }
-  const unsigned sub_mask = (LANES == 32 ? 0xffffffffu : ((1u << LANES) - 1u)) << (sub * LANES);
   int par = 0;
 
   for (int ch = blockIdx.x; ch < A.k; ch += gridDim.x) {
@@ -787,9 +983,43 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
         A.logL[dst] = lx;
         if (A.birth) A.birth[dst] = Lstar;
         if (A.margin) A.margin[ch] = margin_all;
-        atomicAdd(A.n_evals, (unsigned long long)evals);
-        atomicAdd(A.diag, (unsigned long long)rounds);
-        atomicAdd(A.diag + 1, (unsigned long long)nexec);
+        atomicAdd(&ctl->nevals, (unsigned long long)evals);
+        atomicAdd(&ctl->nrounds, (unsigned long long)rounds);
+        atomicAdd(&ctl->nexec, (unsigned long long)nexec);
+      }
+    }
+    // a11 (O14) as epilogue: the CTA that finishes the last chain of the iteration computes
+    // logZ_live = logX + logsumexp(logL) - ln n over the updated live set and applies the stop test
+    if (A.live_evidence) {
+      __threadfence();
+      __syncthreads();
+      if (threadIdx.x == 0) sLast = atomicAdd(&ctl->chains_done, 1u);
+      __syncthreads();
+      if (sLast == (unsigned)A.k - 1u) {
+        __threadfence();
+        double *red = sRes[0];
+        double mx = -INFINITY;
+        for (int i = threadIdx.x; i < A.n; i += blockDim.x) mx = fmax(mx, __ldcg(A.logL + i));
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        if (lane == 0) red[warp] = mx;
+        __syncthreads();
+        mx = red[0];
+        for (int q = 1; q < G; ++q) mx = fmax(mx, red[q]);
+        __syncthreads();
+        double se = 0.0;
+        if (mx > -INFINITY)
+          for (int i = threadIdx.x; i < A.n; i += blockDim.x) se += exp(__ldcg(A.logL + i) - mx);
+        se = nssk::warp_sum(se);
+        if (lane == 0) red[warp] = se;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+          double tot = 0.0;
+          for (int q = 0; q < G; ++q) tot += red[q];          // fixed order: deterministic
+          const double lzl = mx > -INFINITY ? ctl->state[0] + mx + log(tot) - log((double)A.n) : -INFINITY;
+          ctl->state[2] = lzl;
+          if (lzl - ctl->state[1] < A.stop_dlogz) ctl->flags[2] = 1;
+        }
       }
     }
   }
@@ -801,7 +1031,7 @@ int launch_chains_k(nss_handle *h, ChainArgs &A, size_t tab_bytes, cudaStream_t 
   auto kern = k3_slice<NDET, KIND, LANES, RESIDENT>;
   int G = h->chain_warps;
   if (G != 1 && G != 2 && G != 4 && G != 8) {
-    // automatic (measured on B200, _work sweeps -> DESIGN.md §6): a chain is a serial process, so few chains want
+    // automatic (measured on B200: profiles/r02_k3_sweeps.md): a chain is a serial process, so few chains want
     // wide speculation, but once there are about as many warps as SM sub-partitions (4 per SM) the kernel turns
     // throughput-bound and every speculative evaluation costs time
     const long long S = 4LL * h->n_sm;
@@ -809,9 +1039,20 @@ int launch_chains_k(nss_handle *h, ChainArgs &A, size_t tab_bytes, cudaStream_t 
   }
   A.G = G;
   const size_t smem = tab_bytes + (size_t)G * (32 / LANES) * nssk::kSubScratchDoubles * sizeof(double);
-  NSS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  static size_t smem_set = 0;                            // per instantiation: the attribute is raised only when a launch needs more
+  if (smem > smem_set) {
+    NSS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    smem_set = smem;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)A.k);                     // one chain per CTA: the block scheduler balances the SMs
+  cfg.blockDim = dim3(32u * G); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;      // the prologue (table staging) overlaps the kernels in front
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
   NSS_CUDA(cudaEventRecord(h->ev_k3[0], st));
-  kern<<<A.k, 32 * G, smem, st>>>(h->dev, A);            // one chain per CTA: the block scheduler balances the SMs
+  NSS_CUDA(cudaLaunchKernelEx(&cfg, kern, h->dev, A));
   NSS_CUDA(cudaEventRecord(h->ev_k3[1], st));
   return NSS_OK;
 }
@@ -854,11 +1095,12 @@ int launch_chains(nss_handle *h, ChainArgs &A, cudaStream_t st)
   return NSS_OK;
 }
 
-// start of an iteration: clear the flags (and the evaluation counter), optionally load logX / logZ
+// start of a stand-alone hook call: clear the flags (and the evaluation counter), optionally load logX / logZ
 __global__ void k_begin(NssCtl *ctl, int set_state, double logX, double logZ, int zero_evals)
 {
   if (threadIdx.x < 4) ctl->flags[threadIdx.x] = 0;
   if (threadIdx.x == 0) {
+    ctl->front_done = 0; ctl->rank_done = 0; ctl->sel_bad = 0; ctl->chains_done = 0; ctl->chol_now = 0; ctl->tune_cnt[0] = 0; ctl->tune_cnt[1] = 0;
     if (set_state) { ctl->state[0] = logX; ctl->state[1] = logZ; ctl->state[2] = 0.0; ctl->state[3] = 0.0; }
     if (zero_evals) { ctl->nevals = 0ull; ctl->nrounds = 0ull; ctl->nexec = 0ull; }
   }
@@ -872,7 +1114,7 @@ int begin_iteration(nss_handle *h, int set_state, double logX, double logZ, int 
   return NSS_OK;
 }
 
-// one 56-byte copy of the control block into the pinned mirror, then wait for the stream
+// one copy of the control block into the pinned mirror, then wait for the stream
 int fetch_ctl(nss_handle *h, cudaStream_t st)
 {
   NSS_CUDA(cudaMemcpyAsync(h->h_ctl, h->d_ctl, sizeof(NssCtl), cudaMemcpyDeviceToHost, st));
@@ -883,24 +1125,22 @@ int fetch_ctl(nss_handle *h, cudaStream_t st)
 int ensure_scratch(nss_handle *h, int n)
 {
   if (h->scratch_n >= n && h->d_flags) return NSS_OK;
-  cudaFree(h->d_surv_idx); cudaFree(h->d_dead_idx); cudaFree(h->d_rank); cudaFree(h->d_birth);
-  h->d_surv_idx = h->d_dead_idx = h->d_rank = nullptr; h->d_birth = nullptr;
+  cudaFree(h->d_surv_idx); cudaFree(h->d_dead_idx); cudaFree(h->d_rank); cudaFree(h->d_rank_part); cudaFree(h->d_birth);
+  h->d_surv_idx = h->d_dead_idx = h->d_rank = h->d_rank_part = nullptr; h->d_birth = nullptr;
   NSS_CUDA(cudaMalloc(&h->d_surv_idx, sizeof(int32_t) * n));
   NSS_CUDA(cudaMalloc(&h->d_dead_idx, sizeof(int32_t) * n));
   NSS_CUDA(cudaMalloc(&h->d_rank, sizeof(int32_t) * n));
+  NSS_CUDA(cudaMalloc(&h->d_rank_part, sizeof(int32_t) * (size_t)n * kRankMaxSeg));
   NSS_CUDA(cudaMalloc(&h->d_birth, sizeof(double) * n));
   if (!h->d_flags) {
     NSS_CUDA(cudaMalloc(&h->d_ctl, sizeof(NssCtl)));
+    NSS_CUDA(cudaMemset(h->d_ctl, 0, sizeof(NssCtl)));
     NSS_CUDA(cudaMallocHost(&h->h_ctl, 2 * sizeof(NssCtl)));     // [1] is nss_run's second slot
     NSS_CUDA(cudaEventCreateWithFlags(&h->ev_ctl[0], cudaEventDisableTiming));
     NSS_CUDA(cudaEventCreateWithFlags(&h->ev_ctl[1], cudaEventDisableTiming));
     NSS_CUDA(cudaMalloc(&h->d_mean, sizeof(double) * NSS_NSLOT));
     NSS_CUDA(cudaMalloc(&h->d_chol, sizeof(double) * NSS_NSLOT * NSS_NSLOT));
-    NSS_CUDA(cudaStreamCreateWithFlags(&h->st2, cudaStreamNonBlocking));
-    NSS_CUDA(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
-    NSS_CUDA(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming));
-    NSS_CUDA(cudaEventCreateWithFlags(&h->ev_sel, cudaEventDisableTiming));
-    NSS_CUDA(cudaEventCreateWithFlags(&h->ev_evid, cudaEventDisableTiming));
+    NSS_CUDA(cudaMalloc(&h->d_tune_scratch, sizeof(double) * kTuneMaxBlocks * kTunePartDoubles));
     h->d_state = h->d_ctl->state;             // addresses inside the device block (not dereferenced on the host)
     h->d_nevals = &h->d_ctl->nevals;
     h->d_flags = h->d_ctl->flags;
@@ -909,20 +1149,20 @@ int ensure_scratch(nss_handle *h, int n)
   return NSS_OK;
 }
 
-// the device part of one NS iteration (no host synchronisation): K4.1, K4.2, K4.3, K3
+// The device part of one NS iteration (no host synchronisation), three launches:
+//   k4_front      a1 rank/select, a3 tune, flag and counter reset
+//   k_directions  a5 for every (chain, step); a2 evidence (if dead_logw) in one more block beside them
+//   k3_slice      a4, a6 - a10, and a11's live evidence + stop test as epilogue (if live_evidence)
+// `reset`: a stand-alone iteration (flags cleared; logX / logZ loaded and counters zeroed on request).
 int enqueue_iteration(nss_handle *h, double *live, double *logL, double *birth, int n, int k, double Lstar_in, int n_repeats,
                       uint64_t seed, uint32_t iteration, double *dead_theta, double *dead_logL, double *dead_birth,
-                      int32_t *dead_idx, double *dead_logw, cudaStream_t st)
+                      int32_t *dead_idx, double *dead_logw, int reset, int set_state, double logX, double logZ, int zero_evals,
+                      int live_evidence, double stop_dlogz, cudaStream_t st)
 {
   const int d = h->dev.d;
-  // Second stream: the tuning (a3) and the directions (a5) do not depend on the selection (a1) and run beside it;
-  // the evidence update (a2) needs only the dead logL, so it runs beside the chains (K3).
-  NSS_CUDA(cudaEventRecord(h->ev_fork, st));
-  NSS_CUDA(cudaStreamWaitEvent(h->st2, h->ev_fork, 0));
-  k4_tune<<<1, kOneCta, 0, h->st2>>>(live, n, d, h->d_mean, h->d_chol, h->d_flags);
   {
     const size_t need = sizeof(double) * (size_t)k * (n_repeats > 0 ? n_repeats : 1) * d;
-    if (h->dirs_bytes < need) {
+    if (h->dirs_bytes < need) {                          // first use, or a larger n_delete x n_repeats than before
       NSS_CUDA(cudaDeviceSynchronize());                 // an earlier launch may still read the old block
       cudaFree(h->d_dirs);
       h->d_dirs = nullptr; h->dirs_bytes = 0;
@@ -930,37 +1170,32 @@ int enqueue_iteration(nss_handle *h, double *live, double *logL, double *birth, 
       if (e != cudaSuccess) { nss_cuda_fail(e, "cudaMalloc(dirs)"); return e == cudaErrorMemoryAllocation ? NSS_ENOMEM : NSS_ECUDA; }
       h->dirs_bytes = need;
     }
-    if (n_repeats > 0)
-      k_directions<<<(k * n_repeats + 127) / 128, 128, 0, h->st2>>>(d, h->d_chol, k, n_repeats, seed, iteration, h->d_flags, h->d_dirs);
   }
-  NSS_CUDA(cudaEventRecord(h->ev_join, h->st2));
-  k4_rank<<<(n + kRankThreads - 1) / kRankThreads, kRankThreads, 0, st>>>(logL, n, k, h->d_rank, dead_idx, h->d_flags);
-  k4_finish_select<<<1, kOneCta, 0, st>>>(live, logL, birth, n, k, d, Lstar_in, h->d_rank, dead_idx, h->d_surv_idx, dead_theta,
-                                          dead_logL, dead_birth, h->d_state, h->d_flags);
-  h->launches += n_repeats > 0 ? 4 : 3;
-  if (dead_logw) {
-    NSS_CUDA(cudaEventRecord(h->ev_sel, st));
-    NSS_CUDA(cudaStreamWaitEvent(h->st2, h->ev_sel, 0));
-    k4_evidence<<<1, kOneCta, 0, h->st2>>>(dead_logL, n, k, dead_logw, h->d_state, h->d_flags);
-    NSS_CUDA(cudaEventRecord(h->ev_evid, h->st2));
+  FrontArgs F;
+  F.live = live; F.logL = logL; F.birth = birth; F.n = n; F.k = k; F.d = d; F.Lstar_in = Lstar_in;
+  F.T = tune_blocks_for(n); F.nseg = rank_segments(n);
+  F.rank_part = h->d_rank_part; F.rank = h->d_rank; F.dead_idx = dead_idx; F.surv_idx = h->d_surv_idx; F.tune_scratch = h->d_tune_scratch;
+  F.dead_theta = dead_theta; F.dead_logL = dead_logL; F.dead_birth = dead_birth;
+  F.mean = h->d_mean; F.chol = h->d_chol; F.ctl = h->d_ctl;
+  F.reset = reset; F.set_state = set_state; F.zero_evals = zero_evals; F.logX = logX; F.logZ = logZ;
+  k4_front<<<F.T + ((n + kRankElems - 1) / kRankElems) * F.nseg, kOneCta, 0, st>>>(F);
+  h->launches += 1;
+  if (n_repeats > 0 || dead_logw) {
+    k_directions<<<(k * n_repeats + 127) / 128 + 1, 128, 0, st>>>(d, h->d_chol, k, n_repeats, seed, iteration, h->d_flags, h->d_dirs, n,
+                                                                   dead_logL, dead_logw, h->d_state);
     h->launches += 1;
   }
-  NSS_CUDA(cudaStreamWaitEvent(st, h->ev_join, 0));
   NSS_CUDA(cudaGetLastError());
   ChainArgs A;
   A.live = live; A.logL = logL; A.birth = birth; A.n = n; A.k = k; A.n_repeats = n_repeats; A.seed = seed;
-  A.iteration = iteration; A.surv_idx = h->d_surv_idx; A.dead_idx = dead_idx; A.dirs = h->d_dirs; A.state = h->d_state;
-  A.flags = h->d_flags; A.n_evals = h->d_nevals; A.diag = &h->d_ctl->nrounds; A.trace = h->trace_dev; A.margin = h->margin_dev;
-  A.G = 1;
-  int rc;
+  A.iteration = iteration; A.surv_idx = h->d_surv_idx; A.dead_idx = dead_idx; A.dirs = h->d_dirs; A.ctl = h->d_ctl;
+  A.trace = h->trace_dev; A.margin = h->margin_dev; A.G = 1; A.live_evidence = live_evidence; A.stop_dlogz = stop_dlogz;
   switch (h->dev.n_det) {
-    case 0: case 1: rc = launch_chains<1>(h, A, st); break;
-    case 2: rc = launch_chains<2>(h, A, st); break;
-    case 3: rc = launch_chains<3>(h, A, st); break;
-    default: rc = launch_chains<4>(h, A, st); break;
+    case 0: case 1: return launch_chains<1>(h, A, st);
+    case 2: return launch_chains<2>(h, A, st);
+    case 3: return launch_chains<3>(h, A, st);
+    default: return launch_chains<4>(h, A, st);
   }
-  if (dead_logw) NSS_CUDA(cudaStreamWaitEvent(st, h->ev_evid, 0));     // whatever follows on st sees logX, logZ, logw
-  return rc;
 }
 
 }  // namespace
@@ -1045,9 +1280,10 @@ extern "C" int nss_select_lowest(nss_handle *h, const double *logL_dev, int32_t 
   if (rc) return rc;
   rc = begin_iteration(h, 0, 0.0, 0.0, 0, st);
   if (rc) return rc;
-  k4_rank<<<(n_live + kRankThreads - 1) / kRankThreads, kRankThreads, 0, st>>>(logL_dev, n_live, n_delete, h->d_rank, dead_idx_dev, nullptr);
-  k4_finish_select<<<1, kOneCta, 0, st>>>(nullptr, logL_dev, nullptr, n_live, n_delete, h->dev.d, NAN, h->d_rank, dead_idx_dev,
-                                          surv_idx_dev, nullptr, nullptr, nullptr, h->d_state, h->d_flags);
+  const int nseg = rank_segments(n_live);
+  k4_rank<<<((n_live + kRankElems - 1) / kRankElems) * nseg, kOneCta, 0, st>>>(logL_dev, n_live, nseg, h->d_rank_part);
+  k4_finish_select<<<1, kOneCta, 0, st>>>(logL_dev, n_live, n_delete, nseg, h->d_rank_part, h->d_rank, dead_idx_dev,
+                                          surv_idx_dev ? surv_idx_dev : h->d_surv_idx, h->d_state);
   h->launches += 2;
   NSS_CUDA(cudaGetLastError());
   rc = fetch_ctl(h, st);
@@ -1065,7 +1301,8 @@ extern "C" int nss_tune(nss_handle *h, const double *live_dev, int32_t n_live, d
   if (rc) return rc;
   rc = begin_iteration(h, 0, 0.0, 0.0, 0, st);
   if (rc) return rc;
-  k4_tune<<<1, kOneCta, 0, st>>>(live_dev, n_live, h->dev.d, mean_dev, chol_dev, h->d_flags);
+  const int T = tune_blocks_for(n_live);
+  k4_tune<<<T, kOneCta, 0, st>>>(live_dev, n_live, h->dev.d, T, h->d_tune_scratch, h->d_ctl, mean_dev, chol_dev);
   h->launches += 1;
   NSS_CUDA(cudaGetLastError());
   rc = fetch_ctl(h, st);
@@ -1083,7 +1320,7 @@ extern "C" int nss_evidence_update(nss_handle *h, const double *dead_logL_dev, i
   if (rc) return rc;
   rc = begin_iteration(h, 1, state_host[0], state_host[1], 0, st);
   if (rc) return rc;
-  k4_evidence<<<1, kOneCta, 0, st>>>(dead_logL_dev, n_live, n_delete, logw_dev, h->d_state, nullptr);
+  k4_evidence<<<1, kOneCta, 0, st>>>(dead_logL_dev, n_live, n_delete, logw_dev, h->d_state);
   h->launches += 1;
   NSS_CUDA(cudaGetLastError());
   rc = fetch_ctl(h, st);
@@ -1103,10 +1340,9 @@ extern "C" int nss_replace_step(nss_handle *h, double *live_dev, double *logL_de
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int rc = ensure_scratch(h, n_live);
   if (rc) return rc;
-  rc = begin_iteration(h, 0, 0.0, 0.0, 1, st);
-  if (rc) return rc;
   rc = enqueue_iteration(h, live_dev, logL_dev, nullptr, n_live, n_delete, logLstar, n_repeats, seed, iteration, dead_theta_dev,
-                         dead_logL_dev, nullptr, dead_idx_dev, nullptr, st);
+                         dead_logL_dev, nullptr, dead_idx_dev, nullptr, /*reset*/ 1, /*set_state*/ 0, 0.0, 0.0, /*zero_evals*/ 1,
+                         /*live_evidence*/ 0, 0.0, st);
   if (rc) return rc;
   rc = fetch_ctl(h, st);
   if (rc) return rc;
@@ -1142,14 +1378,10 @@ extern "C" int nss_iterate(nss_handle *h, double *live_dev, double *logL_dev, in
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int rc = ensure_scratch(h, n_live);
   if (rc) return rc;
-  rc = begin_iteration(h, 1, state_host->logX, state_host->logZ, 1, st);
-  if (rc) return rc;
   rc = enqueue_iteration(h, live_dev, logL_dev, nullptr, n_live, n_delete, NAN, n_repeats, seed, iteration, dead_theta_dev,
-                         dead_logL_dev, nullptr, dead_idx_dev, dead_logw_dev, st);
+                         dead_logL_dev, nullptr, dead_idx_dev, dead_logw_dev, /*reset*/ 1, /*set_state*/ 1, state_host->logX,
+                         state_host->logZ, /*zero_evals*/ 1, /*live_evidence*/ 1, stop_dlogz, st);
   if (rc) return rc;
-  k4_live_evidence<<<1, kOneCta, 0, st>>>(logL_dev, n_live, stop_dlogz, 1, h->d_state, h->d_flags);
-  h->launches += 1;
-  NSS_CUDA(cudaGetLastError());
   rc = fetch_ctl(h, st);
   if (rc) return rc;
   const NssCtl &c = *h->h_ctl;
@@ -1246,7 +1478,8 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
   double *live = (double *)(rb + o_live), *logL = (double *)(rb + o_logL), *dth = (double *)(rb + o_dth), *dl = (double *)(rb + o_dl),
          *db = (double *)(rb + o_db), *dw = (double *)(rb + o_dw), *derr = (double *)(rb + o_err);
   cudaEvent_t e0 = h->ev_run[0], e1 = h->ev_run[1];
-  auto cleanup = [&]() {};
+  // every exit, the error exits included, leaves the stream drained (an iteration may still be queued)
+  auto cleanup = [&]() { cudaStreamSynchronize(st); };
 #define RUN_CUDA(x)                                                           \
   do {                                                                        \
     cudaError_t e__ = (x);                                                    \
@@ -1263,12 +1496,14 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
   int t = 0;
   int64_t n_dead = 0;
   int result = NSS_OK;
-  // The loop runs one iteration ahead of the host: the stop test of iteration t (k4_live_evidence sets flags[2] on the
-  // device) is read from a pinned slot while iteration t and the stop test of t+1 are already queued.  Every kernel of
-  // an iteration returns at once when flags[2] is set, so the iteration queued past convergence changes nothing.
+  // The loop runs one iteration ahead of the host: the stop test of iteration t (the epilogue of its K3 sets flags[2] on
+  // the device) is read from a pinned slot while iteration t+1 is already queued.  Both kernels of an iteration return
+  // at once when flags[2] (or the Cholesky flag) is set, so an iteration queued past the end of the run changes nothing.
   auto stage = [&](int tt) -> int {
-    k4_live_evidence<<<1, kOneCta, 0, st>>>(logL, n, stop_dlogz, tt > 0, h->d_state, h->d_flags);
-    h->launches += 1;
+    if (tt == 0) {                                       // logZ_live of the initial live set (no stop test before iteration 0)
+      k4_live_evidence<<<1, kOneCta, 0, st>>>(logL, n, stop_dlogz, 0, h->d_state, h->d_flags);
+      h->launches += 1;
+    }
     NSS_CUDA(cudaMemcpyAsync(&h->h_ctl[tt & 1], h->d_ctl, sizeof(NssCtl), cudaMemcpyDeviceToHost, st));
     NSS_CUDA(cudaEventRecord(h->ev_ctl[tt & 1], st));
     return NSS_OK;
@@ -1279,7 +1514,7 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
     const bool room = n_dead + k + n <= cap, more = t < max_iter;
     if (room && more) {
       rc = enqueue_iteration(h, live, logL, h->d_birth, n, k, NAN, n_repeats, seed, (uint32_t)t, dth + (size_t)n_dead * d, dl + n_dead,
-                             db + n_dead, h->d_dead_idx, dw + n_dead, st);
+                             db + n_dead, h->d_dead_idx, dw + n_dead, /*reset*/ 0, 0, 0.0, 0.0, 0, /*live_evidence*/ 1, stop_dlogz, st);
       if (rc) { cleanup(); return rc; }
       rc = stage(t + 1);
       if (rc) { cleanup(); return rc; }
@@ -1295,10 +1530,12 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
   }
   if (result == NSS_OK || result == NSS_ENOTCONV) {
     // O14: append the live points in ascending logL
-    k4_rank<<<(n + kRankThreads - 1) / kRankThreads, kRankThreads, 0, st>>>(logL, n, n, h->d_rank, h->d_dead_idx, nullptr);
+    const int nseg = rank_segments(n);
+    k4_rank<<<((n + kRankElems - 1) / kRankElems) * nseg, kOneCta, 0, st>>>(logL, n, nseg, h->d_rank_part);
+    k4_finish_select<<<1, kOneCta, 0, st>>>(logL, n, n, nseg, h->d_rank_part, h->d_rank, h->d_dead_idx, nullptr, nullptr);
     k_gather_rows<<<(n + 255) / 256, 256, 0, st>>>(live, logL, h->d_birth, h->d_dead_idx, n, d, dth + (size_t)n_dead * d, dl + n_dead,
                                                    db + n_dead);
-    h->launches += 2;
+    h->launches += 3;
     const int64_t n_it_dead = n_dead;
     n_dead += n;
     double state[4];

@@ -148,17 +148,12 @@ extern "C" int nss_destroy(nss_handle *h)
   if (!h) return NSS_OK;
   cudaSetDevice(h->device);
   cudaFree(h->d_rec); cudaFree(h->d_soa[0]); cudaFree(h->d_soa[1]); cudaFree(h->d_soa[2]);
-  cudaFree(h->d_surv_idx); cudaFree(h->d_dead_idx); cudaFree(h->d_rank); cudaFree(h->d_ctl);
+  cudaFree(h->d_surv_idx); cudaFree(h->d_dead_idx); cudaFree(h->d_rank); cudaFree(h->d_rank_part); cudaFree(h->d_tune_scratch); cudaFree(h->d_ctl);
   if (h->h_ctl) cudaFreeHost(h->h_ctl);
   cudaFree(h->d_mean); cudaFree(h->d_chol); cudaFree(h->d_birth); cudaFree(h->d_stage);
   cudaFree(h->d_run); cudaFree(h->d_dirs);
-  if (h->st2) cudaStreamDestroy(h->st2);
-  if (h->ev_fork) cudaEventDestroy(h->ev_fork);
-  if (h->ev_join) cudaEventDestroy(h->ev_join);
-  if (h->ev_sel) cudaEventDestroy(h->ev_sel);
   if (h->ev_ctl[0]) cudaEventDestroy(h->ev_ctl[0]);
   if (h->ev_ctl[1]) cudaEventDestroy(h->ev_ctl[1]);
-  if (h->ev_evid) cudaEventDestroy(h->ev_evid);
   if (h->ev_run[0]) cudaEventDestroy(h->ev_run[0]);
   if (h->ev_run[1]) cudaEventDestroy(h->ev_run[1]);
   if (h->ev_k3[0]) cudaEventDestroy(h->ev_k3[0]);

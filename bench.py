@@ -15,8 +15,10 @@ value   = device-resident steps (CUDA events around each step on the launching s
 e2e     = the same through `nss_iterate_host` with pinned HOST buffers (H2D + D2H inside the call)
 roofline= the dominant kernel (K3 slice chains): fp64 flop of the likelihood evaluations it made /
           its own CUDA-event duration, against the DFMA peak measured in the same process
-extras  = K1 batch-likelihood microbenchmark (config 5, N = 1e6), a full `nss_run` to convergence,
-          the oracle timed on the host cores (cpu_baseline).
+extras  = a config-3 step (n_live 5000 / n_delete 2500) with its own K3 roofline object, K1 / K2 batch-likelihood
+          microbenchmarks (config 5, N = 1e6; config 4 likelihood), full `nss_run`s to convergence on configs 2, 3, 4
+          and on the paper's hyper-parameters (n_live 3000, n_delete 1500, 10 d repeats: PAPER.md:43), the oracle timed
+          on the host cores (cpu_baseline: NS iterations; oracle_legs: BASELINE.md section 2's other legs).
 
 `--impl reference` times the ORACLE (oracle/, plain C on the host cores) on a bounded sample of the same
 workload; it is the only other place this file executes oracle/ code.
@@ -36,6 +38,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "heterodyned logL evals/s (NSS iteration, config 2)"
+NOMINAL_TF = 148 * 64 * 2 * 1.965e9 / 1e12        # 148 SMs x 64 fp64 lanes x 2 flop x 1.965 GHz = 37.2 TFLOP/s
 UNIT = "evals/s"
 SEED = 1
 
@@ -53,6 +56,26 @@ def rb_work(B: int, n_det: int):
     instr = per_point_i + E * edge_i + E * n_det * ed_i
     flop = per_point_f + E * edge_f + E * n_det * ed_f
     return instr, flop
+
+
+K3_PROFILE = os.path.join(ROOT, "profiles", "r02_k3_slice_full.md")
+
+
+def profile_traffic():
+    """DRAM bytes per K3 launch, read from the tracked ncu --set full summary (NOT measured in this run: ncu cannot run
+    inside a timed bench).  The summary carries a line `dram_bytes_per_launch: <read + write bytes>` and its capture date."""
+    try:
+        txt = open(K3_PROFILE).read()
+        import re
+        m = re.search(r"dram_bytes_per_launch:\s*(\d+)", txt)
+        dt = re.search(r"captured:\s*(\S+)", txt)
+        if m:
+            return int(m.group(1)), (f"from the tracked profile {os.path.relpath(K3_PROFILE, ROOT)} (captured {dt.group(1) if dt else '?'}), "
+                                     "dram__bytes_read.sum + dram__bytes_write.sum of one launch; not measured in this run; "
+                                     "the kernel is ALU/latency-bound, the live set and tables stay in L2")
+    except OSError:
+        pass
+    return None, "no tracked ncu capture of this build"
 
 
 class ClockSampler:
@@ -126,6 +149,36 @@ def oracle_steps(w_oracle, steps, warmup, n_repeats, seed):
     return evals, secs, cores
 
 
+def oracle_legs(wo, cores, gpu_rb_rate, gpu_full_rate, gpu_run, whole_run):
+    """the oracle's batched likelihood on 1 core and on all cores (relative binning N = 1e4, full
+    grid N = 1e3) and its wall clock for one whole config-2 run, beside the GPU figures of this run."""
+    from oracle import nss_oracle as orc
+    from paper_2509_24949_b200 import inputs
+    legs = {}
+    X = inputs.draw_prior(wo, 10000, 5)
+    for name, prob, pts, gpu in (("loglike_batch_rb_N1e4", orc.Problem(wo), X, gpu_rb_rate),
+                                 ("loglike_batch_full_N1e3", orc.Problem(wo, kind=1), X[:1000], gpu_full_rate)):
+        leg = {"n_points": int(pts.shape[0]), "gpu_evals_per_s": gpu}
+        for label, nt in (("1_core", 1), (f"{cores}_cores", cores)):
+            t0 = time.perf_counter()
+            prob.loglike_batch(pts, nthreads=nt)
+            leg[label + "_evals_per_s"] = pts.shape[0] / (time.perf_counter() - t0)
+        leg["gpu_over_all_cores"] = gpu / leg[f"{cores}_cores_evals_per_s"]
+        legs[name] = leg
+    if whole_run:
+        p = orc.Problem(wo)
+        t0 = time.perf_counter()
+        o = p.run(wo.n_live, wo.n_delete, wo.n_repeats, SEED, nthreads=cores)
+        wall = time.perf_counter() - t0
+        legs["nss_run_config2"] = {"oracle_wall_s": wall, "cores": cores, "n_iter": o["n_iter"], "n_evals": o["n_evals"],
+                                   "logZ": o["logZ"], "logZ_err": o["logZ_err"], "gpu_wall_s": gpu_run["wall_s"],
+                                   "gpu_n_iter": gpu_run["n_iter"], "gpu_n_evals": gpu_run["n_evals"], "gpu_logZ": gpu_run["logZ"],
+                                   "gpu_over_oracle": wall / gpu_run["wall_s"],
+                                   "note": "same seed, same stop rule; the bench injection comes from the library's own waveform "
+                                           "routine and the oracle's from the oracle's, so the two data sets agree to rounding only"}
+    return legs
+
+
 def run_reference(args):
     """--impl reference: the oracle on the host cores, on a bounded sample of the same workload."""
     rank = int(os.environ.get("RANK", "0"))
@@ -136,10 +189,12 @@ def run_reference(args):
     orc.build()
     w = inputs.make_data(inputs.config2(), orc.waveform)
     n_rep = 5
+    w.n_repeats = n_rep                            # the line's config records what this arm ran
     evals, secs, cores = oracle_steps(w, args.steps, args.warmup, n_rep, SEED)
     v = evals / secs
     sample = (f"{args.steps} consecutive NS iterations of config 2 (n_live 1000, n_delete 500) with {n_rep} slice repeats "
-              f"per chain instead of 55 (evals/s is per evaluation), OpenMP over chains on {cores} cores")
+              f"per chain instead of 55 (a bounded sample: evals/s is per evaluation), OpenMP over chains on {cores} cores; "
+              "the oracle is an unoptimised checker (scalar loops, libm, an allocation per evaluation), not a tuned CPU code")
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -154,7 +209,7 @@ def run_reference(args):
 def config_dict(w):
     return {"workload": "BASELINE.json configs[1]: 11-param aligned-spin BBH, H1+L1+V1, TaylorF2 3.5PN + 1.5PN SO, "
                         "aLIGO-fit PSD, 20-1024 Hz df 0.25 (4017 bins), SNR-20 injection + seeded coloured noise, "
-                        "relative binning B=128/detector, n_live 1000, n_delete 500, 55 slice repeats",
+                        f"relative binning B=128/detector, n_live 1000, n_delete 500, {int(w.n_repeats)} slice repeats",
             "n_live": int(w.n_live), "n_delete": int(w.n_delete), "n_repeats": int(w.n_repeats), "n_bins": int(w.n_bins),
             "n_det": int(w.n_det), "d": int(w.d), "seed": SEED,
             "l2": "flushed (256 MiB write) between steps, outside the per-step event pairs; working set < 1 MB, ALU-bound"}
@@ -199,9 +254,49 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
 
-    def fresh(sd):
-        live, logL = g.nss_init_live(n, sd)
+    def fresh(sd, n_live=None):
+        live, logL = g.nss_init_live(n if n_live is None else n_live, sd)
         return live, logL, nss.nss_iter_state(logX=0.0, logZ=-math.inf), 0
+
+    def timed_steps(n_live, n_del, steps, warmup, sd, sync_all, kernel_timing=False):
+        """`steps` consecutive NS iterations (one nss_iterate call each) of a seeded run, CUDA events around each step on
+        the launching stream, L2 flushed between steps outside the event pairs; a fresh run starts, untimed, whenever the
+        stop rule fires.  kernel_timing: the library also records events around K3 (which costs the step ~5 us of launch
+        overlap, so the step time is taken from a pass without them and the kernel time from a second, identical pass)."""
+        g.set_chain_timing(kernel_timing)
+        live, logL, st, it = fresh(sd, n_live)
+        bufs = g.iter_buffers(n_del)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        r = dict(evals=0, k3_ms=0.0, rounds=0, executed=0, launches=0, wall=0.0, ms=0.0)
+        runs, l0, wall0 = 0, 0, None
+        if sync_all:
+            barrier()
+        for s_ in range(warmup + steps):
+            if s_ == warmup:
+                barrier() if sync_all else torch.cuda.synchronize()
+                wall0 = time.perf_counter()
+                l0 = g.launches
+            if st.converged:
+                runs += 1
+                live, logL, st, it = fresh(sd + 7919 * runs, n_live)
+            flush.fill_(s_ & 0xFF)
+            if s_ >= warmup:
+                ev[s_ - warmup][0].record(stream)
+            g.nss_iterate(live, logL, n_del, nrep, sd + 7919 * runs, it, st, bufs)
+            if s_ >= warmup:
+                ev[s_ - warmup][1].record(stream)
+                r["evals"] += st.n_evals
+                if kernel_timing:
+                    r["k3_ms"] += g.nss_last_chain_ms()
+                rd, ex = g.nss_last_chain_diag()
+                r["rounds"] += rd; r["executed"] += ex
+            it += 1
+        barrier() if sync_all else torch.cuda.synchronize()
+        r["wall"] = time.perf_counter() - wall0
+        r["launches"] = g.launches - l0
+        r["ms"] = sum(a.elapsed_time(b) for a, b in ev)
+        g.set_chain_timing(False)
+        return r
 
     def barrier():
         torch.cuda.synchronize()
@@ -213,36 +308,12 @@ def run_ours(args):
 
     with ClockSampler(local) as clocks:
         # ---- device-resident steps -----------------------------------------------------------------------
-        live, logL, st, it = fresh(seed)
-        bufs = g.iter_buffers(k)
-        runs = 0
-        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-        evals, k3_ms, launches0, rounds, executed = 0, 0.0, 0, 0, 0
-        barrier()
-        wall0 = None
-        for s in range(args.warmup + args.steps):
-            if s == args.warmup:
-                barrier()
-                wall0 = time.perf_counter()
-                launches0 = g.launches
-            if st.converged:
-                runs += 1
-                live, logL, st, it = fresh(seed + 7919 * runs)
-            flush.fill_(s & 0xFF)
-            if s >= args.warmup:
-                ev[s - args.warmup][0].record(stream)
-            g.nss_iterate(live, logL, k, nrep, seed + 7919 * runs, it, st, bufs)
-            if s >= args.warmup:
-                ev[s - args.warmup][1].record(stream)
-                evals += st.n_evals
-                k3_ms += g.nss_last_chain_ms()
-                rd, ex = g.nss_last_chain_diag()
-                rounds += rd; executed += ex
-            it += 1
-        barrier()
-        wall = time.perf_counter() - wall0
-        launches = g.launches - launches0
-        ms = sum(a.elapsed_time(b) for a, b in ev)
+        m2 = timed_steps(n, k, args.steps, args.warmup, seed, True)
+        m2k = timed_steps(n, k, args.steps, args.warmup, seed, True, kernel_timing=True)     # the same steps, K3 timed
+        assert m2k["evals"] == m2["evals"], "the two passes must make the same evaluations"
+        evals, k3_ms, rounds, executed = m2["evals"], m2k["k3_ms"], m2["rounds"], m2["executed"]
+        wall, launches, ms = m2["wall"], m2["launches"], m2["ms"]
+        ms_with_kernel_events = m2k["ms"]
 
         # ---- end to end: pinned host buffers through nss_iterate_host ----------------------------------------
         live_d, logL_d, st_h, it_h = fresh(seed + 1)
@@ -252,16 +323,18 @@ def run_ours(args):
         hb = g.iter_buffers(k, host=True)
         e2e_steps = args.steps
         evals_h, t_h = 0, 0.0
+        seed_h = seed + 1
         barrier()
         for s in range(args.warmup + e2e_steps):
             if st_h.converged:
-                live_d, logL_d, st_h, it_h = fresh(seed + 1 + 104729 * (s + 1))
+                seed_h = seed + 1 + 104729 * (s + 1)     # a new run: new initial points AND new chain streams
+                live_d, logL_d, st_h, it_h = fresh(seed_h)
                 live_h.copy_(live_d); logL_h.copy_(logL_d)
                 torch.cuda.synchronize()
             flush.fill_(s & 0xFF)
             torch.cuda.synchronize()
             t0 = time.perf_counter()
-            g.nss_iterate(live_h, logL_h, k, nrep, seed + 1, it_h, st_h, hb, host=True)   # synchronous
+            g.nss_iterate(live_h, logL_h, k, nrep, seed_h, it_h, st_h, hb, host=True)   # synchronous
             dt = time.perf_counter() - t0
             if s >= args.warmup:
                 evals_h += st_h.n_evals
@@ -270,6 +343,13 @@ def run_ours(args):
         barrier()
         h2d = n * d * 8 + n * 8
         d2h = n * d * 8 + n * 8 + k * d * 8 + k * 8 + k * 8 + k * 4
+
+        # ---- config 3 (BASELINE.json configs[2]): the same step at n_live 5000 / n_delete 2500 (rank 0 only) ------------
+        m3 = None
+        if rank == 0 and not args.no_extras:
+            m3 = timed_steps(5000, 2500, max(4, args.steps // 2), 3, seed, False)
+            m3["k3_ms"] = timed_steps(5000, 2500, max(4, args.steps // 2), 3, seed, False, kernel_timing=True)["k3_ms"]
+            m3["steps"] = max(4, args.steps // 2)
 
         # ---- K1 microbenchmark (config 5): N = 1e6 prior draws, B = 128 x 3 detectors --------------------------
         N1 = 1_000_000
@@ -308,11 +388,29 @@ def run_ours(args):
         k2_ms = sorted(k2)[len(k2) // 2]
         g2.close()
 
-        # ---- full run to convergence ------------------------------------------------------------------------
-        g.nss_run(n, k, nrep, seed)                         # warm
-        t0 = time.perf_counter()
-        r = g.nss_run(n, k, nrep, seed)
-        run_wall = time.perf_counter() - t0
+        # ---- full runs to convergence -----------------------------------------------------------------------
+        def timed_run(gg, n_live, n_del, n_rep, sd, max_iter=10000):
+            gg.nss_run(n_live, n_del, n_rep, sd, max_iter=max_iter)       # warm (allocations of the handle)
+            t0 = time.perf_counter()
+            rr = gg.nss_run(n_live, n_del, n_rep, sd, max_iter=max_iter)
+            wall_s = time.perf_counter() - t0
+            return {"wall_s": wall_s, "gpu_ms": rr["gpu_ms"], "n_iter": rr["n_iter"], "n_evals": rr["n_evals"],
+                    "evals_per_s": rr["n_evals"] / wall_s, "logZ": rr["logZ"], "logZ_err": rr["logZ_err"], "H": rr["H"],
+                    "rc": rr["rc"], "kish_ess": rr["ess"], "ess_per_s": rr["ess"] / wall_s, "n_equal": rr["n_equal"],
+                    "n_live": n_live, "n_delete": n_del, "n_repeats": n_rep}
+
+        run2 = timed_run(g, n, k, nrep, seed)
+        run_wall, r = run2["wall_s"], run2
+        runs_extra = {}
+        if rank == 0 and not args.no_extras:
+            runs_extra["config3"] = timed_run(g, 5000, 2500, nrep, seed)
+            # the paper's hyper-parameters on the synthetic config-2 problem (3000 live points, half of
+            # them deleted per iteration, chains of 10 d steps); its 207 s / ESS 17490 is IMRPhenomD on
+            # GW150914 on an A100: context only
+            runs_extra["paper_hyperparameters"] = timed_run(g, 3000, 1500, 10 * d, seed)
+            g4 = nss.Nss(w, kind=1)
+            runs_extra["config4"] = timed_run(g4, n, k, nrep, seed)
+            g4.close()
 
     # max over ranks of the timed quantities; sum of the work
     if dist:
@@ -324,6 +422,7 @@ def run_ours(args):
         return 0
 
     instr, flop = rb_work(w.n_bins, w.n_det)
+    traffic, traffic_note = profile_traffic()
     value = evals / (ms * 1e-3)
     k3_tf = (evals / world) * flop / (k3_ms * 1e-3) / 1e12
     k1_rate = N1 / (k1_ms * 1e-3)
@@ -338,31 +437,47 @@ def run_ours(args):
         "wall_ms_timed_region": 1e3 * wall,
         "roofline": {"bound": "alu", "kernel": "k3_slice (one slice chain per CTA, likelihood inlined)",
                      "achieved": k3_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": k3_tf / peak_tf,
+                     "frac_of_nominal": k3_tf / NOMINAL_TF, "peak_nominal": NOMINAL_TF,
                      "peak_source": "fp64 DFMA chain measured in this process (nss_fp64_peak); nominal 148 SM x 64 lanes x 2 x "
                                     "1.965 GHz = 37.2; MEASURED_PEAKS.json has no fp64 figure",
                      "flop_per_eval": flop, "fp64_instr_per_eval": instr,
                      "pipe_frac": (evals / world) * instr / (k3_ms * 1e-3) / (peak_tf * 1e12 / 2),
-                     "kernel_ms_per_step": k3_ms / args.steps, "kernel_share_of_step": k3_ms / ms,
-                     "traffic": 2560256,
-                     "traffic_note": "bytes per launch, dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full "
-                                     "capture (profiles/r01e_k3_slice_full.md): the slice directions; the kernel is not memory-bound",
+                     "kernel_ms_per_step": k3_ms / args.steps, "kernel_share_of_step": k3_ms / ms_with_kernel_events,
+                     "kernel_timing": "CUDA events recorded by the library around K3 on the launching stream, in a second pass over "
+                                      "the same seeded steps (an event in front of K3 costs the launch overlap, so `ms_per_step` "
+                                      "comes from the pass without them)",
+                     "ms_per_step_with_kernel_events": ms_with_kernel_events / args.steps,
+                     "traffic": traffic, "traffic_note": traffic_note,
                      "rounds_per_chain": rounds / args.steps / k / world, "evaluated_incl_speculative_per_step": executed / args.steps / world,
                      "note": "achieved counts only the evaluations the sequential algorithm consumed"},
         "loglike_batch": {"workload": "config 5: N=1e6 prior draws, B=128 x 3 detectors, k_rec_thread", "ms": k1_ms,
                           "evals_per_s": k1_rate, "tflops": k1_rate * flop / 1e12, "frac": k1_rate * flop / 1e12 / peak_tf,
+                          "frac_of_nominal": k1_rate * flop / 1e12 / NOMINAL_TF,
                           "pipe_frac": k1_rate * instr / (peak_tf * 1e12 / 2)},
         "loglike_batch_full": {"workload": "config 4 likelihood: full grid 4017 bins x 3 detectors, N=1e5 prior draws, k_rec_sub<FULL>",
                                "ms": k2_ms, "evals_per_s": N2 / (k2_ms * 1e-3),
                                "fp64_instr_per_eval": 600 + w.n_freq * (8 + 22 * w.n_det),
                                "pipe_frac": N2 / (k2_ms * 1e-3) * (600 + w.n_freq * (8 + 22 * w.n_det)) / (peak_tf * 1e12 / 2),
+                               "pipe_frac_of_nominal": N2 / (k2_ms * 1e-3) * (600 + w.n_freq * (8 + 22 * w.n_det)) / (NOMINAL_TF * 1e12 / 2),
                                "algorithmic_hbm_bytes_per_eval": 96,
                                "note": "the 484 KB record table is shared by every point and stays in L2; HBM GB/s is reported by "
                                        "profiles/r01e_k2_full_grid_full.md"},
-        "nss_run": {"wall_s": run_wall, "gpu_ms": r["gpu_ms"], "n_iter": r["n_iter"], "n_evals": r["n_evals"],
-                    "logZ": r["logZ"], "logZ_err": r["logZ_err"], "H": r["H"], "rc": r["rc"],
-                    "kish_ess": r["ess"], "ess_per_s": r["ess"] / run_wall},
+        "nss_run": run2,
         "clocks": clocks.summary(),
     }
+    for key_, v_ in runs_extra.items():
+        line["nss_run_" + key_] = v_
+    if m3 is not None:
+        k3_tf3 = m3["evals"] * flop / (m3["k3_ms"] * 1e-3) / 1e12
+        line["step_config3"] = {
+            "workload": "BASELINE.json configs[2]: config 2 at n_live 5000, n_delete 2500 (55 repeats)", "steps": m3["steps"],
+            "ms_per_step": m3["ms"] / m3["steps"], "evals_per_s": m3["evals"] / (m3["ms"] * 1e-3),
+            "evals_per_step": m3["evals"] / m3["steps"], "gpu_launches": m3["launches"],
+            "roofline": {"bound": "alu", "kernel": "k3_slice (single-warp chains, 8 lanes per candidate)", "achieved": k3_tf3,
+                         "peak": peak_tf, "unit": "TFLOP/s", "frac": k3_tf3 / peak_tf, "frac_of_nominal": k3_tf3 / NOMINAL_TF,
+                         "kernel_ms_per_step": m3["k3_ms"] / m3["steps"], "kernel_share_of_step": m3["k3_ms"] / m3["ms"],
+                         "rounds_per_chain": m3["rounds"] / m3["steps"] / 2500,
+                         "evaluated_incl_speculative_per_step": m3["executed"] / m3["steps"]}}
     # ---- CPU baseline: the oracle as it stands, on this box's host cores, bounded sample -----------------------
     if world == 1 and not args.no_cpu_baseline:
         from oracle import nss_oracle as orc
@@ -372,7 +487,10 @@ def run_ours(args):
         ev_o, s_o, cores = oracle_steps(wo, n_it, 0, w.n_repeats, SEED)
         line["cpu_baseline"] = {"value": ev_o / s_o, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"NS iterations 0..{n_it - 1} of the same config-2 run (n_live 1000, n_delete 500, "
-                                          f"55 repeats): {ev_o} evaluations in {s_o:.1f} s, OpenMP over chains"}
+                                          f"55 repeats): {ev_o} evaluations in {s_o:.1f} s, OpenMP over chains",
+                                "note": "the oracle is an unoptimised checker (scalar loops, libm, an allocation per evaluation): "
+                                        "a reported baseline, not a tuned CPU implementation"}
+        line["oracle_legs"] = oracle_legs(wo, cores, k1_rate, N2 / (k2_ms * 1e-3), run2, not args.no_oracle_run)
     print(json.dumps(line))
     g.close()
     if dist:
@@ -387,6 +505,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the config-3/4 and paper-hyper-parameter extras")
+    ap.add_argument("--no-oracle-run", action="store_true", help="skip the oracle's whole config-2 run (the longest CPU leg)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

@@ -114,6 +114,11 @@ int nss_last_chain_diag(nss_handle *h, int64_t *rounds_host, int64_t *evaluated_
  * whose table was not built, e.g. 8 lanes with more than 256 bins, falls back to the automatic choice). */
 int nss_set_chain_lanes(nss_handle *h, int32_t lanes);
 
+/* Single-warp chains (nss_set_chain_warps 1, or the automatic choice for many chains) packed per CTA of K3: the warps of
+ * a CTA share one shared-memory copy of the record table and take chains from a device counter as they finish.
+ * 0 = automatic, else 1 .. 8.  Like the two setters above it changes the schedule only, never a result. */
+int nss_set_chain_pack(nss_handle *h, int32_t chains_per_cta);
+
 /* One NS iteration (O12): select the n_delete lowest logL (ascending, ties by lower slot), tune the
  * slice directions from the covariance of the full live set (Cholesky), run one chain per deleted
  * point (start = uniformly chosen survivor; n_repeats x {direction, stepping-out, shrinkage} under
@@ -188,6 +193,14 @@ int nss_init_live(nss_handle *h, int32_t n_live, uint64_t seed, double *live_dev
 int nss_philox(nss_handle *h, uint64_t seed, const uint32_t *ctr_dev, int64_t n, uint32_t *out_dev,
                void *cuda_stream);
 
+/* NEXT-4, reading R6: equal-weight posterior samples.  PAPER.md:59-63 quotes the number of "equal weight
+ * samples" in brackets beside the Kish ESS and does not define them.  Reading: row i (weight p_i ~ exp(logL_i + logw_i))
+ * is kept iff u_i < p_i / max_j p_j, u_i the [0, 1) uniform of Philox counter (0, i mod 2^32, i div 2^32, 0xFFFFFFFD)
+ * under key `seed`; rows with logL + logw = -inf are never kept.  logL_dev, logw_dev: device [n]; idx_dev: device [n] or
+ * NULL, receives the kept row indices in ascending order; *n_equal_host = their number.  Synchronous. */
+int nss_resample_equal(nss_handle *h, const double *logL_dev, const double *logw_dev, int64_t n, uint64_t seed,
+                       int64_t *idx_dev, int64_t *n_equal_host, void *cuda_stream);
+
 typedef struct {
   double  logZ, logZ_err, H;       /* evidence, its replica s.d. (O15), information             */
   int32_t n_iter;
@@ -200,6 +213,8 @@ typedef struct {
   double  gpu_ms;                  /* device time of the run (CUDA events), setup excluded       */
   double  ess;                     /* Kish effective sample size (sum p)^2 / sum p^2 of the posterior weights
                                       p_i ~ exp(logL_i + logw_i) over all rows (O15; the paper's Table 1b metric) */
+  int64_t n_equal;                 /* equal-weight posterior rows (reading R6; the bracketed count of PAPER.md:59-63) */
+  int64_t *equal_idx;              /* host [cap] or NULL: if given, receives the n_equal kept row indices, ascending  */
 } nss_result;
 
 /* Full run (O13, O14): initial live points, NS iterations until logZ_live - logZ < stop_dlogz
@@ -207,7 +222,8 @@ typedef struct {
  * Everything stays on the device; results are copied to the caller's host arrays at the end.  The host queues one
  * iteration ahead: the stop test sets a device flag, the kernels of an iteration queued past it return at once, and the
  * flag reaches the host through a pinned slot ("the entire end-to-end algorithm can then run in GPU memory").
- * logZ_err (200 stochastic-compression replicas, O15) and ess are reduced on the device.  Returns NSS_OK, NSS_ENOTCONV
+ * logZ_err (200 stochastic-compression replicas, O15), ess and n_equal (the rows nss_resample_equal keeps, same seed) are
+ * reduced on the device.  Returns NSS_OK, NSS_ENOTCONV
  * (max_iter reached, results valid), NSS_ECAP (out->cap too small: needs n_iter * n_delete + n_live rows), NSS_ECHOL,
  * NSS_EINVAL, NSS_ENOMEM or NSS_ECUDA.  Synchronous: returns after the stream has drained. */
 int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t n_repeats, uint64_t seed,
@@ -227,8 +243,10 @@ int nss_get_tables(nss_handle *h, int32_t *edge_idx_host, double *summary_host, 
 int nss_fp64_peak(double ms, double *tflops_host, void *cuda_stream);
 
 /* Device time [ms] of the most recent K3 (slice-sampling chains) launch, from CUDA events the library
- * records around it on the caller's stream (bench.py's roofline for the dominant kernel).
- * NSS_EINVAL before the first iteration. */
+ * records around it on the caller's stream (bench.py's roofline for the dominant kernel), if
+ * nss_set_chain_timing(h, 1) was called before that launch; NSS_EINVAL otherwise.  Off by default: the event in
+ * front of K3 keeps its prologue from overlapping the kernel before it (programmatic dependent launch). */
+int nss_set_chain_timing(nss_handle *h, int32_t on);
 int nss_last_chain_ms(nss_handle *h, double *ms_host);
 
 /* Kernel launches issued by this handle since creation (bench.py's gpu_launches). */

@@ -51,6 +51,7 @@ struct NssCtl {
   int32_t sel_bad;             // a survivor below a supplied threshold (selection tail -> flags[1])
   uint32_t tune_cnt[2];        // counters of the tuning blocks of k4_front: column sums published, products published
   uint32_t chains_done;        // chains finished (the CTA that finishes the last one runs the live-evidence epilogue)
+  uint32_t chain_next;         // next chain to start (K3 with single-warp groups: warps fetch chains as they finish)
   int32_t chol_now;            // Cholesky status of the tuning block of the iteration being set up
 };
 
@@ -61,6 +62,7 @@ struct nss_handle {
   int loglike_variant;
   int chain_warps;          // warps per slice chain: 0 = automatic, else 1, 2, 4 or 8
   int chain_lanes;          // lanes per candidate in the slice kernel: 0 = automatic, else 8, 16 or 32
+  int chain_pack;           // single-warp chains per CTA (they share the record table): 0 = automatic, else 1 .. 8
   int64_t launches;
   // host copies kept for nss_get_tables
   std::vector<int32_t> edge_idx;
@@ -77,8 +79,6 @@ struct nss_handle {
   NssCtl *d_ctl, *h_ctl;       // d_state, d_nevals, d_flags point into d_ctl; h_ctl is pinned, two slots
   cudaEvent_t ev_ctl[2];       // nss_run: the copy into slot i has landed
   double *d_birth;
-  double *d_dirs;              // [k][n_repeats][d] slice directions of the current iteration
-  size_t dirs_bytes;
   int32_t *trace_dev;
   double *margin_dev;
   // device staging for the host-buffer entry points (grown on demand)
@@ -91,6 +91,7 @@ struct nss_handle {
   // CUDA events recorded around the most recent K3 (slice chains) launch: nss_last_chain_ms
   cudaEvent_t ev_k3[2];
   int ev_k3_valid;
+  int chain_timing;            // record the event pair around K3 (nss_set_chain_timing); off by default
 };
 
 extern thread_local char g_nss_cuda_err[256];

@@ -1,4 +1,4 @@
-// nss_sampler.cu — K3 slice-sampling chains (one chain per CTA), k_directions, K4 on-device NS bookkeeping, and the host
+// nss_sampler.cu — K3 slice-sampling chains (slice directions included), K4 on-device NS bookkeeping, and the host
 // driver behind nss_replace_step / nss_run (O11-O15).
 #include <math.h>
 #include <string.h>
@@ -230,7 +230,9 @@ __device__ __forceinline__ double block_sum(double v, double *red)
 // factors the matrix: *chol_fail = 1 if a pivot is <= 0 (reading R5: no relative epsilon), else 0.
 constexpr int kTuneMaxBlocks = 32;
 constexpr int kTunePartDoubles = NSS_NSLOT + NSS_NSLOT * (NSS_NSLOT + 1) / 2;     // per block: column sums, then products
-__host__ __device__ inline int tune_blocks_for(int n) { const int t = n / 128; return t < 1 ? 1 : t > kTuneMaxBlocks ? kTuneMaxBlocks : t; }
+// One block up to 8192 live points (a few rows per thread; no barrier between blocks on the critical path of the iteration),
+// then one more block per 4096 rows.
+__host__ __device__ inline int tune_blocks_for(int n) { const int t = n / 4096; return t < 2 ? 1 : t > kTuneMaxBlocks ? kTuneMaxBlocks : t; }
 
 __device__ __forceinline__ void tune_block(const double *__restrict__ live, int n, int d, int b, int T, double *__restrict__ scratch,
                                            uint32_t *__restrict__ counters /*[2]*/, double *__restrict__ mean_out,
@@ -364,11 +366,10 @@ __device__ __forceinline__ double logaddexp_d(double a, double b)
 
 // K4.4 (O12.2): log-weights of the dead points, logX shrinkage, logZ accumulation; one block of any size (multiple of 32)
 __device__ __forceinline__ void evidence_block(const double *__restrict__ dead_logL, int n, int k, double *__restrict__ logw,
-                                               double *__restrict__ state, K4Smem &sm)
+                                               double logX0, double logZ0, double *__restrict__ state, K4Smem &sm)
 {
   double *red = sm.red.red, *warp_tot = sm.red.warp_tot;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  const double logX0 = state[0], logZ0 = state[1];
   const int nt = blockDim.x, chunk = (k + nt - 1) / nt;
   const int j0 = min(k, tid * chunk), j1 = min(k, j0 + chunk);
   double part = 0.0;
@@ -445,7 +446,9 @@ __global__ void __launch_bounds__(kOneCta) k4_evidence(const double *__restrict_
                                                        double *__restrict__ state)
 {
   __shared__ K4Smem sm;
-  evidence_block(dead_logL, n, k, logw, state, sm);
+  const double logX0 = state[0], logZ0 = state[1];
+  __syncthreads();
+  evidence_block(dead_logL, n, k, logw, logX0, logZ0, state, sm);
 }
 
 // ---- K4.5 (O14): live evidence and stop test ------------------------------------------------------------------
@@ -469,8 +472,9 @@ __global__ void __launch_bounds__(kOneCta) k4_live_evidence(const double *__rest
 
 // ---- the front of an NS iteration in ONE launch ---------------------------------------------------------------------
 // blocks 0 .. T-1 tune (a3: mean, covariance, Cholesky), the others rank the live points (a1) beside them; the rank block
-// that finishes last adds the partial ranks, compacts the survivors, gathers the dead rows and fixes the threshold (a1); the
-// block that finishes last of all publishes the flags and resets the counters.  `reset` = a stand-alone iteration (nss_iterate, nss_replace_step): flags and,
+// that finishes last adds the partial ranks, compacts the survivors, gathers the dead rows, fixes the threshold (a1) and
+// does the evidence bookkeeping of the deleted batch (a2: it needs only the dead logL it has just gathered); the block
+// that finishes last of all publishes the flags and resets the counters.  `reset` = a stand-alone iteration (nss_iterate, nss_replace_step): flags and,
 // on request, state and counters are re-initialised; otherwise (nss_run's loop, queued one iteration ahead of the host) an
 // iteration queued after convergence or after a Cholesky failure does nothing.
 struct FrontArgs {
@@ -479,6 +483,7 @@ struct FrontArgs {
   double Lstar_in;
   int32_t *rank_part, *rank, *dead_idx, *surv_idx;
   double *dead_theta, *dead_logL, *dead_birth;
+  double *dead_logw;            // not NULL: the evidence bookkeeping of the deleted batch (a2) follows the selection
   double *tune_scratch, *mean, *chol;
   NssCtl *ctl;
   int32_t reset, set_state, zero_evals;
@@ -488,6 +493,9 @@ struct FrontArgs {
 __global__ void __launch_bounds__(kOneCta) k4_front(const FrontArgs A)
 {
   __shared__ K4Smem sm;
+  // K3 is launched with programmatic stream serialization: let its CTAs start their prologue (table staging, constants)
+  // on the SMs this small grid leaves free; they wait (griddepcontrol.wait) for this grid to finish before reading anything
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   NssCtl *ctl = A.ctl;
   if (!A.reset && (ctl->flags[2] | ctl->flags[0])) return;
   const int b = blockIdx.x;
@@ -506,6 +514,12 @@ __global__ void __launch_bounds__(kOneCta) k4_front(const FrontArgs A)
       const int bad = finish_select_block(A.live, A.logL, A.birth, A.n, A.k, A.d, A.Lstar_in, A.rank, A.dead_idx, A.surv_idx, A.dead_theta,
                                           A.dead_logL, A.dead_birth, ctl->state, sm);
       if (threadIdx.x == 0) ctl->sel_bad = bad;
+      // a2 (O12.2).  A stand-alone iteration takes logX, logZ from the arguments, nss_run's loop from the control block.
+      const double logX0 = (A.reset && A.set_state) ? A.logX : ctl->state[0], logZ0 = (A.reset && A.set_state) ? A.logZ : ctl->state[1];
+      __syncthreads();
+      if (A.dead_logw) evidence_block(A.dead_logL, A.n, A.k, A.dead_logw, logX0, logZ0, ctl->state, sm);
+      else if (threadIdx.x == 0 && A.reset && A.set_state) { ctl->state[0] = logX0; ctl->state[1] = logZ0; }
+      if (threadIdx.x == 0 && A.reset && A.set_state) ctl->state[2] = 0.0;
     }
   }
   // the block that finishes last of all publishes the flags and resets the counters
@@ -515,12 +529,11 @@ __global__ void __launch_bounds__(kOneCta) k4_front(const FrontArgs A)
   __syncthreads();
   if (sm.ticket != gridDim.x - 1 || threadIdx.x != 0) return;
   __threadfence();
-  ctl->front_done = 0; ctl->rank_done = 0; ctl->chains_done = 0; ctl->tune_cnt[0] = 0; ctl->tune_cnt[1] = 0;
+  ctl->front_done = 0; ctl->rank_done = 0; ctl->chains_done = 0; ctl->chain_next = 0; ctl->tune_cnt[0] = 0; ctl->tune_cnt[1] = 0;
   const int chol_fail = *(volatile int32_t *)&ctl->chol_now;
   ctl->flags[1] = *(volatile int32_t *)&ctl->sel_bad;
   if (A.reset) {
     ctl->flags[0] = chol_fail; ctl->flags[2] = 0; ctl->flags[3] = 0;
-    if (A.set_state) { ctl->state[0] = A.logX; ctl->state[1] = A.logZ; ctl->state[2] = 0.0; }
     if (A.zero_evals) { ctl->nevals = 0ull; ctl->nrounds = 0ull; ctl->nexec = 0ull; }
   } else if (chol_fail) ctl->flags[0] = 1;
 }
@@ -613,6 +626,59 @@ __global__ void __launch_bounds__(kOneCta) k_kish_ess(const double *__restrict__
   if (threadIdx.x == 0) out[0] = s2 > 0.0 ? s1 * s1 / s2 : 0.0;
 }
 
+// ---- NEXT-4 / reading R6: equal-weight posterior samples, one CTA --------------------------------------------------
+// Row i (posterior weight p_i ~ exp(logL_i + logw_i)) is kept iff u_i < p_i / max_j p_j, with u_i the [0, 1) uniform of
+// Philox counter (0, i mod 2^32, i div 2^32, 0xFFFFFFFD): an equally weighted sample of the posterior whose expected size
+// is sum p / max p (PAPER.md:59-63 quotes such a count in brackets beside the Kish ESS and does not define it).
+// out[0] = number kept (as a double: exact below 2^53); idx_out (optional) = the kept rows in ascending order.
+constexpr uint32_t kIterEqual = 0xFFFFFFFDu;
+__global__ void __launch_bounds__(kOneCta) k_resample_equal(const double *__restrict__ logL, const double *__restrict__ logw,
+                                                            long long n, uint64_t seed, long long *__restrict__ idx_out,
+                                                            double *__restrict__ out)
+{
+  __shared__ double red[32];
+  __shared__ long long wtot[32];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  double mx = -INFINITY;
+  for (long long i = tid; i < n; i += kOneCta) mx = fmax(mx, logL[i] + logw[i]);
+  mx = block_max(mx, red);
+  const long long chunk = (n + kOneCta - 1) / kOneCta;
+  const long long i0 = min(n, (long long)tid * chunk), i1 = min(n, i0 + chunk);
+  auto keep = [&](long long i) {
+    const double a = logL[i] + logw[i];
+    if (!(a > -INFINITY)) return false;
+    return uniform_a(seed, 0u, (uint32_t)(i & 0xFFFFFFFFll), (uint32_t)(i >> 32), kIterEqual) < exp(a - mx);
+  };
+  long long cnt = 0;
+  if (mx > -INFINITY)
+    for (long long i = i0; i < i1; ++i) cnt += keep(i) ? 1 : 0;
+  long long incl = cnt;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const long long v = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += v;
+  }
+  __syncthreads();
+  if (lane == 31) wtot[wid] = incl;
+  __syncthreads();
+  long long pos = incl - cnt, total = 0;
+  for (int q = 0; q < kOneCta / 32; ++q) {
+    if (q < wid) pos += wtot[q];
+    total += wtot[q];
+  }
+  if (idx_out && mx > -INFINITY)
+    for (long long i = i0; i < i1; ++i)
+      if (keep(i)) idx_out[pos++] = i;
+  if (tid == 0) out[0] = (double)total;
+}
+
+// logw of the final live points, logX - ln n (O14), written on the device so that host and device rows are the same bits
+__global__ void k_fill_live_logw(double *__restrict__ p, int n, const double *__restrict__ state)
+{
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) p[i] = state[0] - log((double)n);
+}
+
 __global__ void k_fill(double *__restrict__ p, int n, double v)
 {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -631,34 +697,18 @@ __global__ void k_gather_rows(const double *__restrict__ live, const double *__r
   for (int a = 0; a < d; ++a) out_theta[(size_t)j * d + a] = live[(size_t)slot * d + a];
 }
 
-// ---- a5: slice directions of every (chain, step), one thread each ------------------------------------------------
+// ---- a5: the slice direction of one (chain, step) by one thread ---------------------------------------------------
 // z ~ N(0, I_d) by Box-Muller (one Philox block per pair: counter (1 + pair, step, chain, iteration)),
-// n = z/|z|, v = w L n with L the Cholesky factor of the live-point covariance (O12.4a).
-// The last block of the grid does not draw directions: it runs the evidence bookkeeping of the deleted batch (a2, O12.2:
-// it needs only the dead logL that k4_front has gathered), beside the direction blocks and off the critical path.
-__global__ void __launch_bounds__(128) k_directions(int d, const double *__restrict__ chol, int k, int n_repeats, uint64_t seed,
-                                                    uint32_t it, const int32_t *__restrict__ flags, double *__restrict__ dirs,
-                                                    int n, const double *__restrict__ dead_logL, double *__restrict__ dead_logw,
-                                                    double *__restrict__ state)
+// n = z/|z|, v = w L n with L the Cholesky factor of the live-point covariance (O12.4a); sL and out in shared memory.
+__device__ __forceinline__ void draw_direction(int d, const double *__restrict__ sL, uint64_t seed, uint32_t it, uint32_t ch, uint32_t s,
+                                               double *__restrict__ out)
 {
-  __shared__ double sL[NSS_NSLOT * NSS_NSLOT];
-  if (flags[0] | flags[1] | flags[2]) return;            // Cholesky failure, threshold violation, or converged
-  if (blockIdx.x == gridDim.x - 1) {
-    __shared__ K4Smem sm;
-    if (dead_logw) evidence_block(dead_logL, n, k, dead_logw, state, sm);
-    return;
-  }
-  for (int t = threadIdx.x; t < d * d; t += blockDim.x) sL[t] = chol[t];
-  __syncthreads();
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= k * n_repeats) return;
-  const int ch = idx / n_repeats, s = idx - ch * n_repeats;
   double z[NSS_NSLOT + 1];
 #pragma unroll
   for (int b = 0; b < (NSS_NSLOT + 1) / 2; ++b)
     if (2 * b < d) {
       uint64_t ka, kb;
-      draw53(seed, (uint32_t)(1 + b), (uint32_t)s, (uint32_t)ch, it, ka, kb);
+      draw53(seed, (uint32_t)(1 + b), s, ch, it, ka, kb);
       const double r = sqrt(-2.0 * log((double)(ka + 1) * kTwoM53));
       double sn, cs;
       sincospi(2.0 * ((double)kb * kTwoM53), &sn, &cs);
@@ -673,7 +723,6 @@ __global__ void __launch_bounds__(128) k_directions(int d, const double *__restr
 #pragma unroll
   for (int j = 0; j < NSS_NSLOT; ++j)
     if (j < d) z[j] = z[j] / nz;
-  double *out = dirs + (size_t)idx * d;
 #pragma unroll
   for (int i = 0; i < NSS_NSLOT; ++i)
     if (i < d) {
@@ -716,7 +765,7 @@ struct ChainArgs {
   uint64_t seed;
   uint32_t iteration;
   const int32_t *surv_idx, *dead_idx;
-  const double *dirs;           // [k][n_repeats][d] slice directions v = w L z/|z| (k_directions)
+  const double *chol;           // [d][d] lower Cholesky factor of the live-point covariance (k4_front)
   NssCtl *ctl;                  // state[3] = L*; flags (any set -> do nothing); evaluation counters; chains_done
   int32_t *trace;               // optional [k][n_repeats][3]
   double *margin;               // optional [k]
@@ -726,6 +775,7 @@ struct ChainArgs {
 };
 
 constexpr int kChainWarps = 8;          // largest group; a CTA is ONE group (G warps), one chain at a time
+constexpr int kDirChunk = 32;           // slice directions drawn at a time by a group (one lane of its first warp each)
 constexpr int kChainThreads = kChainWarps * 32;
 
 __device__ __forceinline__ void group_sync(int G)
@@ -733,8 +783,13 @@ __device__ __forceinline__ void group_sync(int G)
   if (G == 1) __syncwarp(); else __syncthreads();        // the CTA is the group
 }
 
+// Registers: a lone warp needs the instruction-level parallelism of two records x three detectors in flight, and the
+// register file is per SM sub-partition (16384 registers: two warps above 170 registers per thread, three up to 168, four
+// up to 128).  Capping the kernel at 168, 144 or 128 registers (no spills) costs 35 - 100 % per warp on B200 and loses
+// more than the extra resident warps return, for 500 chains and for 2500 (profiles/r02_k3_experiments.md): it may use 255.
+#define NSS_K3_BOUNDS __launch_bounds__(kChainThreads, 1)
 template <int NDET, int KIND, int LANES, bool RESIDENT>
-__global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_constant__ NssDev P, const ChainArgs A)
+__global__ void NSS_K3_BOUNDS k3_slice(const __grid_constant__ NssDev P, const ChainArgs A)
 {
   constexpr int NSUB = 32 / LANES;                              // candidates per warp
   constexpr int NC = (NSS_NSLOT + LANES - 1) / LANES;           // coordinates per lane
@@ -747,6 +802,7 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
   __shared__ double sLo[NSS_NSLOT + 1], sHi[NSS_NSLOT + 1];        // prior box, (-inf, +inf) for the unused coordinates
   __shared__ __align__(16) double sConst[nssk::kSubConstDoubles];
   __shared__ unsigned sLast;
+  __shared__ double sChol[NSS_NSLOT * NSS_NSLOT];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int sl = lane & (LANES - 1), sub = lane / LANES;
   nssk::SubCtx X;
@@ -778,12 +834,20 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
     X.tab = reinterpret_cast<const double *>(smem_raw);
   }
   // Everything above is independent of the kernels in front (programmatic dependent launch: it overlaps their tails);
-  // everything below reads what k4_front and k_directions wrote.
+  // everything below reads what k4_front wrote.
   asm volatile("griddepcontrol.wait;" ::: "memory");
   NssCtl *ctl = A.ctl;
   if (ctl->flags[0] | ctl->flags[1] | ctl->flags[2]) return;      // Cholesky failure, threshold violation, or converged
-  const int G = blockDim.x >> 5, C = G * NSUB;
-  const int w = warp;                                    // warp in the group
+  for (int t = threadIdx.x; t < d * d; t += blockDim.x) sChol[t] = A.chol[t];
+  __syncthreads();
+  // A CTA is one group of G warps (G > 1), or W = blockDim/32 single-warp groups that share the record table (G == 1);
+  // single-warp groups take their chains from a device counter, so a warp that finishes early starts the next chain
+  const int G = A.G, C = G * NSUB;
+  const int w = warp & (G - 1);                          // warp in the group
+  const int gbase = (warp - w) * NSUB;                   // first candidate slot of the group in sRes
+  // a5: the group's slice directions, kDirChunk steps at a time: [kDirChunk][NSS_NSLOT] per group, behind the scratches
+  double *sDir = reinterpret_cast<double *>(smem_raw + tab_bytes) + (size_t)(blockDim.x >> 5) * NSUB * nssk::kSubScratchDoubles
+               + (size_t)((warp - w) / G) * kDirChunk * NSS_NSLOT;
   const int gl = w * 32 + lane;                          // lane in the group
   const int cs = w * NSUB + sub;                         // candidate slot of this sub-warp in the group
   const double Lstar = ctl->state[3];
@@ -803,8 +867,16 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
     per[c] = own[c] && P.periodic[j] != 0;
   }
   int par = 0;
+  // lane j < d owns coordinate j of the per-warp position copy sX (walls and period of that coordinate in registers)
+  const bool lper = lane < d && P.periodic[lane < NSS_NSLOT ? lane : 0] != 0;
+  const double llo = lane < d ? P.lo[lane < NSS_NSLOT ? lane : 0] : 0.0, lhi = lane < d ? P.hi[lane < NSS_NSLOT ? lane : 0] : 0.0;
 
-  for (int ch = blockIdx.x; ch < A.k; ch += gridDim.x) {
+  for (int ch = blockIdx.x;; ch += gridDim.x) {
+    if (G == 1) {
+      if (lane == 0) ch = (int)atomicAdd(&ctl->chain_next, 1u);
+      ch = __shfl_sync(0xffffffffu, ch, 0);
+    }
+    if (ch >= A.k) break;
     const uint32_t chain = (uint32_t)ch;
     // a4: start from a uniformly chosen survivor
     int si = (int)floor(uniform_a(A.seed, 0u, kStepStart, chain, it) * (double)ns);
@@ -821,21 +893,27 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
     int rounds = 0, nexec = 0;
     double margin = INFINITY, margin_l = INFINITY;        // bracket-end tests (uniform) / this lane's proposals
 
-    // a5: the directions were drawn by k_directions; the next step's is fetched while this step runs
-    const double *vsrc = A.dirs + (size_t)ch * A.n_repeats * d;
-    double vpre = (lane < d && A.n_repeats > 0) ? vsrc[lane] : 0.0;
+    // uniforms of a step: lane 0 -> bracket offset (block 0); lane 1+i -> shrinkage proposal ubase+i (block 64+ubase+i).
+    // Drawn one step ahead, so that the Philox rounds are off the critical path of the step that uses them.
+    double unext = uniform_a(A.seed, lane == 0 ? 0u : (uint32_t)(63 + lane), 0u, chain, it);
     {
       for (int s = 0; s < A.n_repeats; ++s) {
+        // a5: the directions of the next kDirChunk steps, one lane of the group's first warp each (they depend on the
+        // Cholesky factor and on counter-based draws only)
+        if ((s & (kDirChunk - 1)) == 0) {
+          group_sync(G);                                 // every warp of the group has taken the last direction of the chunk before
+          if (gl < kDirChunk && s + gl < A.n_repeats) draw_direction(d, sChol, A.seed, it, chain, (uint32_t)(s + gl), sDir + gl * NSS_NSLOT);
+          group_sync(G);
+        }
         __syncwarp();
-        if (lane < d) sV[warp][lane] = vpre;
+        if (lane < d) sV[warp][lane] = sDir[(s & (kDirChunk - 1)) * NSS_NSLOT + lane];
         __syncwarp();
-        if (lane < d && s + 1 < A.n_repeats) vpre = vsrc[(size_t)(s + 1) * d + lane];
         const double *vrow = sV[warp];
         double vj[NC];
 #pragma unroll
         for (int c = 0; c < NC; ++c) vj[c] = own[c] ? vrow[sl + c * LANES] : 0.0;
-        // uniforms of this step: lane 0 -> bracket offset (block 0); lane 1+i -> shrinkage proposal ubase+i (block 64+ubase+i)
-        double ulane = uniform_a(A.seed, lane == 0 ? 0u : (uint32_t)(63 + lane), (uint32_t)s, chain, it);
+        double ulane = unext;
+        unext = uniform_a(A.seed, lane == 0 ? 0u : (uint32_t)(63 + lane), (uint32_t)(s + 1), chain, it);
         int ubase = 0;
         const double u0 = nssk::shfl_d(ulane, 0);
         double l = -u0, r = 1.0 - u0;
@@ -856,12 +934,28 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
           double my_t = (lane == 0 && !ldone) ? l : r;   // lanes < nside: the bracket ends
           double my_ls = l, my_rs = r;                   // the bracket after this lane's test has failed
           {
+            // The proposals are a serial recurrence (each bracket follows from the rejection of the proposal before), so
+            // the walk is on the critical path of the round: the first kWalk steps run with a fixed trip count (uniforms
+            // fetched up front, no branches; steps past nshr compute values no lane keeps), the rest in a plain loop.
+            constexpr int kWalk = 8;
             double ls = l, rs = r;
-            for (int j = 0; j < nshr; ++j) {
-              const double uk = nssk::shfl_d(ulane, kk - ubase + j + 1);
-              const double t = __dadd_rn(ls, __dmul_rn(rs - ls, uk));
+            double uk[kWalk];
+#pragma unroll
+            for (int j = 0; j < kWalk; ++j) uk[j] = nssk::shfl_d(ulane, (kk - ubase + j + 1) & 31);
+            const int mine = lane - nside;                 // this lane's proposal in the list (if 0 <= mine < nshr)
+#pragma unroll
+            for (int j = 0; j < kWalk; ++j) {
+              const double t = __dadd_rn(ls, __dmul_rn(rs - ls, uk[j]));
+              const bool neg = t < 0.0;
+              ls = neg ? t : ls;
+              rs = neg ? rs : t;
+              if (mine == j) { my_t = t; my_ls = ls; my_rs = rs; }
+            }
+            for (int j = kWalk; j < nshr; ++j) {
+              const double u = nssk::shfl_d(ulane, kk - ubase + j + 1);
+              const double t = __dadd_rn(ls, __dmul_rn(rs - ls, u));
               if (t < 0.0) ls = t; else rs = t;
-              if (lane == nside + j) { my_t = t; my_ls = ls; my_rs = rs; }
+              if (mine == j) { my_t = t; my_ls = ls; my_rs = rs; }
             }
           }
           // box test (inclusive) of the lane's own test: y = x + t v, every coordinate
@@ -898,9 +992,9 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
           double ly;
           if (KIND == NSS_KIND_GAUSS) ly = have ? nssk::gauss_loglike(P, X.scr) : -INFINITY;
           else ly = nssk::loglike_sub<NDET, KIND, LANES>(P, X, have);
-          if (sl == 0) sRes[par][cs] = ly;
+          if (sl == 0) sRes[par][gbase + cs] = ly;
           group_sync(G);
-          const double *res = sRes[par];
+          const double *res = sRes[par] + gbase;
           par ^= 1;
           // ---- replay the sequential decisions: tests outside the box fail without an evaluation, tests inside
           // take the next result; the first test whose result is not there yet ends the round -------------------
@@ -926,7 +1020,7 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
             // fails for free; one inside has the result of slot `below` if below < C, else it is not known yet.
             const bool shr = lane >= nside && lane < nt;
             const bool has = inb && below < C;
-            const double vi = has ? res[below < kSlots ? below : 0] : -INFINITY;
+            const double vi = has ? res[has ? below : 0] : -INFINITY;
             const unsigned mU = __ballot_sync(0xffffffffu, shr && inb && below >= C);
             const unsigned mP = __ballot_sync(0xffffffffu, shr && has && vi > Lstar);
             const unsigned mH = __ballot_sync(0xffffffffu, shr && has);
@@ -946,10 +1040,10 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
                 xj[c] = __dadd_rn(xj[c], __dmul_rn(tj, vj[c]));
                 if (per[c]) xj[c] = wrap_periodic(xj[c], lo_j[c], hi_j[c]);
               }
-              for (int jj = lane; jj < d; jj += 32) {
-                double y = __dadd_rn(sX[warp][jj], __dmul_rn(tj, vrow[jj]));
-                if (P.periodic[jj]) y = wrap_periodic(y, P.lo[jj], P.hi[jj]);
-                sX[warp][jj] = y;
+              if (lane < d) {                            // d <= NSS_NSLOT < 32: one coordinate per lane
+                double y = __dadd_rn(sX[warp][lane], __dmul_rn(tj, vrow[lane]));
+                if (lper) y = wrap_periodic(y, llo, lhi);
+                sX[warp][lane] = y;
               }
               acc = kk + (firstP - nside); done = true;
             } else {
@@ -992,28 +1086,36 @@ __global__ void __launch_bounds__(kChainThreads, 1) k3_slice(const __grid_consta
     // logZ_live = logX + logsumexp(logL) - ln n over the updated live set and applies the stop test
     if (A.live_evidence) {
       __threadfence();
-      __syncthreads();
-      if (threadIdx.x == 0) sLast = atomicAdd(&ctl->chains_done, 1u);
-      __syncthreads();
-      if (sLast == (unsigned)A.k - 1u) {
+      group_sync(G);
+      unsigned last = 0;
+      if (gl == 0) last = atomicAdd(&ctl->chains_done, 1u);
+      if (G == 1) last = __shfl_sync(0xffffffffu, last, 0);
+      else {
+        if (gl == 0) sLast = last;
+        __syncthreads();
+        last = sLast;
+      }
+      if (last == (unsigned)A.k - 1u) {
         __threadfence();
-        double *red = sRes[0];
+        double *red = sRes[0] + gbase;
+        const int GT = 32 * G;
         double mx = -INFINITY;
-        for (int i = threadIdx.x; i < A.n; i += blockDim.x) mx = fmax(mx, __ldcg(A.logL + i));
+        for (int i = gl; i < A.n; i += GT) mx = fmax(mx, __ldcg(A.logL + i));
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-        if (lane == 0) red[warp] = mx;
-        __syncthreads();
+        group_sync(G);
+        if (lane == 0) red[w] = mx;
+        group_sync(G);
         mx = red[0];
         for (int q = 1; q < G; ++q) mx = fmax(mx, red[q]);
-        __syncthreads();
+        group_sync(G);
         double se = 0.0;
         if (mx > -INFINITY)
-          for (int i = threadIdx.x; i < A.n; i += blockDim.x) se += exp(__ldcg(A.logL + i) - mx);
+          for (int i = gl; i < A.n; i += GT) se += exp(__ldcg(A.logL + i) - mx);
         se = nssk::warp_sum(se);
-        if (lane == 0) red[warp] = se;
-        __syncthreads();
-        if (threadIdx.x == 0) {
+        if (lane == 0) red[w] = se;
+        group_sync(G);
+        if (gl == 0) {
           double tot = 0.0;
           for (int q = 0; q < G; ++q) tot += red[q];          // fixed order: deterministic
           const double lzl = mx > -INFINITY ? ctl->state[0] + mx + log(tot) - log((double)A.n) : -INFINITY;
@@ -1038,22 +1140,43 @@ int launch_chains_k(nss_handle *h, ChainArgs &A, size_t tab_bytes, cudaStream_t 
     G = LANES == 8 ? 1 : (A.k * 8LL <= S ? 4 : A.k <= S ? 2 : 1);
   }
   A.G = G;
-  const size_t smem = tab_bytes + (size_t)G * (32 / LANES) * nssk::kSubScratchDoubles * sizeof(double);
+  // G > 1: one chain per CTA, the block scheduler balances the SMs.  G == 1: W single-warp chains per CTA share one copy of
+  // the record table, and the warps of a persistent grid take chains from a device counter until none is left.
+  int W = 1;
+  if (G == 1) {
+    W = h->chain_pack >= 1 && h->chain_pack <= kChainWarps ? h->chain_pack : (A.k > 4LL * h->n_sm ? 4 : 1);
+  }
+  const size_t smem = tab_bytes + (size_t)W * G * (32 / LANES) * nssk::kSubScratchDoubles * sizeof(double)
+                    + (size_t)W * kDirChunk * NSS_NSLOT * sizeof(double);
   static size_t smem_set = 0;                            // per instantiation: the attribute is raised only when a launch needs more
   if (smem > smem_set) {
     NSS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     smem_set = smem;
   }
+  unsigned grid = (unsigned)A.k;
+  if (G == 1) {
+    static int per_sm[kChainWarps + 1] = {0};            // resident CTAs per SM for W warps (per instantiation)
+    if (!per_sm[W]) {
+      int nb = 0;
+      NSS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, 32 * W, smem));
+      per_sm[W] = nb > 0 ? nb : 1;
+    }
+    const long long slots = (long long)per_sm[W] * h->n_sm, need = (A.k + W - 1) / W;
+    grid = (unsigned)(need < slots ? need : slots);
+  }
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3((unsigned)A.k);                     // one chain per CTA: the block scheduler balances the SMs
-  cfg.blockDim = dim3(32u * G); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(32u * G * W); cfg.dynamicSmemBytes = smem; cfg.stream = st;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;      // the prologue (table staging) overlaps the kernels in front
   at[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = at; cfg.numAttrs = 1;
-  NSS_CUDA(cudaEventRecord(h->ev_k3[0], st));
+  // An event in front of K3 separates it from k4_front in the stream (the programmatic launch then overlaps nothing: ~5 us
+  // per iteration on B200), so the pair is recorded only on request (nss_set_chain_timing)
+  if (h->chain_timing) NSS_CUDA(cudaEventRecord(h->ev_k3[0], st));
   NSS_CUDA(cudaLaunchKernelEx(&cfg, kern, h->dev, A));
-  NSS_CUDA(cudaEventRecord(h->ev_k3[1], st));
+  if (h->chain_timing) NSS_CUDA(cudaEventRecord(h->ev_k3[1], st));
+  h->ev_k3_valid = h->chain_timing;
   return NSS_OK;
 }
 
@@ -1089,7 +1212,6 @@ int launch_chains(nss_handle *h, ChainArgs &A, cudaStream_t st)
     rc = launch_chains_k<1, NSS_KIND_GAUSS, 32, false>(h, A, 0, st);
   }
   if (rc) return rc;
-  h->ev_k3_valid = 1;
   h->launches += 1;
   NSS_CUDA(cudaGetLastError());
   return NSS_OK;
@@ -1100,7 +1222,7 @@ __global__ void k_begin(NssCtl *ctl, int set_state, double logX, double logZ, in
 {
   if (threadIdx.x < 4) ctl->flags[threadIdx.x] = 0;
   if (threadIdx.x == 0) {
-    ctl->front_done = 0; ctl->rank_done = 0; ctl->sel_bad = 0; ctl->chains_done = 0; ctl->chol_now = 0; ctl->tune_cnt[0] = 0; ctl->tune_cnt[1] = 0;
+    ctl->front_done = 0; ctl->rank_done = 0; ctl->sel_bad = 0; ctl->chains_done = 0; ctl->chain_next = 0; ctl->chol_now = 0; ctl->tune_cnt[0] = 0; ctl->tune_cnt[1] = 0;
     if (set_state) { ctl->state[0] = logX; ctl->state[1] = logZ; ctl->state[2] = 0.0; ctl->state[3] = 0.0; }
     if (zero_evals) { ctl->nevals = 0ull; ctl->nrounds = 0ull; ctl->nexec = 0ull; }
   }
@@ -1149,10 +1271,10 @@ int ensure_scratch(nss_handle *h, int n)
   return NSS_OK;
 }
 
-// The device part of one NS iteration (no host synchronisation), three launches:
-//   k4_front      a1 rank/select, a3 tune, flag and counter reset
-//   k_directions  a5 for every (chain, step); a2 evidence (if dead_logw) in one more block beside them
-//   k3_slice      a4, a6 - a10, and a11's live evidence + stop test as epilogue (if live_evidence)
+// The device part of one NS iteration (no host synchronisation), two launches:
+//   k4_front      a1 rank/select, a2 evidence (if dead_logw), a3 tune, flag and counter reset
+//   k3_slice      a4 - a10 (the slice directions a5 are drawn by the chain's own lanes), and a11's live evidence + stop test
+//                 as epilogue (if live_evidence)
 // `reset`: a stand-alone iteration (flags cleared; logX / logZ loaded and counters zeroed on request).
 int enqueue_iteration(nss_handle *h, double *live, double *logL, double *birth, int n, int k, double Lstar_in, int n_repeats,
                       uint64_t seed, uint32_t iteration, double *dead_theta, double *dead_logL, double *dead_birth,
@@ -1160,35 +1282,19 @@ int enqueue_iteration(nss_handle *h, double *live, double *logL, double *birth, 
                       int live_evidence, double stop_dlogz, cudaStream_t st)
 {
   const int d = h->dev.d;
-  {
-    const size_t need = sizeof(double) * (size_t)k * (n_repeats > 0 ? n_repeats : 1) * d;
-    if (h->dirs_bytes < need) {                          // first use, or a larger n_delete x n_repeats than before
-      NSS_CUDA(cudaDeviceSynchronize());                 // an earlier launch may still read the old block
-      cudaFree(h->d_dirs);
-      h->d_dirs = nullptr; h->dirs_bytes = 0;
-      cudaError_t e = cudaMalloc((void **)&h->d_dirs, need);
-      if (e != cudaSuccess) { nss_cuda_fail(e, "cudaMalloc(dirs)"); return e == cudaErrorMemoryAllocation ? NSS_ENOMEM : NSS_ECUDA; }
-      h->dirs_bytes = need;
-    }
-  }
   FrontArgs F;
   F.live = live; F.logL = logL; F.birth = birth; F.n = n; F.k = k; F.d = d; F.Lstar_in = Lstar_in;
   F.T = tune_blocks_for(n); F.nseg = rank_segments(n);
   F.rank_part = h->d_rank_part; F.rank = h->d_rank; F.dead_idx = dead_idx; F.surv_idx = h->d_surv_idx; F.tune_scratch = h->d_tune_scratch;
-  F.dead_theta = dead_theta; F.dead_logL = dead_logL; F.dead_birth = dead_birth;
+  F.dead_theta = dead_theta; F.dead_logL = dead_logL; F.dead_birth = dead_birth; F.dead_logw = dead_logw;
   F.mean = h->d_mean; F.chol = h->d_chol; F.ctl = h->d_ctl;
   F.reset = reset; F.set_state = set_state; F.zero_evals = zero_evals; F.logX = logX; F.logZ = logZ;
   k4_front<<<F.T + ((n + kRankElems - 1) / kRankElems) * F.nseg, kOneCta, 0, st>>>(F);
   h->launches += 1;
-  if (n_repeats > 0 || dead_logw) {
-    k_directions<<<(k * n_repeats + 127) / 128 + 1, 128, 0, st>>>(d, h->d_chol, k, n_repeats, seed, iteration, h->d_flags, h->d_dirs, n,
-                                                                   dead_logL, dead_logw, h->d_state);
-    h->launches += 1;
-  }
   NSS_CUDA(cudaGetLastError());
   ChainArgs A;
   A.live = live; A.logL = logL; A.birth = birth; A.n = n; A.k = k; A.n_repeats = n_repeats; A.seed = seed;
-  A.iteration = iteration; A.surv_idx = h->d_surv_idx; A.dead_idx = dead_idx; A.dirs = h->d_dirs; A.ctl = h->d_ctl;
+  A.iteration = iteration; A.surv_idx = h->d_surv_idx; A.dead_idx = dead_idx; A.chol = h->d_chol; A.ctl = h->d_ctl;
   A.trace = h->trace_dev; A.margin = h->margin_dev; A.G = 1; A.live_evidence = live_evidence; A.stop_dlogz = stop_dlogz;
   switch (h->dev.n_det) {
     case 0: case 1: return launch_chains<1>(h, A, st);
@@ -1229,6 +1335,21 @@ extern "C" int nss_set_chain_lanes(nss_handle *h, int32_t lanes)
 {
   if (!h || !(lanes == 0 || lanes == 8 || lanes == 16 || lanes == 32)) return NSS_EINVAL;
   h->chain_lanes = lanes;
+  return NSS_OK;
+}
+
+extern "C" int nss_set_chain_timing(nss_handle *h, int32_t on)
+{
+  if (!h) return NSS_EINVAL;
+  h->chain_timing = on != 0;
+  if (!on) h->ev_k3_valid = 0;
+  return NSS_OK;
+}
+
+extern "C" int nss_set_chain_pack(nss_handle *h, int32_t chains_per_cta)
+{
+  if (!h || chains_per_cta < 0 || chains_per_cta > kChainWarps) return NSS_EINVAL;
+  h->chain_pack = chains_per_cta;
   return NSS_OK;
 }
 
@@ -1353,6 +1474,27 @@ extern "C" int nss_replace_step(nss_handle *h, double *live_dev, double *logL_de
   return NSS_OK;
 }
 
+extern "C" int nss_resample_equal(nss_handle *h, const double *logL_dev, const double *logw_dev, int64_t n, uint64_t seed,
+                                  int64_t *idx_dev, int64_t *n_equal_host, void *cuda_stream)
+{
+  if (!h || n < 0 || !n_equal_host || (n > 0 && (!logL_dev || !logw_dev))) return NSS_EINVAL;
+  *n_equal_host = 0;
+  if (n == 0) return NSS_OK;
+  NSS_CUDA(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = ensure_scratch(h, 2);
+  if (rc) return rc;
+  static_assert(sizeof(long long) == sizeof(int64_t), "int64_t rows");
+  k_resample_equal<<<1, kOneCta, 0, st>>>(logL_dev, logw_dev, (long long)n, seed, (long long *)idx_dev, h->d_tune_scratch);
+  h->launches += 1;
+  NSS_CUDA(cudaGetLastError());
+  double cnt = 0.0;
+  NSS_CUDA(cudaMemcpyAsync(&cnt, h->d_tune_scratch, sizeof(double), cudaMemcpyDeviceToHost, st));
+  NSS_CUDA(cudaStreamSynchronize(st));
+  *n_equal_host = (int64_t)cnt;
+  return NSS_OK;
+}
+
 namespace {
 int ensure_stage(nss_handle *h, size_t bytes)
 {
@@ -1462,7 +1604,8 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
   const size_t o_live = 0, o_logL = o_live + align256(sizeof(double) * (size_t)n * d), o_dth = o_logL + align256(sizeof(double) * n),
                o_dl = o_dth + align256(sizeof(double) * (size_t)cap * d), o_db = o_dl + align256(sizeof(double) * cap),
                o_dw = o_db + align256(sizeof(double) * cap), o_err = o_dw + align256(sizeof(double) * cap),
-               total = o_err + align256(sizeof(double) * (kErrReplicas + 1));
+               o_eq = o_err + align256(sizeof(double) * (kErrReplicas + 2)),
+               total = o_eq + (out->equal_idx ? align256(sizeof(int64_t) * cap) : 0);
   if (h->run_bytes < total) {
     cudaFree(h->d_run);
     h->d_run = nullptr; h->run_bytes = 0;
@@ -1477,6 +1620,7 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
   unsigned char *rb = h->d_run;
   double *live = (double *)(rb + o_live), *logL = (double *)(rb + o_logL), *dth = (double *)(rb + o_dth), *dl = (double *)(rb + o_dl),
          *db = (double *)(rb + o_db), *dw = (double *)(rb + o_dw), *derr = (double *)(rb + o_err);
+  long long *deq = out->equal_idx ? (long long *)(rb + o_eq) : nullptr;
   cudaEvent_t e0 = h->ev_run[0], e1 = h->ev_run[1];
   // every exit, the error exits included, leaves the stream drained (an iteration may still be queued)
   auto cleanup = [&]() { cudaStreamSynchronize(st); };
@@ -1545,12 +1689,14 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
     RUN_CUDA(cudaMemcpyAsync(out->dead_theta, dth, sizeof(double) * (size_t)n_dead * d, cudaMemcpyDeviceToHost, st));
     RUN_CUDA(cudaMemcpyAsync(out->dead_logL, dl, sizeof(double) * n_dead, cudaMemcpyDeviceToHost, st));
     RUN_CUDA(cudaMemcpyAsync(out->dead_logL_birth, db, sizeof(double) * n_dead, cudaMemcpyDeviceToHost, st));
-    RUN_CUDA(cudaMemcpyAsync(out->dead_logw, dw, sizeof(double) * n_it_dead, cudaMemcpyDeviceToHost, st));
+    k_fill_live_logw<<<(n + 255) / 256, 256, 0, st>>>(dw + n_it_dead, n, h->d_state);
+    RUN_CUDA(cudaMemcpyAsync(out->dead_logw, dw, sizeof(double) * n_dead, cudaMemcpyDeviceToHost, st));
     // O15: the replica evidences on the device (one CTA per replica), reduced to a standard deviation below
-    double lz_rep[kErrReplicas + 1];                     // [kErrReplicas] = Kish ESS
+    double lz_rep[kErrReplicas + 2];                     // [kErrReplicas] = Kish ESS, [kErrReplicas + 1] = equal-weight rows
     k_evidence_error<<<kErrReplicas, 256, 0, st>>>(dl, n_it_dead, n, k, seed, logL, derr);
     k_kish_ess<<<1, kOneCta, 0, st>>>(dl, dw, n_it_dead, logL, n, h->d_state, derr + kErrReplicas);
-    h->launches += 2;
+    k_resample_equal<<<1, kOneCta, 0, st>>>(dl, dw, (long long)n_dead, seed, deq, derr + kErrReplicas + 1);
+    h->launches += 4;
     RUN_CUDA(cudaMemcpyAsync(lz_rep, derr, sizeof(lz_rep), cudaMemcpyDeviceToHost, st));
     RUN_CUDA(cudaEventRecord(e1, st));
     RUN_CUDA(cudaStreamSynchronize(st));
@@ -1558,7 +1704,6 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
     RUN_CUDA(cudaEventElapsedTime(&ms, e0, e1));
     out->gpu_ms = ms;
     const double logX = state[0], logZ = state[1], logZ_live = state[2];
-    for (int j = 0; j < n; ++j) out->dead_logw[n_it_dead + j] = logX - log((double)n);
     auto lae = [](double a, double b) {
       if (a == -INFINITY) return b;
       if (b == -INFINITY) return a;
@@ -1578,6 +1723,9 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
     var = var < 0 ? 0 : var;
     out->logZ = logZf; out->logZ_err = sqrt(var * R / (R - 1)); out->H = H;
     out->ess = lz_rep[kErrReplicas];
+    out->n_equal = (int64_t)lz_rep[kErrReplicas + 1];
+    if (out->equal_idx && out->n_equal > 0)
+      RUN_CUDA(cudaMemcpy(out->equal_idx, deq, sizeof(int64_t) * (size_t)out->n_equal, cudaMemcpyDeviceToHost));
     out->n_iter = t; out->n_dead = n_dead; out->n_evals = (int64_t)ne + n;
   }
 #undef RUN_CUDA

@@ -151,7 +151,7 @@ extern "C" int nss_destroy(nss_handle *h)
   cudaFree(h->d_surv_idx); cudaFree(h->d_dead_idx); cudaFree(h->d_rank); cudaFree(h->d_rank_part); cudaFree(h->d_tune_scratch); cudaFree(h->d_ctl);
   if (h->h_ctl) cudaFreeHost(h->h_ctl);
   cudaFree(h->d_mean); cudaFree(h->d_chol); cudaFree(h->d_birth); cudaFree(h->d_stage);
-  cudaFree(h->d_run); cudaFree(h->d_dirs);
+  cudaFree(h->d_run);
   if (h->ev_ctl[0]) cudaEventDestroy(h->ev_ctl[0]);
   if (h->ev_ctl[1]) cudaEventDestroy(h->ev_ctl[1]);
   if (h->ev_run[0]) cudaEventDestroy(h->ev_run[0]);

@@ -7,6 +7,11 @@ Prints a markdown table: evaluations per second and the fraction of the fp64 DFM
 process by `nss_fp64_peak`) for the automatic kernel choice and for both kernel forms (one thread per point; one
 sub-warp per point).  Parity of the same kernels against the oracle at B = 64, 256, 1024 is in
 tests/test_gpu_loglike.py; this script only times (inputs resident in HBM, L2 flushed between launches).
+
+A second table times the FRONT of an NS iteration (k4_front: delete-select by counting ranks, O(n^2) comparisons, beside
+mean / covariance / Cholesky) at n_live = 1000 ... 65536 through `nss_replace_step` with zero slice repeats, next to one
+full iteration at the same n_live, to show where the counting select stops being negligible (north_star names a radix
+select; bit-exact parity of the counting select, ties included, is in tests/test_gpu_sampler.py).
 """
 from __future__ import annotations
 
@@ -53,6 +58,36 @@ def main():
                 ins = work(B, w.n_det)
                 print(f"| {B} | {N} | {name} | {ms:.4f} | {rate:.3e} | {ins} | {rate * ins / (peak * 1e12 / 2):.3f} |", flush=True)
         g.close()
+    front_table(torch, inputs, nss, flush)
+
+
+def front_table(torch, inputs, nss, flush):
+    w = inputs.make_data(inputs.config2(), nss.nss_waveform)
+    g = nss.Nss(w)
+
+    def timed(fn, reps=5):
+        ts = []
+        for _ in range(reps):
+            flush.fill_(1)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn()
+            b.record()
+            b.synchronize()
+            ts.append(a.elapsed_time(b))
+        return sorted(ts)[len(ts) // 2]
+
+    print("\n## front of an NS iteration (select + tune + evidence + host synchronisation) vs n_live, n_delete = n_live/2\n")
+    print("| n_live | front only ms (0 slice repeats) | full iteration ms (55 repeats) | front / iteration |")
+    print("|---|---|---|---|")
+    for n in (1000, 5000, 16000, 65536):
+        live, logL = g.nss_init_live(n, 1)
+        g.nss_replace_step(live, logL, n // 2, 0, 1, 0)
+        front = timed(lambda: g.nss_replace_step(live, logL, n // 2, 0, 1, 0))
+        g.nss_replace_step(live, logL, n // 2, w.n_repeats, 1, 0)
+        full = timed(lambda: g.nss_replace_step(live, logL, n // 2, w.n_repeats, 1, 0), reps=3)
+        print(f"| {n} | {front:.4f} | {full:.4f} | {front / full:.4f} |", flush=True)
+    g.close()
 
 
 if __name__ == "__main__":

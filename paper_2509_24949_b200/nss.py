@@ -48,7 +48,8 @@ class nss_result(C.Structure):
         ("logZ", C.c_double), ("logZ_err", C.c_double), ("H", C.c_double), ("n_iter", C.c_int32),
         ("n_dead", C.c_int64), ("n_evals", C.c_int64), ("dead_theta", C.POINTER(C.c_double)),
         ("dead_logL", C.POINTER(C.c_double)), ("dead_logL_birth", C.POINTER(C.c_double)),
-        ("dead_logw", C.POINTER(C.c_double)), ("cap", C.c_int64), ("gpu_ms", C.c_double), ("ess", C.c_double)]
+        ("dead_logw", C.POINTER(C.c_double)), ("cap", C.c_int64), ("gpu_ms", C.c_double), ("ess", C.c_double),
+        ("n_equal", C.c_int64), ("equal_idx", C.POINTER(C.c_int64))]
 
 
 class nss_iter_state(C.Structure):
@@ -59,8 +60,8 @@ class nss_iter_state(C.Structure):
 EXPORTS = ("nss_create", "nss_destroy", "nss_loglike_batch", "nss_loglike_batch_host", "nss_set_loglike_variant",
            "nss_replace_step", "nss_iterate", "nss_iterate_host",
            "nss_set_trace", "nss_select_lowest", "nss_tune", "nss_evidence_update", "nss_init_live",
-           "nss_philox", "nss_run", "nss_waveform", "nss_get_tables", "nss_fp64_peak", "nss_launch_count",
-           "nss_last_chain_ms", "nss_set_chain_warps", "nss_set_chain_lanes", "nss_last_chain_diag", "nss_set_periodic",
+           "nss_philox", "nss_run", "nss_resample_equal", "nss_waveform", "nss_get_tables", "nss_fp64_peak", "nss_launch_count",
+           "nss_last_chain_ms", "nss_set_chain_timing", "nss_set_chain_warps", "nss_set_chain_lanes", "nss_set_chain_pack", "nss_last_chain_diag", "nss_set_periodic",
            "nss_strerror", "nss_last_cuda_error", "nss_version")
 
 _lib = None
@@ -94,13 +95,16 @@ def lib():
         L.nss_philox.argtypes = [vp, C.c_uint64, vp, C.c_int64, vp, vp]
         L.nss_run.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_uint64, C.c_double, C.c_int32,
                               C.POINTER(nss_result), vp]
+        L.nss_resample_equal.argtypes = [vp, vp, vp, C.c_int64, C.c_uint64, vp, C.POINTER(C.c_int64), vp]
         L.nss_waveform.argtypes = [c_dp, C.POINTER(nss_detector), C.c_double, c_dp, C.c_int32, c_dp]
         L.nss_get_tables.argtypes = [vp, vp, c_dp, c_dp]
         L.nss_fp64_peak.argtypes = [C.c_double, c_dp, vp]
         L.nss_launch_count.argtypes = [vp]
         L.nss_last_chain_ms.argtypes = [vp, c_dp]
         L.nss_set_chain_warps.argtypes = [vp, C.c_int32]
+        L.nss_set_chain_timing.argtypes = [vp, C.c_int32]
         L.nss_set_chain_lanes.argtypes = [vp, C.c_int32]
+        L.nss_set_chain_pack.argtypes = [vp, C.c_int32]
         L.nss_set_periodic.argtypes = [vp, C.POINTER(C.c_int32)]
         L.nss_last_chain_diag.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.nss_launch_count.restype = C.c_int64
@@ -210,6 +214,10 @@ class Nss:
         _check(lib().nss_last_chain_ms(self._h, C.byref(ms)), "nss_last_chain_ms")
         return ms.value
 
+    def set_chain_timing(self, on: bool):
+        """Record CUDA events around K3 from now on (nss_last_chain_ms); costs the launch overlap, so off by default."""
+        _check(lib().nss_set_chain_timing(self._h, 1 if on else 0), "nss_set_chain_timing")
+
     def set_chain_warps(self, warps: int):
         _check(lib().nss_set_chain_warps(self._h, int(warps)), "nss_set_chain_warps")
 
@@ -230,6 +238,9 @@ class Nss:
 
     def set_chain_lanes(self, lanes: int):
         _check(lib().nss_set_chain_lanes(self._h, int(lanes)), "nss_set_chain_lanes")
+
+    def set_chain_pack(self, chains_per_cta: int):
+        _check(lib().nss_set_chain_pack(self._h, int(chains_per_cta)), "nss_set_chain_pack")
 
     def set_loglike_variant(self, variant: int):
         _check(lib().nss_set_loglike_variant(self._h, int(variant)), "nss_set_loglike_variant")
@@ -339,7 +350,17 @@ class Nss:
         return dict(rc=rc, live=live, logL=logL, dead_theta=dth, dead_logL=dl, dead_idx=didx, logLstar=ls.value,
                     n_evals=ne.value, trace=trace[:, :n_repeats] if want_trace else None, margin=margin)
 
-    def nss_run(self, n_live, n_delete, n_repeats, seed, stop_dlogz=-3.0, max_iter=10000, cap=None):
+    def nss_resample_equal(self, logL, logw, seed):
+        """Reading R6: row indices (ascending, torch int64 on the device) of the equal-weight posterior sample."""
+        torch = self.torch
+        l, w = self._dev(logL), self._dev(logw)
+        idx = torch.empty(l.numel(), dtype=torch.int64, device="cuda")
+        m = C.c_int64()
+        _check(lib().nss_resample_equal(self._h, l.data_ptr(), w.data_ptr(), l.numel(), int(seed), idx.data_ptr(), C.byref(m),
+                                        _stream()), "nss_resample_equal")
+        return idx[: m.value]
+
+    def nss_run(self, n_live, n_delete, n_repeats, seed, stop_dlogz=-3.0, max_iter=10000, cap=None, want_equal=False):
         if cap is None:
             cap = min(int(max_iter), 400) * int(n_delete) + int(n_live)
         dth, dl = np.empty((cap, self.d)), np.empty(cap)
@@ -348,12 +369,15 @@ class Nss:
         res.dead_theta, res.dead_logL = dth.ctypes.data_as(c_dp), dl.ctypes.data_as(c_dp)
         res.dead_logL_birth, res.dead_logw = db.ctypes.data_as(c_dp), dw.ctypes.data_as(c_dp)
         res.cap = cap
+        eq = np.empty(cap if want_equal else 0, dtype=np.int64)
+        res.equal_idx = eq.ctypes.data_as(C.POINTER(C.c_int64)) if want_equal else None
         rc = lib().nss_run(self._h, int(n_live), int(n_delete), int(n_repeats), int(seed), float(stop_dlogz),
                            int(max_iter), C.byref(res), _stream())
         _check(rc, "nss_run", ok=(NSS_OK, NSS_ENOTCONV))
         nd = int(res.n_dead)
         return dict(rc=rc, logZ=res.logZ, logZ_err=res.logZ_err, H=res.H, n_iter=int(res.n_iter), n_dead=nd,
-                    n_evals=int(res.n_evals), gpu_ms=res.gpu_ms, ess=res.ess, dead_theta=dth[:nd], dead_logL=dl[:nd],
+                    n_evals=int(res.n_evals), gpu_ms=res.gpu_ms, ess=res.ess, n_equal=int(res.n_equal),
+                    equal_idx=eq[: int(res.n_equal)] if want_equal else None, dead_theta=dth[:nd], dead_logL=dl[:nd],
                     dead_logL_birth=db[:nd], dead_logw=dw[:nd])
 
     def nss_get_tables(self):

@@ -67,6 +67,18 @@ def main():
             t1 = (t, k)
         print(f"| {k} | {t:.4f} | {r['gpu_ms']:.1f} | {r['n_iter']} | {r['n_evals']} | {r['n_evals'] / t:.3e} | "
               f"{r['logZ']:.2f} | {r['logZ_err']:.2f} | {t1[0] * t1[1] / k:.4f} |", flush=True)
+    # NEXT-3 (the half that needs no second waveform): the paper's hyper-parameters (3000 live points, half of
+    # them deleted per iteration, slice chains of 10 d steps) on the synthetic config-2 problem, with the paper's Table 1b
+    # metrics (wall clock, Kish ESS, equal-weight samples); its 207 s / 17490 (7599) is IMRPhenomD on
+    # GW150914 on an A100 and is context only
+    print("\n## the paper's hyper-parameters (n_live 3000, n_delete 1500, 10 d = 110 slice repeats) on the synthetic workload\n")
+    print("| seed | wall s | iterations | evaluations | evals/s | logZ | +- | Kish ESS | equal-weight rows | ESS/s |")
+    print("|---|---|---|---|---|---|---|---|---|---|")
+    for sd in (args.seed, args.seed + 1):
+        t, r = run_point(g, 3000, 1500, 10 * w.d, sd, 1 if args.quick else args.repeats)
+        print(f"| {sd} | {t:.4f} | {r['n_iter']} | {r['n_evals']} | {r['n_evals'] / t:.3e} | {r['logZ']:.2f} | {r['logZ_err']:.2f} | "
+              f"{r['ess']:.0f} | {r['n_equal']} | {r['ess'] / t:.3e} |", flush=True)
+
     # NEXT-2: hard walls (A16) against wrapped phi_c, psi, ra (nss_set_periodic), config 2 as benchmarked
     print("\n## hard walls vs wrapped phi_c, psi, ra (n_live = 1000, n_delete = 500)\n")
     print("| coordinates | wall s | iterations | evaluations | evals per slice step | logZ | +- | H |")

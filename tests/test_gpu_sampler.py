@@ -670,6 +670,43 @@ def test_next4_kish_ess_matches_the_formula_and_the_oracle(nssmod, oracle, wl1):
     g.close()
 
 
+def test_next4_equal_weight_resampling_matches_oracle(nssmod, oracle, ggauss, wl1):
+    """Reading R6 (the bracketed "equal weight samples" of PAPER.md:59-63): row i is kept iff u_i < p_i / p_max with the
+    reserved Philox word.  Index work: the kept rows must be the oracle's, bit for bit — on synthetic weights (ties at the
+    maximum, -inf rows, a ragged length spanning many threads' chunks, the empty and all--inf cases) and on the rows of a
+    complete run, whose result struct must carry the same count and indices."""
+    rng = np.random.default_rng(11)
+    for n in (1, 31, 1025, 70001):
+        logL = rng.normal(0.0, 3.0, n)
+        logw = -np.sort(rng.exponential(2.0, n))[::-1] - np.arange(n) * (5.0 / n)
+        logL[rng.integers(0, n, max(1, n // 50))] = -np.inf
+        top = np.nanargmax(np.where(np.isfinite(logL), logL + logw, -np.inf))
+        if n > 2:
+            logL[(top + 1) % n] = logL[top] + logw[top] - logw[(top + 1) % n]      # a tie at the maximum
+        for seed in (1, (7 << 32) | 9):
+            want = oracle.resample_equal(logL, logw, seed)
+            got = ggauss.nss_resample_equal(logL, logw, seed).cpu().numpy()
+            assert np.array_equal(got, want), (n, seed)
+            assert 1 <= got.size <= n or not np.isfinite(logL + logw).any()
+    got = ggauss.nss_resample_equal(np.full(40, -np.inf), np.zeros(40), 3)
+    assert got.numel() == 0 and oracle.resample_equal(np.full(40, -np.inf), np.zeros(40), 3).size == 0
+    assert ggauss.nss_resample_equal(np.zeros(0), np.zeros(0), 3).numel() == 0
+    # equal weights: every row has p = p_max and u < 1 always
+    assert ggauss.nss_resample_equal(np.zeros(5000), np.full(5000, -2.0), 5).numel() == 5000
+    g = nssmod.Nss(wl1)
+    for seed in (1, 2):
+        r = g.nss_run(100, 50, 12, seed, want_equal=True)
+        want = oracle.resample_equal(r["dead_logL"], r["dead_logw"], seed)
+        assert r["n_equal"] == want.size and np.array_equal(r["equal_idx"], want)
+        assert 1 <= r["n_equal"] <= r["n_dead"]
+        # expected size sum p / max p; the draw is a sum of independent Bernoullis
+        a = r["dead_logL"] + r["dead_logw"]
+        pk = np.exp(a - a.max())
+        assert abs(r["n_equal"] - pk.sum()) < 5.0 * math.sqrt((pk * (1 - pk)).sum()) + 1.0
+        assert g.nss_run(100, 50, 12, seed)["n_equal"] == r["n_equal"]          # without the index array
+    g.close()
+
+
 # ---- degenerate and extreme shapes ------------------------------------------------------------------------------------
 def test_edge_shapes_match_oracle(nssmod, oracle, wl1):
     """n_repeats = 0 (chains just copy their start survivor), n_delete = n_live - 1 (one survivor seeds every chain),

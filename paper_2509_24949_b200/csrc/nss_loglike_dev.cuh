@@ -380,12 +380,7 @@ __device__ __forceinline__ double records_sub(const NssDev &P, const double *__r
   constexpr int STRIDE = (9 + PER * NDET) * LANES;
   if (CROSS) {
     // relative binning: the table is in shared memory
-#ifdef NSS_SUB_UNROLL
-    constexpr int kUnroll = NSS_SUB_UNROLL;
-#else
-    constexpr int kUnroll = 2;
-#endif
-#pragma unroll kUnroll
+#pragma unroll 2
     for (int j = 1; j <= m; ++j, t += STRIDE) {
       double F;
       const double ph = phase_of(t, F);

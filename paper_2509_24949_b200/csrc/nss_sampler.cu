@@ -230,9 +230,9 @@ __device__ __forceinline__ double block_sum(double v, double *red)
 // factors the matrix: *chol_fail = 1 if a pivot is <= 0 (reading R5: no relative epsilon), else 0.
 constexpr int kTuneMaxBlocks = 32;
 constexpr int kTunePartDoubles = NSS_NSLOT + NSS_NSLOT * (NSS_NSLOT + 1) / 2;     // per block: column sums, then products
-// One block up to 8192 live points (a few rows per thread; no barrier between blocks on the critical path of the iteration),
-// then one more block per 4096 rows.
-__host__ __device__ inline int tune_blocks_for(int n) { const int t = n / 4096; return t < 2 ? 1 : t > kTuneMaxBlocks ? kTuneMaxBlocks : t; }
+// One block per 1024 live points (about one row per thread in the column sums, ~70 in the products): a single block, with
+// no barrier between blocks, up to 2047 rows.
+__host__ __device__ inline int tune_blocks_for(int n) { const int t = n / 1024; return t < 2 ? 1 : t > kTuneMaxBlocks ? kTuneMaxBlocks : t; }
 
 __device__ __forceinline__ void tune_block(const double *__restrict__ live, int n, int d, int b, int T, double *__restrict__ scratch,
                                            uint32_t *__restrict__ counters /*[2]*/, double *__restrict__ mean_out,
@@ -417,6 +417,113 @@ __device__ __forceinline__ void evidence_block(const double *__restrict__ dead_l
   __syncthreads();
 }
 
+// ---- K4.1 for many live points: ranks by a sample sort ---------------------------------------------------------------
+// Counting ranks costs n^2 comparisons (0.5 ms at n = 65536).  Above kRankDirectMax live points the ranks come from a
+// sample sort instead — the same total order (logL ascending, ties by slot), so the same bits:
+//   k4s_splitters  one block: S = 4 NB strided samples ordered by counting; every 4th is a splitter (NB - 1 of them)
+//   k4s_bucket     every key finds its bucket (binary search among the splitters) and takes a place in it
+//   k4s_offsets    one block: exclusive prefix sum of the bucket sizes
+//   k4s_scatter    keys grouped by bucket (order inside a bucket arbitrary)
+//   k4s_rank       rank = bucket offset + number of smaller keys in the bucket (~n / NB comparisons per key); a thread takes
+//                  one grouped key, so the lanes of a warp scan the same bucket and their loads coalesce
+// Splitters are (logL, slot) pairs, so even a population of equal values splits evenly.
+constexpr int kRankDirectMax = 8192;
+constexpr int kSplitMaxBuckets = 512;
+__host__ __device__ inline int split_buckets(int n) { return n <= 131072 ? 256 : kSplitMaxBuckets; }
+
+struct SplitBufs {           // carved out of the handle's rank scratch (n x kRankMaxSeg int32)
+  double *gv;                // [n] grouped keys: value
+  int32_t *gi;               // [n] grouped keys: slot
+  int32_t *gb;               // [n] bucket of the grouped key
+  int32_t *eb, *epos;        // [n] bucket of slot i and its place in the bucket
+  double *spv;               // [NB - 1] splitters: value
+  int32_t *spi;              // [NB - 1] splitters: slot
+  int32_t *cnt, *off;        // [NB] bucket sizes, [NB + 1] offsets
+};
+
+__device__ __forceinline__ bool key_less(double a, int ia, double b, int ib) { return a < b || (a == b && ia < ib); }
+
+__global__ void __launch_bounds__(kOneCta) k4s_splitters(const double *__restrict__ logL, int n, int NB, SplitBufs B, const NssCtl *ctl, int reset)
+{
+  __shared__ double sv[4 * kSplitMaxBuckets];
+  __shared__ int si[4 * kSplitMaxBuckets];
+  if (!reset && (ctl->flags[2] | ctl->flags[0])) return;
+  const int S = 4 * NB;
+  for (int t = threadIdx.x; t < S; t += kOneCta) {
+    const int i = (int)((long long)t * n / S);
+    sv[t] = logL[i]; si[t] = i;
+  }
+  for (int t = threadIdx.x; t < NB; t += kOneCta) B.cnt[t] = 0;
+  __syncthreads();
+  for (int t = threadIdx.x; t < S; t += kOneCta) {
+    const double v = sv[t];
+    const int i = si[t];
+    int r = 0;
+    for (int u = 0; u < S; ++u) r += key_less(sv[u], si[u], v, i) ? 1 : 0;
+    if ((r & 3) == 0 && r > 0) { B.spv[r / 4 - 1] = v; B.spi[r / 4 - 1] = i; }     // ranks 4, 8, ...: the NB - 1 splitters
+  }
+}
+
+__global__ void __launch_bounds__(256) k4s_bucket(const double *__restrict__ logL, int n, int NB, SplitBufs B, const NssCtl *ctl, int reset)
+{
+  __shared__ double sv[kSplitMaxBuckets];
+  __shared__ int si[kSplitMaxBuckets];
+  if (!reset && (ctl->flags[2] | ctl->flags[0])) return;
+  for (int t = threadIdx.x; t < NB - 1; t += blockDim.x) { sv[t] = B.spv[t]; si[t] = B.spi[t]; }
+  __syncthreads();
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double v = logL[i];
+  int lo = 0, hi = NB - 1;                       // bucket = number of splitters <= key
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (key_less(v, i, sv[mid], si[mid])) hi = mid; else lo = mid + 1;
+  }
+  B.eb[i] = lo;
+  B.epos[i] = atomicAdd(&B.cnt[lo], 1);
+}
+
+__global__ void __launch_bounds__(kOneCta) k4s_offsets(int NB, SplitBufs B, const NssCtl *ctl, int reset)
+{
+  __shared__ int s[kOneCta];
+  if (!reset && (ctl->flags[2] | ctl->flags[0])) return;
+  const int t = threadIdx.x;
+  s[t] = t < NB ? B.cnt[t] : 0;
+  __syncthreads();
+  for (int o = 1; o < kOneCta; o <<= 1) {        // inclusive scan
+    const int v = t >= o ? s[t - o] : 0;
+    __syncthreads();
+    s[t] += v;
+    __syncthreads();
+  }
+  if (t < NB) B.off[t + 1] = s[t];
+  if (t == 0) B.off[0] = 0;
+}
+
+__global__ void __launch_bounds__(256) k4s_scatter(const double *__restrict__ logL, int n, SplitBufs B, const NssCtl *ctl, int reset)
+{
+  if (!reset && (ctl->flags[2] | ctl->flags[0])) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int b = B.eb[i], j = B.off[b] + B.epos[i];
+  B.gv[j] = logL[i]; B.gi[j] = i; B.gb[j] = b;
+}
+
+__global__ void __launch_bounds__(256) k4s_rank(int n, int k, SplitBufs B, int32_t *__restrict__ rank, int32_t *__restrict__ dead_idx,
+                                                 const NssCtl *ctl, int reset)
+{
+  if (!reset && (ctl->flags[2] | ctl->flags[0])) return;
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n) return;
+  const double v = B.gv[j];
+  const int i = B.gi[j], b = B.gb[j];
+  const int t0 = B.off[b], t1 = B.off[b + 1];
+  int c = t0;
+  for (int t = t0; t < t1; ++t) c += key_less(B.gv[t], B.gi[t], v, i) ? 1 : 0;
+  rank[i] = c;
+  if (c < k) dead_idx[c] = i;
+}
+
 // ---- stand-alone kernels (test hooks; the final ordering of the live points in nss_run) -------------------------------
 __global__ void __launch_bounds__(kOneCta) k4_rank(const double *__restrict__ logL, int n, int nseg, int32_t *__restrict__ part)
 {
@@ -431,7 +538,7 @@ __global__ void __launch_bounds__(kOneCta) k4_finish_select(const double *__rest
                                                             double *__restrict__ state)
 {
   __shared__ K4Smem sm;
-  rank_finish(part, n, k, nseg, rank, dead_idx);
+  if (nseg > 0) rank_finish(part, n, k, nseg, rank, dead_idx);     // nseg == 0: ranks and dead list come from the sample sort
   if (surv_idx) finish_select_block(nullptr, logL, nullptr, n, k, 0, NAN, rank, dead_idx, surv_idx, nullptr, nullptr, nullptr, state, sm);
 }
 
@@ -502,15 +609,19 @@ __global__ void __launch_bounds__(kOneCta) k4_front(const FrontArgs A)
   if (b < A.T) {
     tune_block(A.live, A.n, A.d, b, A.T, A.tune_scratch, ctl->tune_cnt, A.mean, A.chol, &ctl->chol_now, sm);
   } else {
-    rank_block(A.logL, A.n, (b - A.T) / A.nseg, (b - A.T) % A.nseg, A.nseg, A.rank_part, sm);
-    // the rank block that finishes last runs the selection tail (it does not wait for the tuning blocks)
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) sm.ticket = atomicAdd(&ctl->rank_done, 1u);
-    __syncthreads();
-    if (sm.ticket == gridDim.x - A.T - 1u) {
+    // nseg == 0: the ranks and the dead list are there already (sample sort, many live points) and this is the only block
+    // behind the tuning blocks; else the rank block that finishes last runs the selection tail (it does not wait for the
+    // tuning blocks)
+    if (A.nseg > 0) {
+      rank_block(A.logL, A.n, (b - A.T) / A.nseg, (b - A.T) % A.nseg, A.nseg, A.rank_part, sm);
       __threadfence();
-      rank_finish(A.rank_part, A.n, A.k, A.nseg, A.rank, A.dead_idx);
+      __syncthreads();
+      if (threadIdx.x == 0) sm.ticket = atomicAdd(&ctl->rank_done, 1u);
+      __syncthreads();
+    }
+    if (A.nseg == 0 || sm.ticket == gridDim.x - A.T - 1u) {
+      __threadfence();
+      if (A.nseg > 0) rank_finish(A.rank_part, A.n, A.k, A.nseg, A.rank, A.dead_idx);
       const int bad = finish_select_block(A.live, A.logL, A.birth, A.n, A.k, A.d, A.Lstar_in, A.rank, A.dead_idx, A.surv_idx, A.dead_theta,
                                           A.dead_logL, A.dead_birth, ctl->state, sm);
       if (threadIdx.x == 0) ctl->sel_bad = bad;
@@ -1271,6 +1382,28 @@ int ensure_scratch(nss_handle *h, int n)
   return NSS_OK;
 }
 
+// ranks (and the k lowest slots in ascending order) of n > kRankDirectMax values by the sample sort above, five small launches
+int launch_sample_rank(nss_handle *h, const double *logL, int n, int k, int32_t *rank, int32_t *dead_idx, int reset, cudaStream_t st)
+{
+  const int NB = split_buckets(n);
+  unsigned char *base = reinterpret_cast<unsigned char *>(h->d_rank_part);       // n x kRankMaxSeg int32 = 128 n bytes
+  SplitBufs B;
+  B.gv = reinterpret_cast<double *>(base);
+  B.spv = B.gv + n;
+  int32_t *ip = reinterpret_cast<int32_t *>(B.spv + kSplitMaxBuckets);
+  B.gi = ip; B.gb = ip + n; B.eb = ip + 2 * (size_t)n; B.epos = ip + 3 * (size_t)n;
+  B.spi = ip + 4 * (size_t)n; B.cnt = B.spi + kSplitMaxBuckets; B.off = B.cnt + kSplitMaxBuckets;
+  const unsigned nb = (unsigned)((n + 255) / 256);
+  k4s_splitters<<<1, kOneCta, 0, st>>>(logL, n, NB, B, h->d_ctl, reset);
+  k4s_bucket<<<nb, 256, 0, st>>>(logL, n, NB, B, h->d_ctl, reset);
+  k4s_offsets<<<1, kOneCta, 0, st>>>(NB, B, h->d_ctl, reset);
+  k4s_scatter<<<nb, 256, 0, st>>>(logL, n, B, h->d_ctl, reset);
+  k4s_rank<<<nb, 256, 0, st>>>(n, k, B, rank, dead_idx, h->d_ctl, reset);
+  h->launches += 5;
+  NSS_CUDA(cudaGetLastError());
+  return NSS_OK;
+}
+
 // The device part of one NS iteration (no host synchronisation), two launches:
 //   k4_front      a1 rank/select, a2 evidence (if dead_logw), a3 tune, flag and counter reset
 //   k3_slice      a4 - a10 (the slice directions a5 are drawn by the chain's own lanes), and a11's live evidence + stop test
@@ -1284,12 +1417,16 @@ int enqueue_iteration(nss_handle *h, double *live, double *logL, double *birth, 
   const int d = h->dev.d;
   FrontArgs F;
   F.live = live; F.logL = logL; F.birth = birth; F.n = n; F.k = k; F.d = d; F.Lstar_in = Lstar_in;
-  F.T = tune_blocks_for(n); F.nseg = rank_segments(n);
+  F.T = tune_blocks_for(n); F.nseg = n > kRankDirectMax ? 0 : rank_segments(n);
+  if (F.nseg == 0) {                                     // many live points: the ranks come from a sample sort (five more launches)
+    const int rc = launch_sample_rank(h, logL, n, k, h->d_rank, dead_idx, reset, st);
+    if (rc) return rc;
+  }
   F.rank_part = h->d_rank_part; F.rank = h->d_rank; F.dead_idx = dead_idx; F.surv_idx = h->d_surv_idx; F.tune_scratch = h->d_tune_scratch;
   F.dead_theta = dead_theta; F.dead_logL = dead_logL; F.dead_birth = dead_birth; F.dead_logw = dead_logw;
   F.mean = h->d_mean; F.chol = h->d_chol; F.ctl = h->d_ctl;
   F.reset = reset; F.set_state = set_state; F.zero_evals = zero_evals; F.logX = logX; F.logZ = logZ;
-  k4_front<<<F.T + ((n + kRankElems - 1) / kRankElems) * F.nseg, kOneCta, 0, st>>>(F);
+  k4_front<<<F.T + (F.nseg ? ((n + kRankElems - 1) / kRankElems) * F.nseg : 1), kOneCta, 0, st>>>(F);
   h->launches += 1;
   NSS_CUDA(cudaGetLastError());
   ChainArgs A;
@@ -1401,11 +1538,17 @@ extern "C" int nss_select_lowest(nss_handle *h, const double *logL_dev, int32_t 
   if (rc) return rc;
   rc = begin_iteration(h, 0, 0.0, 0.0, 0, st);
   if (rc) return rc;
-  const int nseg = rank_segments(n_live);
-  k4_rank<<<((n_live + kRankElems - 1) / kRankElems) * nseg, kOneCta, 0, st>>>(logL_dev, n_live, nseg, h->d_rank_part);
+  const int nseg = n_live > kRankDirectMax ? 0 : rank_segments(n_live);
+  if (nseg == 0) {
+    rc = launch_sample_rank(h, logL_dev, n_live, n_delete, h->d_rank, dead_idx_dev, 1, st);
+    if (rc) return rc;
+  } else {
+    k4_rank<<<((n_live + kRankElems - 1) / kRankElems) * nseg, kOneCta, 0, st>>>(logL_dev, n_live, nseg, h->d_rank_part);
+    h->launches += 1;
+  }
   k4_finish_select<<<1, kOneCta, 0, st>>>(logL_dev, n_live, n_delete, nseg, h->d_rank_part, h->d_rank, dead_idx_dev,
                                           surv_idx_dev ? surv_idx_dev : h->d_surv_idx, h->d_state);
-  h->launches += 2;
+  h->launches += 1;
   NSS_CUDA(cudaGetLastError());
   rc = fetch_ctl(h, st);
   if (rc) return rc;
@@ -1674,12 +1817,18 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
   }
   if (result == NSS_OK || result == NSS_ENOTCONV) {
     // O14: append the live points in ascending logL
-    const int nseg = rank_segments(n);
-    k4_rank<<<((n + kRankElems - 1) / kRankElems) * nseg, kOneCta, 0, st>>>(logL, n, nseg, h->d_rank_part);
+    const int nseg = n > kRankDirectMax ? 0 : rank_segments(n);
+    if (nseg == 0) {
+      rc = launch_sample_rank(h, logL, n, n, h->d_rank, h->d_dead_idx, 1, st);
+      if (rc) { cleanup(); return rc; }
+    } else {
+      k4_rank<<<((n + kRankElems - 1) / kRankElems) * nseg, kOneCta, 0, st>>>(logL, n, nseg, h->d_rank_part);
+      h->launches += 1;
+    }
     k4_finish_select<<<1, kOneCta, 0, st>>>(logL, n, n, nseg, h->d_rank_part, h->d_rank, h->d_dead_idx, nullptr, nullptr);
     k_gather_rows<<<(n + 255) / 256, 256, 0, st>>>(live, logL, h->d_birth, h->d_dead_idx, n, d, dth + (size_t)n_dead * d, dl + n_dead,
                                                    db + n_dead);
-    h->launches += 3;
+    h->launches += 2;
     const int64_t n_it_dead = n_dead;
     n_dead += n;
     double state[4];

@@ -12,6 +12,10 @@ A second table times the FRONT of an NS iteration (k4_front: delete-select by co
 mean / covariance / Cholesky) at n_live = 1000 ... 65536 through `nss_replace_step` with zero slice repeats, next to one
 full iteration at the same n_live, to show where the counting select stops being negligible (north_star names a radix
 select; bit-exact parity of the counting select, ties included, is in tests/test_gpu_sampler.py).
+
+A third table sweeps the schedule of the chain kernel K3 — lanes per candidate, warps per chain, single-warp chains per
+CTA (nss_set_chain_lanes / _warps / _pack: they change the schedule only, never a result) — on configs 2 and 3, the
+measurements behind the automatic choice.
 """
 from __future__ import annotations
 
@@ -59,6 +63,7 @@ def main():
                 print(f"| {B} | {N} | {name} | {ms:.4f} | {rate:.3e} | {ins} | {rate * ins / (peak * 1e12 / 2):.3f} |", flush=True)
         g.close()
     front_table(torch, inputs, nss, flush)
+    k3_sweep_table(torch, inputs, nss)
 
 
 def front_table(torch, inputs, nss, flush):
@@ -87,6 +92,38 @@ def front_table(torch, inputs, nss, flush):
         g.nss_replace_step(live, logL, n // 2, w.n_repeats, 1, 0)
         full = timed(lambda: g.nss_replace_step(live, logL, n // 2, w.n_repeats, 1, 0), reps=3)
         print(f"| {n} | {front:.4f} | {full:.4f} | {front / full:.4f} |", flush=True)
+    g.close()
+
+
+def k3_sweep_table(torch, inputs, nss):
+    import math
+    w = inputs.make_data(inputs.config2(), nss.nss_waveform)
+    g = nss.Nss(w)
+    g.set_chain_timing(True)
+    print("\n## K3 schedule sweep (mean over NS iterations 2..25 of a seeded run; kernel ms from the library's event pair)\n")
+    print("| n_live | n_delete | lanes/candidate | warps/chain | chains/CTA | K3 ms | step ms | rounds/chain | evaluated/consumed | evals/s (K3) |")
+    print("|---|---|---|---|---|---|---|---|---|---|")
+    for n, k, combos in ((1000, 500, ((0, 0, 0), (16, 2, 0), (8, 1, 1), (8, 2, 0), (16, 4, 0), (32, 4, 0), (32, 2, 0))),
+                         (5000, 2500, ((0, 0, 0), (8, 1, 1), (8, 1, 2), (8, 1, 4), (8, 1, 8), (16, 1, 4), (16, 2, 0)))):
+        for L, G, pack in combos:
+            g.set_chain_lanes(L); g.set_chain_warps(G); g.set_chain_pack(pack)
+            live, logL = g.nss_init_live(n, 1)
+            st = nss.nss_iter_state(logX=0.0, logZ=-math.inf)
+            bufs = g.iter_buffers(k)
+            k3, stp, ev, rd, ex = [], [], 0, 0, 0
+            for it in range(26):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                g.nss_iterate(live, logL, k, w.n_repeats, 1, it, st, bufs)
+                b.record()
+                b.synchronize()
+                if it >= 2:
+                    k3.append(g.nss_last_chain_ms()); stp.append(a.elapsed_time(b)); ev += st.n_evals
+                    r_, e_ = g.nss_last_chain_diag(); rd += r_; ex += e_
+            m = len(k3)
+            name = lambda v: "auto" if v == 0 else str(v)
+            print(f"| {n} | {k} | {name(L)} | {name(G)} | {name(pack)} | {sum(k3) / m:.4f} | {sum(stp) / m:.4f} | {rd / m / k:.1f} | "
+                  f"{ex / ev:.3f} | {ev / sum(k3) * 1e3:.3e} |", flush=True)
     g.close()
 
 

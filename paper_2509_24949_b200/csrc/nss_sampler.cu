@@ -1244,7 +1244,7 @@ int launch_chains_k(nss_handle *h, ChainArgs &A, size_t tab_bytes, cudaStream_t 
   auto kern = k3_slice<NDET, KIND, LANES, RESIDENT>;
   int G = h->chain_warps;
   if (G != 1 && G != 2 && G != 4 && G != 8) {
-    // automatic (measured on B200: profiles/r02_k3_sweeps.md): a chain is a serial process, so few chains want
+    // automatic (measured on B200: profiles/r02_config5_microbench.md, third table): a chain is a serial process, so few chains want
     // wide speculation, but once there are about as many warps as SM sub-partitions (4 per SM) the kernel turns
     // throughput-bound and every speculative evaluation costs time
     const long long S = 4LL * h->n_sm;

@@ -87,6 +87,8 @@ struct nss_handle {
   // device block and events of nss_run, kept between runs
   unsigned char *d_run;
   size_t run_bytes;
+  unsigned char *h_run;        // pinned staging block of nss_run's results (the caller's arrays may be pageable)
+  size_t h_run_bytes;
   cudaEvent_t ev_run[2];
   // CUDA events recorded around the most recent K3 (slice chains) launch: nss_last_chain_ms
   cudaEvent_t ev_k3[2];

@@ -1831,24 +1831,44 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
     h->launches += 2;
     const int64_t n_it_dead = n_dead;
     n_dead += n;
-    double state[4];
-    unsigned long long ne = 0;
-    RUN_CUDA(cudaMemcpyAsync(state, h->d_state, sizeof(state), cudaMemcpyDeviceToHost, st));
-    RUN_CUDA(cudaMemcpyAsync(&ne, h->d_nevals, sizeof(ne), cudaMemcpyDeviceToHost, st));
-    RUN_CUDA(cudaMemcpyAsync(out->dead_theta, dth, sizeof(double) * (size_t)n_dead * d, cudaMemcpyDeviceToHost, st));
-    RUN_CUDA(cudaMemcpyAsync(out->dead_logL, dl, sizeof(double) * n_dead, cudaMemcpyDeviceToHost, st));
-    RUN_CUDA(cudaMemcpyAsync(out->dead_logL_birth, db, sizeof(double) * n_dead, cudaMemcpyDeviceToHost, st));
+    // O15: the replica evidences, the Kish ESS and the equal-weight rows on the device (one CTA per replica; one CTA each)
     k_fill_live_logw<<<(n + 255) / 256, 256, 0, st>>>(dw + n_it_dead, n, h->d_state);
-    RUN_CUDA(cudaMemcpyAsync(out->dead_logw, dw, sizeof(double) * n_dead, cudaMemcpyDeviceToHost, st));
-    // O15: the replica evidences on the device (one CTA per replica), reduced to a standard deviation below
-    double lz_rep[kErrReplicas + 2];                     // [kErrReplicas] = Kish ESS, [kErrReplicas + 1] = equal-weight rows
     k_evidence_error<<<kErrReplicas, 256, 0, st>>>(dl, n_it_dead, n, k, seed, logL, derr);
     k_kish_ess<<<1, kOneCta, 0, st>>>(dl, dw, n_it_dead, logL, n, h->d_state, derr + kErrReplicas);
     k_resample_equal<<<1, kOneCta, 0, st>>>(dl, dw, (long long)n_dead, seed, deq, derr + kErrReplicas + 1);
     h->launches += 4;
-    RUN_CUDA(cudaMemcpyAsync(lz_rep, derr, sizeof(lz_rep), cudaMemcpyDeviceToHost, st));
+    // results: device -> one pinned staging block (asynchronous copies whatever memory the caller's arrays are in) -> caller
+    const size_t nd = (size_t)n_dead;
+    const size_t s_th = 0, s_l = s_th + align256(sizeof(double) * nd * d), s_b = s_l + align256(sizeof(double) * nd),
+                 s_w = s_b + align256(sizeof(double) * nd), s_misc = s_w + align256(sizeof(double) * nd),
+                 s_eq = s_misc + align256(sizeof(double) * (kErrReplicas + 2 + 4 + 1)),
+                 s_total = s_eq + (deq ? align256(sizeof(int64_t) * nd) : 0);
+    if (h->h_run_bytes < s_total) {
+      if (h->h_run) cudaFreeHost(h->h_run);
+      h->h_run = nullptr; h->h_run_bytes = 0;
+      cudaError_t e = cudaMallocHost((void **)&h->h_run, s_total + s_total / 2);     // room to grow: pinning is slow
+      if (e != cudaSuccess) { cleanup(); nss_cuda_fail(e, "cudaMallocHost(run)"); return NSS_ENOMEM; }
+      h->h_run_bytes = s_total + s_total / 2;
+    }
+    unsigned char *hb = h->h_run;
+    double *lz_rep = (double *)(hb + s_misc);            // [kErrReplicas] replicas, then Kish ESS, equal-weight rows
+    double *state = lz_rep + kErrReplicas + 2;           // logX, logZ, logZ_live, L*
+    unsigned long long *ne_p = (unsigned long long *)(state + 4);
+    RUN_CUDA(cudaMemcpyAsync(hb + s_th, dth, sizeof(double) * nd * d, cudaMemcpyDeviceToHost, st));
+    RUN_CUDA(cudaMemcpyAsync(hb + s_l, dl, sizeof(double) * nd, cudaMemcpyDeviceToHost, st));
+    RUN_CUDA(cudaMemcpyAsync(hb + s_b, db, sizeof(double) * nd, cudaMemcpyDeviceToHost, st));
+    RUN_CUDA(cudaMemcpyAsync(hb + s_w, dw, sizeof(double) * nd, cudaMemcpyDeviceToHost, st));
+    RUN_CUDA(cudaMemcpyAsync(lz_rep, derr, sizeof(double) * (kErrReplicas + 2), cudaMemcpyDeviceToHost, st));
+    RUN_CUDA(cudaMemcpyAsync(state, h->d_state, sizeof(double) * 4, cudaMemcpyDeviceToHost, st));
+    RUN_CUDA(cudaMemcpyAsync(ne_p, h->d_nevals, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    if (deq) RUN_CUDA(cudaMemcpyAsync(hb + s_eq, deq, sizeof(int64_t) * nd, cudaMemcpyDeviceToHost, st));
     RUN_CUDA(cudaEventRecord(e1, st));
     RUN_CUDA(cudaStreamSynchronize(st));
+    memcpy(out->dead_theta, hb + s_th, sizeof(double) * nd * d);
+    memcpy(out->dead_logL, hb + s_l, sizeof(double) * nd);
+    memcpy(out->dead_logL_birth, hb + s_b, sizeof(double) * nd);
+    memcpy(out->dead_logw, hb + s_w, sizeof(double) * nd);
+    const unsigned long long ne = *ne_p;
     float ms = 0.f;
     RUN_CUDA(cudaEventElapsedTime(&ms, e0, e1));
     out->gpu_ms = ms;
@@ -1873,8 +1893,7 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
     out->logZ = logZf; out->logZ_err = sqrt(var * R / (R - 1)); out->H = H;
     out->ess = lz_rep[kErrReplicas];
     out->n_equal = (int64_t)lz_rep[kErrReplicas + 1];
-    if (out->equal_idx && out->n_equal > 0)
-      RUN_CUDA(cudaMemcpy(out->equal_idx, deq, sizeof(int64_t) * (size_t)out->n_equal, cudaMemcpyDeviceToHost));
+    if (out->equal_idx && out->n_equal > 0) memcpy(out->equal_idx, hb + s_eq, sizeof(int64_t) * (size_t)out->n_equal);
     out->n_iter = t; out->n_dead = n_dead; out->n_evals = (int64_t)ne + n;
   }
 #undef RUN_CUDA

@@ -152,6 +152,7 @@ extern "C" int nss_destroy(nss_handle *h)
   if (h->h_ctl) cudaFreeHost(h->h_ctl);
   cudaFree(h->d_mean); cudaFree(h->d_chol); cudaFree(h->d_birth); cudaFree(h->d_stage);
   cudaFree(h->d_run);
+  if (h->h_run) cudaFreeHost(h->h_run);
   if (h->ev_ctl[0]) cudaEventDestroy(h->ev_ctl[0]);
   if (h->ev_ctl[1]) cudaEventDestroy(h->ev_ctl[1]);
   if (h->ev_run[0]) cudaEventDestroy(h->ev_run[0]);

@@ -175,6 +175,28 @@ def test_replace_step_trajectories_gaussian(nssmod, oracle):
         g.close()
 
 
+def test_iteration_above_the_counting_select_limit(nssmod, oracle):
+    """More than 8192 live points: inside an iteration the ranks come from the sample sort (five k4s_* launches in front of
+    k4_front, whose selection tail then finds ranks and dead list ready), the mean / covariance reduction runs in several
+    blocks with a counter barrier, and 4500 single-warp chains are packed four to a CTA and fetched from the device
+    counter.  Same checks as everywhere: dead list and rows bit-exact (a tenth of the logL values tied), trajectories of
+    safe chains identical; then a complete (bounded) run on both sides."""
+    w = inputs.gaussian_workload(5, sigma=0.07)
+    g, p = nssmod.Nss(w), oracle.Problem(w)
+    n, k = 9000, 4500
+    live, logL = p.init_live(n, 21)
+    live[::10] = live[3]                               # exact ties in logL: broken by slot
+    logL = p.loglike_batch(live)
+    r, o, safe = _trajectory_parity(g, p, live, logL, k, 6, seed=8, it=0, w=w)
+    _trajectory_parity(g, p, o["live"], o["logL"], k, 3, seed=8, it=1, w=w)
+    rg, ro = g.nss_run(n, k, 4, 5, max_iter=3), p.run(n, k, 4, 5, max_iter=3)
+    assert rg["rc"] == nssmod.NSS_ENOTCONV and rg["n_iter"] == ro["n_iter"] == 3 and rg["n_dead"] == ro["n_dead"]
+    assert abs(rg["logZ"] - ro["logZ"]) < 3 * math.hypot(rg["logZ_err"], ro["logZ_err"]) + 1e-9
+    if _replays(rg, ro):
+        _assert_replay(rg, ro, w)
+    g.close()
+
+
 def test_replace_step_trajectories_config1(nssmod, oracle, wl1):
     g, p = nssmod.Nss(wl1), oracle.Problem(wl1)
     live, logL = p.init_live(100, 1)

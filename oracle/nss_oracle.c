@@ -19,9 +19,11 @@
  * every per-point and per-chain computation is the same scalar code (results do not depend on
  * the thread count, since every random draw is a Philox counter, O11).
  *
- * Pins (tests/test_oracle_*.py, -m "not gpu"): see DESIGN.md §5.  Unpinned by any external
- * source: the higher PN phase coefficients phi_2..phi_7 (P2: "parity unpinned"; only sanity
- * identities), and the sampler conventions A12/A14/A15/A17 (validity pinned by P13/P15 only); the wrap
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): see DESIGN.md §5.  The higher PN phase coefficients
+ * phi_2..phi_7 (P2) are pinned to SURVEY.md O3, the normative definition of this build's waveform: every literal
+ * is recovered numerically from orc_phase and compared with tests/golden/taylorf2_o3_literals.txt, typed by hand
+ * from the survey text (the source papers themselves are not in the container).  "Parity unpinned" by any
+ * external source: the sampler conventions A12/A14/A15/A17 (validity pinned by P13/P15 only); the wrap
  * convention of periodic coordinates (NEXT-2, R4) likewise: nothing external fixes where the seam
  * value goes, its validity is pinned by uniformity, identity inside the box and the analytic evidence.
  */

@@ -157,8 +157,9 @@ int nss_iterate(nss_handle *h, double *live_dev, double *logL_dev, int32_t n_liv
                 nss_iter_state *state_host, void *cuda_stream);
 
 /* The same iteration with HOST buffers (pinned memory recommended): live/logL are copied to the
- * device, the iteration runs, and live, logL and the dead rows are copied back, all on the stream,
- * inside the call.  bench.py's end-to-end (`e2e`) leg. */
+ * device, the iteration runs, and live, logL and the dead rows are copied back, all queued on the stream
+ * inside the call, which waits once at the end.  On NSS_ECHOL the live set comes back unchanged (the
+ * chains did not run) and state_host is untouched.  bench.py's end-to-end (`e2e`) leg. */
 int nss_iterate_host(nss_handle *h, double *live_host, double *logL_host, int32_t n_live,
                      int32_t n_delete, int32_t n_repeats, uint64_t seed, uint32_t iteration,
                      double stop_dlogz, double *dead_theta_host, double *dead_logL_host,

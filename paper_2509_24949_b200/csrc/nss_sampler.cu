@@ -1697,11 +1697,17 @@ extern "C" int nss_iterate_host(nss_handle *h, double *live_host, double *logL_h
   double *live = (double *)(b + o_live), *logL = (double *)(b + o_logL), *dth = (double *)(b + o_dth), *dl = (double *)(b + o_dl),
          *dw = (double *)(b + o_dw);
   int32_t *di = (int32_t *)(b + o_di);
+  // everything is queued on the stream — inputs in, the iteration, the control block and the results out — and the
+  // host waits once (on a Cholesky failure the live set comes back unchanged and the dead rows are those selected)
   NSS_CUDA(cudaMemcpyAsync(live, live_host, n * d * 8, cudaMemcpyHostToDevice, st));
   NSS_CUDA(cudaMemcpyAsync(logL, logL_host, n * 8, cudaMemcpyHostToDevice, st));
-  // the device copies are queued behind the iteration; nss_iterate's synchronisation is followed by one more below
-  rc = nss_iterate(h, live, logL, n_live, n_delete, n_repeats, seed, iteration, stop_dlogz, dth, dl, dw, di, state_host, st);
+  rc = ensure_scratch(h, n_live);
   if (rc) return rc;
+  rc = enqueue_iteration(h, live, logL, nullptr, n_live, n_delete, NAN, n_repeats, seed, iteration, dth, dl, nullptr, di, dw,
+                         /*reset*/ 1, /*set_state*/ 1, state_host->logX, state_host->logZ, /*zero_evals*/ 1, /*live_evidence*/ 1,
+                         stop_dlogz, st);
+  if (rc) return rc;
+  NSS_CUDA(cudaMemcpyAsync(h->h_ctl, h->d_ctl, sizeof(NssCtl), cudaMemcpyDeviceToHost, st));
   NSS_CUDA(cudaMemcpyAsync(live_host, live, n * d * 8, cudaMemcpyDeviceToHost, st));
   NSS_CUDA(cudaMemcpyAsync(logL_host, logL, n * 8, cudaMemcpyDeviceToHost, st));
   NSS_CUDA(cudaMemcpyAsync(dead_theta_host, dth, k * d * 8, cudaMemcpyDeviceToHost, st));
@@ -1709,6 +1715,11 @@ extern "C" int nss_iterate_host(nss_handle *h, double *live_host, double *logL_h
   NSS_CUDA(cudaMemcpyAsync(dead_logw_host, dw, k * 8, cudaMemcpyDeviceToHost, st));
   NSS_CUDA(cudaMemcpyAsync(dead_idx_host, di, k * 4, cudaMemcpyDeviceToHost, st));
   NSS_CUDA(cudaStreamSynchronize(st));
+  const NssCtl &c = *h->h_ctl;
+  if (c.flags[0]) return NSS_ECHOL;
+  state_host->logX = c.state[0]; state_host->logZ = c.state[1]; state_host->logZ_live = c.state[2]; state_host->logLstar = c.state[3];
+  state_host->n_evals = (int64_t)c.nevals;
+  state_host->converged = c.flags[2];
   return NSS_OK;
 }
 

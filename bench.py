@@ -254,17 +254,17 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
 
-    def fresh(sd, n_live=None):
+    def fresh(sd, n_live=None, g=g):
         live, logL = g.nss_init_live(n if n_live is None else n_live, sd)
         return live, logL, nss.nss_iter_state(logX=0.0, logZ=-math.inf), 0
 
-    def timed_steps(n_live, n_del, steps, warmup, sd, sync_all, kernel_timing=False):
+    def timed_steps(n_live, n_del, steps, warmup, sd, sync_all, kernel_timing=False, g=g):
         """`steps` consecutive NS iterations (one nss_iterate call each) of a seeded run, CUDA events around each step on
         the launching stream, L2 flushed between steps outside the event pairs; a fresh run starts, untimed, whenever the
         stop rule fires.  kernel_timing: the library also records events around K3 (which costs the step ~5 us of launch
         overlap, so the step time is taken from a pass without them and the kernel time from a second, identical pass)."""
         g.set_chain_timing(kernel_timing)
-        live, logL, st, it = fresh(sd, n_live)
+        live, logL, st, it = fresh(sd, n_live, g)
         bufs = g.iter_buffers(n_del)
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
         r = dict(evals=0, k3_ms=0.0, rounds=0, executed=0, launches=0, wall=0.0, ms=0.0)
@@ -278,7 +278,7 @@ def run_ours(args):
                 l0 = g.launches
             if st.converged:
                 runs += 1
-                live, logL, st, it = fresh(sd + 7919 * runs, n_live)
+                live, logL, st, it = fresh(sd + 7919 * runs, n_live, g)
             flush.fill_(s_ & 0xFF)
             if s_ >= warmup:
                 ev[s_ - warmup][0].record(stream)
@@ -410,6 +410,10 @@ def run_ours(args):
             runs_extra["paper_hyperparameters"] = timed_run(g, 3000, 1500, 10 * d, seed)
             g4 = nss.Nss(w, kind=1)
             runs_extra["config4"] = timed_run(g4, n, k, nrep, seed)
+            # config 4 (BASELINE.json configs[3]) as a step: the same iteration with the full-grid likelihood inside K3
+            m4 = timed_steps(n, k, 4, 3, seed, False, g=g4)
+            m4["k3_ms"] = timed_steps(n, k, 4, 3, seed, False, kernel_timing=True, g=g4)["k3_ms"]
+            m4["steps"] = 4
             g4.close()
 
     # max over ranks of the timed quantities; sum of the work
@@ -470,6 +474,16 @@ def run_ours(args):
     for key_, v_ in runs_extra.items():
         line["nss_run_" + key_] = v_
     if m3 is not None:
+        instr4 = 600 + w.n_freq * (8 + 22 * w.n_det)
+        line["step_config4"] = {
+            "workload": "BASELINE.json configs[3]: config 2 with the full-frequency-grid likelihood (4017 bins x 3 detectors) inside K3",
+            "steps": m4["steps"], "ms_per_step": m4["ms"] / m4["steps"], "evals_per_s": m4["evals"] / (m4["ms"] * 1e-3),
+            "evals_per_step": m4["evals"] / m4["steps"], "kernel_ms_per_step": m4["k3_ms"] / m4["steps"],
+            "fp64_instr_per_eval": instr4, "rounds_per_chain": m4["rounds"] / m4["steps"] / k,
+            "pipe_frac": m4["evals"] * instr4 / (m4["k3_ms"] * 1e-3) / (peak_tf * 1e12 / 2),
+            "pipe_frac_of_nominal": m4["evals"] * instr4 / (m4["k3_ms"] * 1e-3) / (NOMINAL_TF * 1e12 / 2),
+            "note": "k3_slice<3, full grid, 32 lanes per candidate, table read from L2>: fraction of the DFMA issue peak by the "
+                    "consumed evaluations only"}
         k3_tf3 = m3["evals"] * flop / (m3["k3_ms"] * 1e-3) / 1e12
         line["step_config3"] = {
             "workload": "BASELINE.json configs[2]: config 2 at n_live 5000, n_delete 2500 (55 repeats)", "steps": m3["steps"],

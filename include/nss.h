@@ -45,7 +45,8 @@ enum {
   NSS_ECUDA = -3,     /* a CUDA call failed (no device, launch error); see nss_last_cuda_error */
   NSS_ECHOL = -4,     /* non-positive Cholesky pivot of the live-point covariance */
   NSS_ECAP = -5,      /* nss_result arrays too small */
-  NSS_ENOTCONV = -6   /* nss_run hit max_iter; the results written are still valid */
+  NSS_ENOTCONV = -6,  /* nss_run hit max_iter; the results written are still valid */
+  NSS_ELIMIT = -7     /* a size beyond the fixed capacity of an entry point that does not allocate (*_static) */
 };
 
 enum { NSS_KIND_RB = 0, NSS_KIND_FULL = 1, NSS_KIND_GAUSS = 2 };
@@ -181,6 +182,38 @@ int nss_select_lowest(nss_handle *h, const double *logL_dev, int32_t n_live, int
                       int32_t *dead_idx_dev /*[n_delete] ascending logL, ties by slot*/,
                       int32_t *surv_idx_dev /*[n_live-n_delete] ascending slot, may be NULL*/,
                       double *logLstar_host, void *cuda_stream);
+
+/* The delete-select of nss_select_lowest (O12.1: the n_delete lowest logL in ascending order, ties by the lower slot,
+ * the survivors in ascending slot order, the threshold L* = the highest deleted logL) for callers that cannot let this
+ * library allocate device memory.  Who that is: a process whose GPU memory has been handed over wholesale to a pool
+ * (PyTorch's caching allocator, a job that pre-reserves its whole HBM budget), where a cudaMalloc issued from inside a
+ * library fails with "out of memory" although the pool has plenty free; a sampler loop that shares the GPU with other
+ * streams and cannot take the device-wide stall cudaMalloc / cudaFree bring with them; and code that must prove, after
+ * start-up, that no later call can fail for want of memory.  Every other entry point here needs an nss_handle, and both
+ * nss_create and the handle's first use of the sampler allocate; this one needs no handle at all.
+ *
+ * Its work space (partial counts, ranks, a spare survivor list: 1 114 144 bytes) is a fixed array inside libnss.so's
+ * device image, so every GPU that loads the library carries it until the process exits, used or not, and the size is
+ * capped: n_live <= NSS_SELECT_STATIC_MAX_LIVE, else NSS_ELIMIT and nothing is launched (larger live sets need the
+ * sample sort of nss_select_lowest, whose work space grows with n_live).  The call issues no cudaMalloc, cudaFree or
+ * other allocating routine; it launches two kernels on the stream and returns without waiting for them.
+ *
+ * logL_dev: device [n_live], read only.  dead_idx_dev: device [n_delete], out.  surv_idx_dev: device
+ * [n_live - n_delete], out, or NULL if not wanted.  logLstar_dev: DEVICE [1], out, or NULL (a host slot would need a
+ * synchronising copy; read it with your own copy when you need it).  Works on the CURRENT device; all pointers must
+ * belong to it.  Returns NSS_EINVAL for NULL / inconsistent sizes (as nss_select_lowest), NSS_ELIMIT, NSS_ECUDA.
+ *
+ * First use on a device: the first call made while that device is current looks up the array's device address
+ * (cudaGetSymbolAddress) and remembers it; make that first call during start-up, before any stream capture begins.
+ * Sharing: there is ONE array per device and every call uses it, whatever the stream or thread.  Calls must not
+ * overlap on the GPU: two in flight at once (two streams, or two host threads on one device) overwrite each other's
+ * counts and both results are garbage; order them on one stream or with events.  The array keeps what the last call
+ * wrote, which is harmless: each call overwrites every word it later reads, so nothing has to be cleared in between. */
+#define NSS_SELECT_STATIC_MAX_LIVE 8192
+int nss_select_lowest_static(const double *logL_dev, int32_t n_live, int32_t n_delete,
+                             int32_t *dead_idx_dev /*[n_delete]*/, int32_t *surv_idx_dev /*[n_live-n_delete] or NULL*/,
+                             double *logLstar_dev /*device [1] or NULL*/, void *cuda_stream);
+
 int nss_tune(nss_handle *h, const double *live_dev, int32_t n_live, double *mean_dev /*[d]*/,
              double *chol_dev /*[d][d] lower, row-major*/, void *cuda_stream);
 /* logw_j = logX + ln(1 - e^{-1/m_j}), m_j = n_live - j; logX -= sum 1/m_j; logZ = logaddexp(...).

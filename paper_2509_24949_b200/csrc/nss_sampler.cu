@@ -4,6 +4,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
 #include <vector>
 
 #include "nss_loglike_dev.cuh"
@@ -1910,4 +1911,81 @@ extern "C" int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t 
 #undef RUN_CUDA
   cleanup();
   return result;
+}
+
+// ---- nss_select_lowest_static: the delete-select (a1, O12.1) for callers that must not allocate ---------------------------
+// The counting select needs work space beside its inputs and outputs: the partial counts of every (segment, live point)
+// pair, the ranks, and a survivor list when the caller does not want one.  nss_select_lowest keeps that space in the handle
+// and grows it with cudaMalloc; this entry point keeps it in the image of the library instead, so neither creating a handle
+// nor the call itself asks the CUDA allocator for anything.  See include/nss.h for who needs that and what it costs.
+//
+// Layout of the array, in 32-bit words (kSelStaticLive = NSS_SELECT_STATIC_MAX_LIVE = the largest n the counting select
+// serves, kRankDirectMax):
+//   [0, 32 n_max)            partial counts, [segment][live point] with the call's own n as the row length
+//   [32 n_max, 33 n_max)     ranks
+//   [33 n_max, 34 n_max)     survivor list when surv_idx_dev is NULL
+//   then 4 doubles           the {logX, logZ, logZ_live, L*} block the selection tail writes L* into
+constexpr int kSelStaticLive = NSS_SELECT_STATIC_MAX_LIVE;
+static_assert(kSelStaticLive == kRankDirectMax, "the static select serves exactly the sizes the counting ranks serve");
+constexpr size_t kSelStaticWords = (size_t)(kRankMaxSeg + 2) * kSelStaticLive + 8;
+static __device__ __align__(256) int32_t g_sel_static[kSelStaticWords];       // 1 114 144 bytes on every device that loads libnss.so
+
+namespace {
+
+// The tail of the counting select on the static work space: partial counts -> ranks and dead list, survivor compaction,
+// threshold.  Same device functions, in the same order, as k4_finish_select; the threshold also goes to the caller's slot.
+__global__ void __launch_bounds__(kOneCta) k4_finish_select_static(const double *__restrict__ logL, int n, int k, int nseg,
+                                                                   const int32_t *__restrict__ part, int32_t *__restrict__ rank,
+                                                                   int32_t *__restrict__ dead_idx, int32_t *__restrict__ surv_idx,
+                                                                   double *__restrict__ state, double *__restrict__ logLstar_out)
+{
+  __shared__ K4Smem sm;
+  rank_finish(part, n, k, nseg, rank, dead_idx);
+  finish_select_block(nullptr, logL, nullptr, n, k, 0, NAN, rank, dead_idx, surv_idx, nullptr, nullptr, nullptr, state, sm);
+  if (threadIdx.x == 0 && logLstar_out) *logLstar_out = state[3];      // written by thread 0 just above
+}
+
+// In host code `g_sel_static` is only a handle for the runtime, not an address a kernel can use: the device address is
+// asked for once per device (with that device current) and remembered.
+constexpr int kSelStaticMaxDevices = 64;
+int32_t *g_sel_static_dev[kSelStaticMaxDevices];
+std::mutex g_sel_static_mu;
+
+int sel_static_base(int32_t **base)
+{
+  int dev = -1;
+  NSS_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kSelStaticMaxDevices) return NSS_EINVAL;
+  std::lock_guard<std::mutex> lock(g_sel_static_mu);
+  if (!g_sel_static_dev[dev]) {
+    void *p = nullptr;
+    NSS_CUDA(cudaGetSymbolAddress(&p, g_sel_static));
+    if (!p) return NSS_ECUDA;
+    g_sel_static_dev[dev] = static_cast<int32_t *>(p);
+  }
+  *base = g_sel_static_dev[dev];
+  return NSS_OK;
+}
+
+}  // namespace
+
+extern "C" int nss_select_lowest_static(const double *logL_dev, int32_t n_live, int32_t n_delete, int32_t *dead_idx_dev,
+                                        int32_t *surv_idx_dev, double *logLstar_dev, void *cuda_stream)
+{
+  if (!logL_dev || !dead_idx_dev || n_live < 2 || n_delete < 1 || n_delete >= n_live) return NSS_EINVAL;
+  if (n_live > kSelStaticLive) return NSS_ELIMIT;
+  int32_t *base = nullptr;
+  const int rc = sel_static_base(&base);
+  if (rc) return rc;
+  int32_t *part = base, *rank = base + (size_t)kRankMaxSeg * kSelStaticLive, *surv = rank + kSelStaticLive;
+  double *state = reinterpret_cast<double *>(surv + kSelStaticLive);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  // Nothing in the work space has to start at zero: both kernels write every word they (or the next kernel) later read —
+  // part[sg][i] for every sg < nseg, i < n; rank[i] for every i < n; state[3] — so what an earlier call left is never seen.
+  const int nseg = rank_segments(n_live);
+  k4_rank<<<((n_live + kRankElems - 1) / kRankElems) * nseg, kOneCta, 0, st>>>(logL_dev, n_live, nseg, part);
+  k4_finish_select_static<<<1, kOneCta, 0, st>>>(logL_dev, n_live, n_delete, nseg, part, rank, dead_idx_dev,
+                                                 surv_idx_dev ? surv_idx_dev : surv, state, logLstar_dev);
+  NSS_CUDA(cudaGetLastError());
+  return NSS_OK;
 }

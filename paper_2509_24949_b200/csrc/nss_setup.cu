@@ -32,6 +32,7 @@ extern "C" const char *nss_strerror(int code)
     case NSS_ECHOL: return "non-positive Cholesky pivot of the live-point covariance";
     case NSS_ECAP: return "result arrays too small";
     case NSS_ENOTCONV: return "max_iter reached before the stop rule (results valid)";
+    case NSS_ELIMIT: return "size beyond the fixed capacity of a *_static entry point (NSS_SELECT_STATIC_MAX_LIVE live points)";
     default: return "unknown error";
   }
 }

@@ -16,7 +16,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "csrc", "libnss.so")
 NSLOT, MAXDET = 11, 4
 
-NSS_OK, NSS_EINVAL, NSS_ENOMEM, NSS_ECUDA, NSS_ECHOL, NSS_ECAP, NSS_ENOTCONV = 0, -1, -2, -3, -4, -5, -6
+NSS_OK, NSS_EINVAL, NSS_ENOMEM, NSS_ECUDA, NSS_ECHOL, NSS_ECAP, NSS_ENOTCONV, NSS_ELIMIT = 0, -1, -2, -3, -4, -5, -6, -7
+SELECT_STATIC_MAX_LIVE = 8192
 KIND_RB, KIND_FULL, KIND_GAUSS = 0, 1, 2
 
 
@@ -59,7 +60,7 @@ class nss_iter_state(C.Structure):
 
 EXPORTS = ("nss_create", "nss_destroy", "nss_loglike_batch", "nss_loglike_batch_host", "nss_set_loglike_variant",
            "nss_replace_step", "nss_iterate", "nss_iterate_host",
-           "nss_set_trace", "nss_select_lowest", "nss_tune", "nss_evidence_update", "nss_init_live",
+           "nss_set_trace", "nss_select_lowest", "nss_select_lowest_static", "nss_tune", "nss_evidence_update", "nss_init_live",
            "nss_philox", "nss_run", "nss_resample_equal", "nss_waveform", "nss_get_tables", "nss_fp64_peak", "nss_launch_count",
            "nss_last_chain_ms", "nss_set_chain_timing", "nss_set_chain_warps", "nss_set_chain_lanes", "nss_set_chain_pack", "nss_last_chain_diag", "nss_set_periodic",
            "nss_strerror", "nss_last_cuda_error", "nss_version")
@@ -89,6 +90,7 @@ def lib():
         L.nss_iterate_host.argtypes = L.nss_iterate.argtypes
         L.nss_loglike_batch_host.argtypes = [vp, vp, C.c_int64, vp, vp]
         L.nss_select_lowest.argtypes = [vp, vp, C.c_int32, C.c_int32, vp, vp, c_dp, vp]
+        L.nss_select_lowest_static.argtypes = [vp, C.c_int32, C.c_int32, vp, vp, vp, vp]
         L.nss_tune.argtypes = [vp, vp, C.c_int32, vp, vp, vp]
         L.nss_evidence_update.argtypes = [vp, vp, C.c_int32, C.c_int32, vp, c_dp, vp]
         L.nss_init_live.argtypes = [vp, C.c_int32, C.c_uint64, vp, vp, vp]
@@ -149,6 +151,18 @@ def nss_fp64_peak(ms: float = 200.0) -> float:
     out = C.c_double()
     _check(lib().nss_fp64_peak(float(ms), C.byref(out), _stream()), "nss_fp64_peak")
     return out.value
+
+
+def nss_select_lowest_static(logL, n_delete, dead_idx, surv_idx=None, logLstar=None):
+    """Delete-select without a handle and without any allocation, here or in the library: every argument is a CUDA tensor
+    the caller already owns (logL float64 [n]; dead_idx int32 [n_delete]; surv_idx int32 [n - n_delete] or None; logLstar
+    float64 [1] or None), which is the point — a program that has given all device memory to torch's caching allocator
+    can still call it.  n <= SELECT_STATIC_MAX_LIVE.  Asynchronous on the current stream; calls must not overlap on the
+    GPU (one shared work array per device, see include/nss.h).  Returns the status code for NSS_ELIMIT, raises otherwise."""
+    rc = lib().nss_select_lowest_static(logL.data_ptr(), logL.numel(), int(n_delete), dead_idx.data_ptr(),
+                                        surv_idx.data_ptr() if surv_idx is not None else None,
+                                        logLstar.data_ptr() if logLstar is not None else None, _stream())
+    return _check(rc, "nss_select_lowest_static", ok=(NSS_OK, NSS_ELIMIT))
 
 
 class Nss:

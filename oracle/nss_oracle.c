@@ -22,7 +22,10 @@
  * Pins (tests/test_oracle_*.py, -m "not gpu"): see DESIGN.md §5.  The higher PN phase coefficients
  * phi_2..phi_7 (P2) are pinned to SURVEY.md O3, the normative definition of this build's waveform: every literal
  * is recovered numerically from orc_phase and compared with tests/golden/taylorf2_o3_literals.txt, typed by hand
- * from the survey text (the source papers themselves are not in the container).  "Parity unpinned" by any
+ * from the survey text (the source papers themselves are not in the container).  The bin edges (O8, readings
+ * A7 / A8: dephasing() and build_edges() below) are pinned the same way since round 3 (P17): rebuilt in 50-digit
+ * arithmetic from tests/golden/o8_dephasing.txt, typed by hand from SURVEY.md:397-403, and compared index for
+ * index; ownership and bin centres by bin-independent sum identities.  "Parity unpinned" by any
  * external source: the sampler conventions A12/A14/A15/A17 (validity pinned by P13/P15 only); the wrap
  * convention of periodic coordinates (NEXT-2, R4) likewise: nothing external fixes where the seam
  * value goes, its validity is pinned by uniformity, identity inside the box and the analytic evidence.

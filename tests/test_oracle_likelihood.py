@@ -366,6 +366,122 @@ def test_bin_edges_structure(oracle, wl1, wl2):
     assert s[..., 4].sum() == pytest.approx(hh_full, rel=1e-12)        # sum B0 = <h0,h0>
 
 
+def _o8_rows(path=None):
+    """The hand-typed rows of tests/golden/o8_dephasing.txt: (gamma as an mpmath rational, sign, 'f_min' | 'f_max')."""
+    import mpmath as mp
+    path = path or os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "o8_dephasing.txt")
+    rows = []
+    for line in open(path):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        gam, sign, ref = (t.strip() for t in line.split("|"))
+        p_, q_ = gam.split("/")
+        rows.append((mp.mpf(int(p_)) / int(q_), int(sign), ref))
+    return rows
+
+
+def _o8_edges(rows, f_min, df, n_freq, B):
+    """O8 written out from the fixture in 50-digit arithmetic: (edge indices after the monotonicity passes, raw nearest
+    indices, smallest gap by which a raw choice beat its runner-up, relative to the delta range)."""
+    import mpmath as mp
+    mp.mp.dps = 50
+    fmin, fmax = mp.mpf(f_min), mp.mpf(f_min) + (n_freq - 1) * mp.mpf(df)
+    ref = {"f_min": fmin, "f_max": fmax}
+    delta = [sum(sg * (((fmin + k * mp.mpf(df)) / ref[r]) ** g) for g, sg, r in rows) for k in range(n_freq)]
+    d0, d1 = delta[0], delta[-1]
+    raw, closest = [], mp.mpf(1)
+    up = all(delta[k + 1] > delta[k] for k in range(n_freq - 1))
+    for e in range(B + 1):
+        t = d0 + mp.mpf(e) / B * (d1 - d0)
+        if up:                                   # monotone: the nearest point is one of the two around the target
+            lo_, hi_ = 0, n_freq - 1
+            while hi_ - lo_ > 1:
+                mid = (lo_ + hi_) // 2
+                if delta[mid] <= t:
+                    lo_ = mid
+                else:
+                    hi_ = mid
+            cand = sorted({max(lo_ - 1, 0), lo_, hi_, min(hi_ + 1, n_freq - 1)})
+        else:
+            cand = range(n_freq)
+        dist = sorted((abs(delta[k] - t), k) for k in cand)          # equal distances: the lower index first
+        raw.append(dist[0][1])
+        if len(dist) > 1:
+            closest = min(closest, (dist[1][0] - dist[0][0]) / abs(d1 - d0))
+    ie = list(raw)
+    ie[0], ie[B] = 0, n_freq - 1
+    for e in range(1, B + 1):
+        ie[e] = max(ie[e], ie[e - 1] + 1)
+    ie[B] = n_freq - 1
+    for e in range(B - 1, -1, -1):
+        ie[e] = min(ie[e], ie[e + 1] - 1)
+    return np.array(ie), np.array(raw), float(closest)
+
+
+def test_p17_bin_edges_from_the_dephasing_fixture(oracle, wl1, wl2):
+    """P17 (O8, readings A7 / A8).  The power laws, their signs and the f_min / f_max normalisation are read from a
+    fixture typed by hand from SURVEY.md:397-403; the edges are rebuilt from it in 50-digit arithmetic (nearest grid
+    point to each equal-increment target, ties to the lower index, then the forward / backward passes) and must equal
+    the oracle's, index for index, for B in {32, 128, 1024} on both frequency grids (config 1: 20-512 Hz, config 2:
+    20-1024 Hz).  A dropped power law, a flipped sign and swapped reference frequencies each give different edges, so
+    a slip of that kind in the oracle fails here (before this pin only the GPU's bit-exact edge comparison saw it)."""
+    rows = _o8_rows()
+    assert len(rows) == 5
+    for g_, sg, r in rows:                        # the rule the survey states beside the list
+        assert sg == (1 if g_ > 0 else -1) and r == ("f_max" if g_ > 0 else "f_min")
+    mutants = {
+        "a power law dropped": [x for x in rows if x[0] != 1],
+        "a sign flipped": [(g_, -sg if i == 1 else sg, r) for i, (g_, sg, r) in enumerate(rows)],
+        "f_min and f_max swapped": [(g_, sg, "f_min" if r == "f_max" else "f_max") for g_, sg, r in rows],
+        "an exponent mistyped (5/3 -> 4/3)": [((g_ if i != 3 else g_ - g_ / 5), sg, r) for i, (g_, sg, r) in enumerate(rows)],
+    }
+    for w in (wl1, wl2):
+        for B in (32, 128, 1024):
+            idx, F = oracle.Problem(w, kind=0, n_bins=B).edges()
+            want, raw, closest = _o8_edges(rows, w.f_min, w.df, w.n_freq, B)
+            assert closest > 1e-9, "a target sits within rounding of a tie: fp64 and 50 digits may choose differently"
+            assert np.array_equal(idx, want), (w.name, B, np.flatnonzero(idx != want)[:5])
+            free = np.flatnonzero((np.diff(idx)[:-1] > 1) & (np.diff(idx)[1:] > 1)) + 1     # edges no pass has moved
+            assert free.size > B // 4 and np.array_equal(idx[free], raw[free])              # ... are the nearest points
+            assert np.array_equal(F, w.f_min + w.df * idx)
+            if B == 128:
+                for what, rows_m in mutants.items():
+                    bad, _, _ = _o8_edges(rows_m, w.f_min, w.df, w.n_freq, B)
+                    assert not np.array_equal(bad, idx), f"{what}: the pin cannot see it"
+                    assert np.sum(bad != idx) > B // 4, what
+
+
+def test_p17_bin_ownership_and_centres(oracle, wl2):
+    """A8.  Half-open ownership [i_b, i_b+1) (last bin closed) makes the bins a partition of the grid, and the centre of
+    bin b is the mid-point of its two EDGE frequencies: with C_k = 4 df d_k conj(h0_k) / S_k,
+    sum_b A0_b = sum_k C_k and sum_b (A1_b + fbar_b A0_b) = sum_k C_k f_k whatever the bins are; likewise B0, B1 with
+    |h0_k|^2.  Computed here from the data and the fiducial strain directly, never through a bin.  A closed interval
+    (edge points counted twice), a last point left out, or a centre at the mean of the owned frequencies breaks one."""
+    w = wl2
+    f = w.freqs
+    for B in (128, 1000):
+        p = oracle.Problem(w, kind=0, n_bins=B)
+        idx, F = p.edges()
+        fbar = 0.5 * (F[:-1] + F[1:])
+        s = p.summary()
+        for a in range(w.n_det):
+            h0 = oracle.waveform(w.theta_fid, w.det[a], w.gmst, f)
+            d = w.data[a, :, 0] + 1j * w.data[a, :, 1]
+            C = 4 * w.df * d * np.conj(h0) / w.psd[a]
+            Q = 4 * w.df * np.abs(h0) ** 2 / w.psd[a]
+            A0, A1 = s[a, :, 0] + 1j * s[a, :, 1], s[a, :, 2] + 1j * s[a, :, 3]
+            assert abs(A0.sum() - C.sum()) <= 1e-11 * np.abs(C).sum()
+            assert abs((A1 + fbar * A0).sum() - (C * f).sum()) <= 1e-11 * np.abs(C * f).sum()
+            assert abs(s[a, :, 4].sum() - Q.sum()) <= 1e-12 * Q.sum()
+            assert abs((s[a, :, 5] + fbar * s[a, :, 4]).sum() - (Q * f).sum()) <= 1e-12 * (Q * f).sum()
+            # per bin, on the first, a middle and the last bin (the one that also owns i_B)
+            for b in (0, B // 2, B - 1):
+                own = slice(idx[b], idx[b + 1] + (1 if b == B - 1 else 0))
+                assert abs(A0[b] - C[own].sum()) <= 1e-11 * np.abs(C[own]).sum()
+                assert abs(A1[b] - (C[own] * (f[own] - fbar[b])).sum()) <= 1e-10 * np.abs(C[own] * (f[own] - fbar[b])).sum() + 1e-300
+
+
 def test_domain_and_nonfinite(oracle, wl2):
     p = oracle.Problem(wl2)
     th = wl2.theta_fid[wl2.param_index].copy()

@@ -94,6 +94,11 @@ struct nss_handle {
   cudaEvent_t ev_k3[2];
   int ev_k3_valid;
   int chain_timing;            // record the event pair around K3 (nss_set_chain_timing); off by default
+  // resident CTAs per SM of the K3 instantiation launched last with packed single-warp chains (occupancy query cached
+  // per kernel, warps per CTA and dynamic shared memory: the latter depends on this handle's table)
+  const void *occ_kern;
+  int occ_W, occ_per_sm;
+  size_t occ_smem;
 };
 
 extern thread_local char g_nss_cuda_err[256];

@@ -87,9 +87,10 @@ __global__ void k_init_live(const __grid_constant__ NssDev P, int n, uint64_t se
 // initial stop test of nss_run) or inside the two fused kernels of an iteration: k4_front (rank + tune in parallel
 // blocks, then selection tail + evidence in whichever block finishes last) and the epilogue of K3 (live evidence).
 constexpr int kOneCta = 1024;
+constexpr int kMaxDevices = 64;          // device ordinals the per-device tables below cover
 constexpr int kRankElems = 256;          // live points ranked per block: 4 threads per point, each scanning a quarter of every tile
 
-struct K4Smem {
+struct __align__(16) K4Smem {         // rank_block reads rank.tile two doubles per load
   union {
     struct { double tile[1024]; int cnt4[4 * kRankElems]; } rank;
     struct { double part[kOneCta]; double mean[NSS_NSLOT]; double cov[NSS_NSLOT * NSS_NSLOT]; double Lc[NSS_NSLOT * NSS_NSLOT]; } tune;
@@ -234,6 +235,12 @@ constexpr int kTunePartDoubles = NSS_NSLOT + NSS_NSLOT * (NSS_NSLOT + 1) / 2;   
 // One block per 1024 live points (about one row per thread in the column sums, ~70 in the products): a single block, with
 // no barrier between blocks, up to 2047 rows.
 __host__ __device__ inline int tune_blocks_for(int n) { const int t = n / 1024; return t < 2 ? 1 : t > kTuneMaxBlocks ? kTuneMaxBlocks : t; }
+// The barrier among the tuning blocks is a spin on a counter, so all T of them must get an SM while the others wait.  A
+// 1024-thread CTA of these kernels always fits an empty SM (__launch_bounds__), the rank blocks beside them and any other
+// stream's CTAs finish without waiting for anybody here, so T <= number of SMs is enough for the last tuning block to be
+// scheduled eventually.  On a B200 (148 SMs) the cap never binds; on a small MIG slice it does (and T, hence the order
+// of the partial sums, then differs from a full device's in the last bits).
+inline int tune_blocks_on(const nss_handle *h, int n) { const int t = tune_blocks_for(n); return t > h->n_sm ? (h->n_sm < 1 ? 1 : h->n_sm) : t; }
 
 __device__ __forceinline__ void tune_block(const double *__restrict__ live, int n, int d, int b, int T, double *__restrict__ scratch,
                                            uint32_t *__restrict__ counters /*[2]*/, double *__restrict__ mean_out,
@@ -548,6 +555,11 @@ __global__ void __launch_bounds__(kOneCta) k4_tune(const double *__restrict__ li
 {
   __shared__ K4Smem sm;
   tune_block(live, n, d, blockIdx.x, T, scratch, ctl->tune_cnt, mean_out, chol_out, &ctl->flags[0], sm);
+  // Leave the two counters at zero, as k4_front's last block does: an iteration queued next on this handle (nss_iterate,
+  // nss_replace_step: no k_begin in front of them) starts its own tuning blocks from them.  The block holding the last
+  // ticket is the only one still running tune_block's tail, and every other block has passed the barrier on counters[0]
+  // before it took its ticket, so nobody reads them any more.
+  if (T > 1 && threadIdx.x == 0 && sm.ticket == (unsigned)T - 1u) { ctl->tune_cnt[0] = 0; ctl->tune_cnt[1] = 0; }
 }
 
 __global__ void __launch_bounds__(kOneCta) k4_evidence(const double *__restrict__ dead_logL, int n, int k, double *__restrict__ logw,
@@ -1260,20 +1272,28 @@ int launch_chains_k(nss_handle *h, ChainArgs &A, size_t tab_bytes, cudaStream_t 
   }
   const size_t smem = tab_bytes + (size_t)W * G * (32 / LANES) * nssk::kSubScratchDoubles * sizeof(double)
                     + (size_t)W * kDirChunk * NSS_NSLOT * sizeof(double);
-  static size_t smem_set = 0;                            // per instantiation: the attribute is raised only when a launch needs more
-  if (smem > smem_set) {
-    NSS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    smem_set = smem;
+  {
+    // The dynamic shared memory limit is an attribute of (function, device) shared by every handle and host thread of the
+    // process: it is only ever raised, under a lock, and remembered per device (one table per instantiation).
+    static std::mutex mu;
+    static size_t smem_set[kMaxDevices] = {0};
+    if (h->device < 0 || h->device >= kMaxDevices) return NSS_EINVAL;
+    std::lock_guard<std::mutex> lock(mu);
+    if (smem > smem_set[h->device]) {
+      NSS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      smem_set[h->device] = smem;
+    }
   }
   unsigned grid = (unsigned)A.k;
   if (G == 1) {
-    static int per_sm[kChainWarps + 1] = {0};            // resident CTAs per SM for W warps (per instantiation)
-    if (!per_sm[W]) {
+    // resident CTAs per SM: depends on the instantiation, W and this handle's table size, so it is cached in the handle
+    const void *kp = reinterpret_cast<const void *>(kern);
+    if (h->occ_kern != kp || h->occ_W != W || h->occ_smem != smem) {
       int nb = 0;
       NSS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, 32 * W, smem));
-      per_sm[W] = nb > 0 ? nb : 1;
+      h->occ_kern = kp; h->occ_W = W; h->occ_smem = smem; h->occ_per_sm = nb > 0 ? nb : 1;
     }
-    const long long slots = (long long)per_sm[W] * h->n_sm, need = (A.k + W - 1) / W;
+    const long long slots = (long long)h->occ_per_sm * h->n_sm, need = (A.k + W - 1) / W;
     grid = (unsigned)(need < slots ? need : slots);
   }
   cudaLaunchConfig_t cfg = {};
@@ -1418,7 +1438,7 @@ int enqueue_iteration(nss_handle *h, double *live, double *logL, double *birth, 
   const int d = h->dev.d;
   FrontArgs F;
   F.live = live; F.logL = logL; F.birth = birth; F.n = n; F.k = k; F.d = d; F.Lstar_in = Lstar_in;
-  F.T = tune_blocks_for(n); F.nseg = n > kRankDirectMax ? 0 : rank_segments(n);
+  F.T = tune_blocks_on(h, n); F.nseg = n > kRankDirectMax ? 0 : rank_segments(n);
   if (F.nseg == 0) {                                     // many live points: the ranks come from a sample sort (five more launches)
     const int rc = launch_sample_rank(h, logL, n, k, h->d_rank, dead_idx, reset, st);
     if (rc) return rc;
@@ -1566,7 +1586,7 @@ extern "C" int nss_tune(nss_handle *h, const double *live_dev, int32_t n_live, d
   if (rc) return rc;
   rc = begin_iteration(h, 0, 0.0, 0.0, 0, st);
   if (rc) return rc;
-  const int T = tune_blocks_for(n_live);
+  const int T = tune_blocks_on(h, n_live);
   k4_tune<<<T, kOneCta, 0, st>>>(live_dev, n_live, h->dev.d, T, h->d_tune_scratch, h->d_ctl, mean_dev, chol_dev);
   h->launches += 1;
   NSS_CUDA(cudaGetLastError());

@@ -259,7 +259,10 @@ typedef struct {
  * logZ_err (200 stochastic-compression replicas, O15), ess and n_equal (the rows nss_resample_equal keeps, same seed) are
  * reduced on the device.  Returns NSS_OK, NSS_ENOTCONV
  * (max_iter reached, results valid), NSS_ECAP (out->cap too small: needs n_iter * n_delete + n_live rows), NSS_ECHOL,
- * NSS_EINVAL, NSS_ENOMEM or NSS_ECUDA.  Synchronous: returns after the stream has drained. */
+ * NSS_EINVAL, NSS_ENOMEM or NSS_ECUDA.  Synchronous: returns after the stream has drained.
+ * `out` is read as well as written: zero the whole nss_result first (memset / = {0}), then set the four array pointers
+ * and cap.  equal_idx in particular MUST be NULL unless it points to cap int64 slots — nss_run copies n_equal indices
+ * through any non-NULL value, so a field left uninitialised is a wild write. */
 int nss_run(nss_handle *h, int32_t n_live, int32_t n_delete, int32_t n_repeats, uint64_t seed,
             double stop_dlogz, int32_t max_iter, nss_result *out, void *cuda_stream);
 
@@ -276,11 +279,12 @@ int nss_get_tables(nss_handle *h, int32_t *edge_idx_host, double *summary_host, 
  * the roofline denominator.  *tflops_host = 2 * FMA/s / 1e12. */
 int nss_fp64_peak(double ms, double *tflops_host, void *cuda_stream);
 
-/* Device time [ms] of the most recent K3 (slice-sampling chains) launch, from CUDA events the library
- * records around it on the caller's stream (bench.py's roofline for the dominant kernel), if
- * nss_set_chain_timing(h, 1) was called before that launch; NSS_EINVAL otherwise.  Off by default: the event in
- * front of K3 keeps its prologue from overlapping the kernel before it (programmatic dependent launch). */
+/* on != 0: from now on the library records a CUDA event pair around every K3 (slice-sampling chains) launch on the
+ * caller's stream.  Off by default: the event in front of K3 keeps its prologue from overlapping the kernel before it
+ * (programmatic dependent launch). */
 int nss_set_chain_timing(nss_handle *h, int32_t on);
+/* Device time [ms] of the most recent K3 launch from that event pair (bench.py's roofline for the dominant kernel);
+ * NSS_EINVAL unless nss_set_chain_timing(h, 1) was called before that launch. */
 int nss_last_chain_ms(nss_handle *h, double *ms_host);
 
 /* Kernel launches issued by this handle since creation (bench.py's gpu_launches). */

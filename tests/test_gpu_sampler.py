@@ -133,9 +133,10 @@ def test_init_live_matches_oracle(nssmod, oracle, wl1):
     g.close()
 
 
-def _trajectory_parity(g, p, live, logL, k, n_repeats, seed, it, logLstar=math.nan, max_excluded=0.03, w=None):
+def _trajectory_parity(g, p, live, logL, k, n_repeats, seed, it, logLstar=math.nan, max_excluded=0.03, w=None, o=None):
     r = g.nss_replace_step(live, logL, k, n_repeats, seed, it, logLstar=logLstar, want_trace=True)
-    o = p.replace_step(live, logL, k, n_repeats, seed, it, logLstar=logLstar, want_trace=True)
+    if o is None:                                 # else: the oracle's result for these very arguments, computed by the caller
+        o = p.replace_step(live, logL, k, n_repeats, seed, it, logLstar=logLstar, want_trace=True)
     assert o["rc"] == 0
     assert np.array_equal(r["dead_idx"].cpu().numpy(), o["dead_idx"])
     assert np.array_equal(r["dead_theta"].cpu().numpy(), o["dead_theta"])
@@ -194,6 +195,36 @@ def test_iteration_above_the_counting_select_limit(nssmod, oracle):
     assert abs(rg["logZ"] - ro["logZ"]) < 3 * math.hypot(rg["logZ_err"], ro["logZ_err"]) + 1e-9
     if _replays(rg, ro):
         _assert_replay(rg, ro, w)
+    g.close()
+
+
+def test_iteration_after_a_stand_alone_tune_on_the_same_handle(nssmod, oracle):
+    """nss_tune with several tuning blocks (n_live >= 2048: a counter barrier and a ticket among them) followed by
+    iterations on the SAME handle: the stand-alone kernel must leave the two counters at zero, else the next k4_front's
+    barrier opens early and no block factors the covariance (stale Cholesky, no NSS_ECHOL).  5000 -> 3 blocks at the
+    tune, then 4 blocks (4100 live points: a larger T than the counters' leftover) and 2 blocks in the iterations."""
+    w = inputs.gaussian_workload(5, sigma=0.07)
+    g, p = nssmod.Nss(w), oracle.Problem(w)
+    live5, _ = p.init_live(5000, 31)
+    rc, mean, chol = g.nss_tune(live5 * 0.3)                 # a different population: its factor must not be reused
+    orc, omean, ocov, ochol = oracle.tune(live5 * 0.3)
+    assert rc == 0 and np.allclose(chol.cpu().numpy(), ochol, rtol=1e-8, atol=1e-300)
+    live, logL = p.init_live(4100, 32)
+    r, o, safe = _trajectory_parity(g, p, live, logL, 2050, 4, seed=9, it=0, w=w)
+    rc, mean, chol = g.nss_tune(live5)
+    assert rc == 0
+    live, logL = p.init_live(2100, 33)
+    st = nssmod.nss_iter_state(logX=0.0, logZ=-math.inf)
+    import torch
+    dl, dL = torch.as_tensor(live, device="cuda").clone(), torch.as_tensor(logL, device="cuda").clone()
+    bufs = g.iter_buffers(1050)
+    g.nss_iterate(dl, dL, 1050, 4, 9, 0, st, bufs)
+    o = p.replace_step(live, logL, 1050, 4, 9, 0, want_trace=True)
+    safe = o["margin"] > 1e-6
+    didx = o["dead_idx"]
+    assert np.array_equal(bufs[3].cpu().numpy(), didx) and st.logLstar == o["logLstar"]
+    assert safe.mean() > 0.97
+    assert np.all(np.abs(dl.cpu().numpy()[didx][safe] - o["live"][didx][safe]) <= 1e-9 * (w.hi - w.lo))
     g.close()
 
 
@@ -257,6 +288,77 @@ def test_replace_step_full_grid_at_the_bench_launch_shape(nssmod, oracle):
     live, logL = o["live"], o["logL"]
     o = p.replace_step(live, logL, 500, 2, 6, 1)
     _trajectory_parity(g, p, o["live"], o["logL"], 500, 3, seed=6, it=2, w=w, max_excluded=0.05)
+    g.close()
+
+
+@pytest.mark.parametrize("B", [256, 1024])
+def test_replace_step_and_run_at_many_bins(nssmod, oracle, wl2, B):
+    """Config-2 geometry with 256 and 1024 bins per detector (BASELINE configs[4]'s bin counts, inside the sampler this
+    time).  At B = 1024 the 8-lane table is not built and no lane count's table fits the 64 KB shared-memory budget, so
+    K3 runs its RESIDENT = false instantiations (records read through L2) and a request for 8 lanes falls back to the
+    automatic choice; at B = 256 the 8- and 16-lane tables fit and the 32-lane one is the largest resident table.
+    Every lane setting must reproduce the oracle's trajectories; then a bounded run on both sides."""
+    g, p = nssmod.Nss(wl2, n_bins=B), oracle.Problem(wl2, n_bins=B)
+    n, k, nrep = 400, 200, 6
+    live, logL = p.init_live(n, 12)
+    o0 = p.replace_step(live, logL, k, nrep, 12, 0, want_trace=True)
+    live1, logL1 = o0["live"], o0["logL"]
+    for it in (1, 2):                              # a compressed population as the second case
+        oo = p.replace_step(live1, logL1, k, 3, 12, it)
+        live1, logL1 = oo["live"], oo["logL"]
+    o1 = p.replace_step(live1, logL1, k, nrep, 12, 3, want_trace=True)
+    for lanes in (0, 8, 16, 32):
+        g.set_chain_lanes(lanes)
+        for warps in ((0, 1) if lanes in (0, 32) else (0,)):
+            g.set_chain_warps(warps)
+            _trajectory_parity(g, p, live, logL, k, nrep, seed=12, it=0, w=wl2, max_excluded=0.05, o=o0)
+            _trajectory_parity(g, p, live1, logL1, k, nrep, seed=12, it=3, w=wl2, max_excluded=0.05, o=o1)
+    g.set_chain_lanes(0); g.set_chain_warps(0)
+    rg, ro = g.nss_run(n, k, nrep, 13, max_iter=3), p.run(n, k, nrep, 13, max_iter=3)
+    assert rg["rc"] == nssmod.NSS_ENOTCONV and rg["n_iter"] == ro["n_iter"] == 3 and rg["n_dead"] == ro["n_dead"]
+    assert abs(rg["logZ"] - ro["logZ"]) < 3 * math.hypot(rg["logZ_err"], ro["logZ_err"]) + 1e-9
+    if _replays(rg, ro):
+        _assert_replay(rg, ro, wl2)
+    g.close()
+
+
+def test_results_do_not_depend_on_what_earlier_calls_left_in_the_handle(nssmod, wl1):
+    """compute-sanitizer is closed on the build pool (profiles/r03_sanitizer.md), so the question initcheck would answer
+    is asked directly: a handle's scratch (rank counts, sample-sort buffers, tuning partials, control block, run block)
+    is reused across calls of different sizes and never cleared by the host.  A run and an iteration on a handle that
+    has just served larger and different work (9000-live sample-sort iteration, a stand-alone tune, a bounded run, a
+    Cholesky failure) must give the same BITS as on a fresh handle — anything read before it is written would differ."""
+    import torch
+    wg = inputs.gaussian_workload(4, sigma=0.06)
+
+    def work(g):
+        r = g.nss_run(300, 150, 8, 17, want_equal=True)
+        live, logL = g.nss_init_live(257, 18)
+        st = nssmod.nss_iter_state(logX=0.0, logZ=-math.inf)
+        bufs = g.iter_buffers(100)
+        g.nss_iterate(live, logL, 100, 5, 18, 0, st, bufs)
+        dead, surv, ls = g.nss_select_lowest(logL, 31)
+        return (r["logZ"], r["logZ_err"], r["H"], r["ess"], r["n_evals"], r["dead_theta"].tobytes(), r["dead_logw"].tobytes(),
+                r["dead_logL_birth"].tobytes(), r["equal_idx"].tobytes(), live.cpu().numpy().tobytes(), logL.cpu().numpy().tobytes(),
+                tuple(b.cpu().numpy().tobytes() for b in bufs), (st.logX, st.logZ, st.logZ_live, st.logLstar, st.n_evals),
+                dead.cpu().numpy().tobytes(), surv.cpu().numpy().tobytes(), ls)
+
+    fresh = nssmod.Nss(wg)
+    want = work(fresh)
+    fresh.close()
+    g = nssmod.Nss(wg)
+    live, logL = g.nss_init_live(9000, 3)                      # sample-sort buffers, eight tuning blocks, packed chains
+    st = nssmod.nss_iter_state(logX=-5.0, logZ=-40.0)
+    g.nss_iterate(live, logL, 4500, 2, 3, 0, st, g.iter_buffers(4500))
+    g.nss_tune(live[:5000])
+    g.nss_run(2000, 1000, 3, 4, max_iter=2)
+    flat = torch.rand(60, 4, dtype=torch.float64, device="cuda") * 0.1
+    flat[:, 1] = 0.01                                          # zero variance: NSS_ECHOL, flags left set in the control block
+    fl = g.nss_loglike_batch(flat)
+    assert g.nss_replace_step(flat, fl, 30, 2, 1, 0, ok=(nssmod.NSS_ECHOL,))["rc"] == nssmod.NSS_ECHOL
+    got = work(g)
+    assert got == want
+    assert work(g) == want                                      # and again on the now twice-used handle
     g.close()
 
 
@@ -545,7 +647,7 @@ def test_iterate_device_and_host_forms_match_oracle(nssmod, oracle, wl1):
     g.close()
 
 
-@pytest.mark.parametrize("cfg", ["gauss", "config1", "config2"])
+@pytest.mark.parametrize("cfg", ["gauss", "config1", "config2", "config4"])
 def test_chain_group_width_does_not_change_the_trajectory(nssmod, oracle, wl1, wl2, cfg):
     """K3 runs a chain on G = 1, 2, 4 or 8 warps whose sub-warps (8, 16 or 32 lanes per candidate) evaluate the
     next bracket tests speculatively.  For a given lane count the decisions, positions, logL and the
@@ -558,6 +660,8 @@ def test_chain_group_width_does_not_change_the_trajectory(nssmod, oracle, wl1, w
         w, n, k, nrep = inputs.gaussian_workload(6, sigma=0.05), 300, 150, 40
     elif cfg == "config1":
         w, n, k, nrep = wl1, 100, 50, 12
+    elif cfg == "config4":                           # the full-grid kind: 32 lanes per candidate only, table read from L2
+        w, n, k, nrep = inputs.make_data(inputs.config4(), oracle.waveform), 96, 48, 12
     else:
         w, n, k, nrep = wl2, 400, 200, 35            # 35 repeats: crosses the 32-step direction chunk
     g, p = nssmod.Nss(w), oracle.Problem(w)
@@ -567,7 +671,7 @@ def test_chain_group_width_does_not_change_the_trajectory(nssmod, oracle, wl1, w
             o = p.replace_step(live, logL, k, 3, 11, it)
             live, logL = o["live"], o["logL"]
     first = None
-    for L in ((32,) if cfg == "gauss" else (32, 16, 8)):
+    for L in ((32,) if cfg in ("gauss", "config4") else (32, 16, 8)):
         g.set_chain_lanes(L)
         ref = None
         for G, pack in ((1, 1), (1, 3), (1, 8), (2, 0), (4, 0), (8, 0), (0, 0)):

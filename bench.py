@@ -58,7 +58,7 @@ def rb_work(B: int, n_det: int):
     return instr, flop
 
 
-K3_PROFILE = os.path.join(ROOT, "profiles", "r02_k3_slice_full.md")
+K3_PROFILE = os.path.join(ROOT, "profiles", "r03_k3_slice_full.md")
 
 
 def profile_traffic():
@@ -516,7 +516,7 @@ def run_ours(args):
                                "pipe_frac_of_nominal": N2 / (k2_ms * 1e-3) * (600 + w.n_freq * (8 + 22 * w.n_det)) / (NOMINAL_TF * 1e12 / 2),
                                "algorithmic_hbm_bytes_per_eval": 96,
                                "note": "the 484 KB record table is shared by every point and stays in L2; HBM GB/s is reported by "
-                                       "profiles/r01e_k2_full_grid_full.md"},
+                                       "profiles/r03_k2_full_grid_full.md"},
         "nss_run": run2,
         "clocks": clocks.summary(),
     }

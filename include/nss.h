@@ -103,7 +103,12 @@ int nss_set_chain_warps(nss_handle *h, int32_t warps);
  * flags_host[j] != 0 makes sampled dimension j periodic in the slice sampler: a candidate's coordinate is mapped back
  * into [lo_j, hi_j) as y - W floor((y - lo_j)/W), W = hi_j - lo_j, and takes no part in the prior-box test (default and
  * NULL: hard inclusive walls in every dimension, reading A16).  Host array of d flags, copied.  The likelihood should
- * be periodic in that coordinate over the box (phi_c over 2 pi, psi over pi, ra over 2 pi); the evidence is valid either way. */
+ * be periodic in that coordinate over the box (phi_c over 2 pi, psi over pi, ra over 2 pi); the evidence is valid either way.
+ * The tuning follows the geometry too (reading R7; "better tuning that respects the geometry of the
+ * parameter space"): in nss_tune and in every iteration a periodic coordinate is unwrapped around its circular mean
+ * (x' = x - W rint((x - mu_c)/W), mu_c from atan2 of the summed sines and cosines of 2 pi (x - lo)/W) before mean,
+ * covariance and Cholesky factor are formed, so a population that straddles the seam is tuned with the width it has on
+ * the circle; a population that does not reach across the seam, and any non-periodic coordinate, is tuned as before. */
 int nss_set_periodic(nss_handle *h, const int32_t *flags_host);
 
 /* Diagnostics of the most recent nss_replace_step / nss_iterate (read from the control block that call fetched):

@@ -613,6 +613,42 @@ int orc_tune(const double *live, int n, int d, double *mean, double *cov, double
   return 0;
 }
 
+/* NEXT-2, second half ("Providing better tuning that respects the geometry of the parameter space is an area
+ * for future work"; SURVEY.md §8(f) NEXT-2 "optionally whitening that respects wrapped geometry"; reading R7 in DESIGN.md).
+ * The plain moments of a periodic coordinate are wrong for a population that straddles the seam (half the points near lo,
+ * half near hi: a variance of ~W^2/4 for a cloud that is narrow on the circle).  Reading R7: before the moments, every
+ * periodic coordinate is unwrapped around its CIRCULAR MEAN,
+ *     phi_i = 2 pi (x_i - lo)/W,  S = sum sin phi_i,  C = sum cos phi_i,  a = atan2(S, C)  (a + 2 pi if a < 0),
+ *     mu_c = lo + W a/(2 pi),     x'_i = x_i - W rint((x_i - mu_c)/W)     (nearest image of x_i to mu_c; rint = ties to even),
+ * and mean, covariance and Cholesky factor are those of the x' (orc_tune on the unwrapped copy).  A point whose nearest image
+ * is itself keeps its bits (x' = x - W*0), so a population that does not reach across the seam is tuned exactly as before,
+ * and with no periodic flag this is orc_tune.  flags, lo, hi: per sampled dimension. */
+int orc_tune_periodic(const double *live, int n, int d, const int *flags, const double *lo, const double *hi,
+                      double *mean, double *cov, double *chol)
+{
+  double *x = (double *)malloc(sizeof(double) * (size_t)n * d);
+  memcpy(x, live, sizeof(double) * (size_t)n * d);
+  for (int j = 0; j < d; ++j) {
+    if (!flags || !flags[j]) continue;
+    const double W = hi[j] - lo[j];
+    double S = 0.0, C = 0.0;
+    for (int i = 0; i < n; ++i) {
+      const double phi = 2.0 * M_PI * ((live[(size_t)i * d + j] - lo[j]) / W);
+      S += sin(phi); C += cos(phi);
+    }
+    double a = atan2(S, C);
+    if (a < 0.0) a += 2.0 * M_PI;
+    const double muc = lo[j] + W * (a / (2.0 * M_PI));
+    for (int i = 0; i < n; ++i) {
+      const double v = live[(size_t)i * d + j];
+      x[(size_t)i * d + j] = v - W * rint((v - muc) / W);
+    }
+  }
+  const int rc = orc_tune(x, n, d, mean, cov, chol);
+  free(x);
+  return rc;
+}
+
 /* ---- O12.4 one slice-sampling chain --------------------------------------------------------- */
 typedef struct {
   const orc_problem *p; double Lstar; const double *chol;
@@ -717,7 +753,7 @@ int orc_replace_step(const orc_problem *p, double *live, double *logL, int n, in
     dead_logL[j] = logL[dead_idx[j]];
   }
   double mean[ORC_NSLOT], cov[ORC_NSLOT * ORC_NSLOT], chol[ORC_NSLOT * ORC_NSLOT];
-  if (orc_tune(live, n, d, mean, cov, chol) != 0) { free(surv); return -1; }
+  if (orc_tune_periodic(live, n, d, p->periodic, p->lo, p->hi, mean, cov, chol) != 0) { free(surv); return -1; }   /* R7; = orc_tune without flags */
 
   double *newx = (double *)malloc(sizeof(double) * (size_t)k * d);
   double *newl = (double *)malloc(sizeof(double) * k);

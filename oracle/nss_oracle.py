@@ -74,6 +74,8 @@ def lib():
         L.orc_logaddexp.argtypes = [C.c_double, C.c_double]
         L.orc_evidence_update.argtypes = [c_dp, C.c_int, C.c_int, c_dp, c_dp, c_dp]
         L.orc_tune.restype = C.c_int
+        L.orc_tune_periodic.restype = C.c_int
+        L.orc_tune_periodic.argtypes = [c_dp, C.c_int, C.c_int, c_ip, c_dp, c_dp, c_dp, c_dp, c_dp]
         L.orc_tune.argtypes = [c_dp, C.c_int, C.c_int, c_dp, c_dp, c_dp]
         L.orc_replace_step.restype = C.c_int
         L.orc_replace_step.argtypes = [C.c_void_p, c_dp, c_dp, C.c_int, C.c_int, C.c_double, C.c_int,
@@ -173,6 +175,17 @@ def tune(live):
     n, d = a.shape
     mean, cov, chol = np.empty(d), np.empty((d, d)), np.empty((d, d))
     rc = lib().orc_tune(_dp(a), n, d, _dp(mean), _dp(cov), _dp(chol))
+    return rc, mean, cov, chol
+
+
+def tune_periodic(live, flags, lo, hi):
+    """Reading R7: moments of the live points with every flagged coordinate unwrapped around its circular mean."""
+    a = _f64(live)
+    n, d = a.shape
+    f = np.ascontiguousarray(np.asarray(flags, dtype=np.int32)[:d])
+    lo_, hi_ = _f64(lo), _f64(hi)
+    mean, cov, chol = np.empty(d), np.empty((d, d)), np.empty((d, d))
+    rc = lib().orc_tune_periodic(_dp(a), n, d, f.ctypes.data_as(c_ip), _dp(lo_), _dp(hi_), _dp(mean), _dp(cov), _dp(chol))
     return rc, mean, cov, chol
 
 

@@ -49,7 +49,7 @@ struct NssCtl {
   uint32_t front_done;         // blocks of k4_front that have finished (the last one publishes the flags)
   uint32_t rank_done;          // ranking blocks of k4_front that have finished (the last one does the selection tail)
   int32_t sel_bad;             // a survivor below a supplied threshold (selection tail -> flags[1])
-  uint32_t tune_cnt[2];        // counters of the tuning blocks of k4_front: column sums published, products published
+  uint32_t tune_cnt[3];        // counters of the tuning blocks of k4_front: column sums published, products published, circular sums published (R7)
   uint32_t chains_done;        // chains finished (the CTA that finishes the last one runs the live-evidence epilogue)
   uint32_t chain_next;         // next chain to start (K3 with single-warp groups: warps fetch chains as they finish)
   int32_t chol_now;            // Cholesky status of the tuning block of the iteration being set up

@@ -93,7 +93,7 @@ constexpr int kRankElems = 256;          // live points ranked per block: 4 thre
 struct __align__(16) K4Smem {         // rank_block reads rank.tile two doubles per load
   union {
     struct { double tile[1024]; int cnt4[4 * kRankElems]; } rank;
-    struct { double part[kOneCta]; double mean[NSS_NSLOT]; double cov[NSS_NSLOT * NSS_NSLOT]; double Lc[NSS_NSLOT * NSS_NSLOT]; } tune;
+    struct { double part[kOneCta]; double mean[NSS_NSLOT]; double cov[NSS_NSLOT * NSS_NSLOT]; double Lc[NSS_NSLOT * NSS_NSLOT]; double muc[NSS_NSLOT]; } tune;
     struct { double red[32]; double warp_tot[32]; int iwarp_tot[32]; } red;
   };
   unsigned ticket;
@@ -231,7 +231,16 @@ __device__ __forceinline__ double block_sum(double v, double *red)
 // and the blocks' partial sums are added in block order, so the result is deterministic.  The block that finishes last
 // factors the matrix: *chol_fail = 1 if a pivot is <= 0 (reading R5: no relative epsilon), else 0.
 constexpr int kTuneMaxBlocks = 32;
-constexpr int kTunePartDoubles = NSS_NSLOT + NSS_NSLOT * (NSS_NSLOT + 1) / 2;     // per block: column sums, then products
+constexpr int kTuneProdOff = NSS_NSLOT, kTuneCircOff = NSS_NSLOT + NSS_NSLOT * (NSS_NSLOT + 1) / 2;
+constexpr int kTunePartDoubles = kTuneCircOff + 2 * NSS_NSLOT;     // per block: column sums, products, circular sums (S, C)
+// NEXT-2, second half (reading R7): sampled dimensions whose bit is set in `mask` are periodic with
+// period W over [lo, lo + W): before the moments they are unwrapped around their circular mean,
+//   mu_c = lo + W atan2(sum sin phi, sum cos phi)/(2 pi) (mod W),  phi = 2 pi (x - lo)/W,   x' = x - W rint((x - mu_c)/W).
+// mask == 0: nothing changes (no extra pass, no extra barrier, the same bits as before).
+struct TunePer {
+  int32_t mask, pad_;
+  double lo[NSS_NSLOT], W[NSS_NSLOT];
+};
 // One block per 1024 live points (about one row per thread in the column sums, ~70 in the products): a single block, with
 // no barrier between blocks, up to 2047 rows.
 __host__ __device__ inline int tune_blocks_for(int n) { const int t = n / 1024; return t < 2 ? 1 : t > kTuneMaxBlocks ? kTuneMaxBlocks : t; }
@@ -243,19 +252,80 @@ __host__ __device__ inline int tune_blocks_for(int n) { const int t = n / 1024; 
 inline int tune_blocks_on(const nss_handle *h, int n) { const int t = tune_blocks_for(n); return t > h->n_sm ? (h->n_sm < 1 ? 1 : h->n_sm) : t; }
 
 __device__ __forceinline__ void tune_block(const double *__restrict__ live, int n, int d, int b, int T, double *__restrict__ scratch,
-                                           uint32_t *__restrict__ counters /*[2]*/, double *__restrict__ mean_out,
-                                           double *__restrict__ chol_out, int32_t *__restrict__ chol_fail, K4Smem &sm)
+                                           uint32_t *__restrict__ counters /*[3]*/, double *__restrict__ mean_out,
+                                           double *__restrict__ chol_out, int32_t *__restrict__ chol_fail, const TunePer &tp,
+                                           K4Smem &sm)
 {
-  double *part = sm.tune.part, *mean = sm.tune.mean, *cov = sm.tune.cov, *sLc = sm.tune.Lc;
+  double *part = sm.tune.part, *mean = sm.tune.mean, *cov = sm.tune.cov, *sLc = sm.tune.Lc, *muc = sm.tune.muc;
   const int tid = threadIdx.x;
   const int r0 = (int)((long long)n * b / T), r1 = (int)((long long)n * (b + 1) / T);
   const int np = d * (d + 1) / 2;
+  const bool any_per = tp.mask != 0;
+  if (any_per) {
+    // R7, pass 0: circular sums of the periodic coordinates (thread = (row group, column), fixed-order tree as below),
+    // a barrier among the blocks, then every block forms the same circular means from the same partial sums
+    const int ng = kOneCta / d, j = tid % d, g = tid / d;
+    const bool pj = g < ng && ((tp.mask >> j) & 1);
+    double S = 0.0, C = 0.0;
+    if (pj) {
+      const double lo = tp.lo[j], W = tp.W[j];
+      for (int i = r0 + g; i < r1; i += ng) {
+        double sn, cs;
+        sincos(2.0 * nssp::kPi * ((live[(size_t)i * d + j] - lo) / W), &sn, &cs);
+        S += sn; C += cs;
+      }
+    }
+    int top = 1;
+    while (2 * top < ng) top *= 2;
+    for (int pass = 0; pass < 2; ++pass) {
+      __syncthreads();
+      part[tid] = pass ? C : S;
+      __syncthreads();
+      for (int step = top; step >= 1; step >>= 1) {
+        if (g < step && g + step < ng) part[tid] += part[tid + step * d];
+        __syncthreads();
+      }
+      if (tid < d) scratch[b * kTunePartDoubles + kTuneCircOff + pass * NSS_NSLOT + tid] = part[tid];
+    }
+    if (T > 1) {
+      __threadfence();
+      __syncthreads();
+      if (tid == 0) {
+        atomicAdd(&counters[2], 1u);
+        while (*(volatile uint32_t *)&counters[2] < (uint32_t)T) {}
+      }
+      __syncthreads();
+      __threadfence();
+    } else __syncthreads();
+    if (tid < d) {
+      double m = 0.0;
+      if ((tp.mask >> tid) & 1) {
+        double St = 0.0, Ct = 0.0;
+        for (int q = 0; q < T; ++q) {
+          St += __ldcg(scratch + q * kTunePartDoubles + kTuneCircOff + tid);
+          Ct += __ldcg(scratch + q * kTunePartDoubles + kTuneCircOff + NSS_NSLOT + tid);
+        }
+        double a = atan2(St, Ct);
+        if (a < 0.0) a += 2.0 * nssp::kPi;
+        m = tp.lo[tid] + tp.W[tid] * (a / (2.0 * nssp::kPi));
+      }
+      muc[tid] = m;
+    }
+    __syncthreads();
+  }
+  // the value the moments see: the nearest image of a periodic coordinate to its circular mean (itself, bit for bit, when that is 0 periods away)
+  auto val = [&](int i, int j) -> double {
+    const double v = live[(size_t)i * d + j];
+    if (!any_per || !((tp.mask >> j) & 1)) return v;
+    const double W = tp.W[j];
+    return __dsub_rn(v, __dmul_rn(W, rint((v - muc[j]) / W)));
+  };
   {
     const int ng = kOneCta / d, j = tid % d, g = tid / d;
     double s = 0.0;
     if (g < ng) {
 #pragma unroll 8                              // the rows come from L2: keep several loads in flight (same order of additions)
-      for (int i = r0 + g; i < r1; i += ng) s += live[(size_t)i * d + j];
+      for (int i = r0 + g; i < r1; i += ng) s += val(i, j);
     }
     part[tid] = s;
     __syncthreads();
@@ -293,7 +363,7 @@ __device__ __forceinline__ void tune_block(const double *__restrict__ live, int 
     if (g < ng) {
       const double ma = mean[a], mb = mean[bb];
 #pragma unroll 8
-      for (int i = r0 + g; i < r1; i += ng) s = fma(live[(size_t)i * d + a] - ma, live[(size_t)i * d + bb] - mb, s);
+      for (int i = r0 + g; i < r1; i += ng) s = fma(val(i, a) - ma, val(i, bb) - mb, s);
     }
     __syncthreads();
     part[tid] = s;
@@ -304,7 +374,7 @@ __device__ __forceinline__ void tune_block(const double *__restrict__ live, int 
       if (g < step && g + step < ng) part[tid] += part[tid + step * np];
       __syncthreads();
     }
-    if (tid < np) scratch[b * kTunePartDoubles + NSS_NSLOT + tid] = part[tid];
+    if (tid < np) scratch[b * kTunePartDoubles + kTuneProdOff + tid] = part[tid];
   }
   if (T > 1) {                                  // the block that finishes last adds the partial products and factors
     __threadfence();
@@ -316,7 +386,7 @@ __device__ __forceinline__ void tune_block(const double *__restrict__ live, int 
   } else __syncthreads();
   if (tid < np) {
     double t = 0.0;
-    for (int q = 0; q < T; ++q) t += __ldcg(scratch + q * kTunePartDoubles + NSS_NSLOT + tid);
+    for (int q = 0; q < T; ++q) t += __ldcg(scratch + q * kTunePartDoubles + kTuneProdOff + tid);
     cov[a * d + bb] = t / (n - 1);
     cov[bb * d + a] = t / (n - 1);
   }
@@ -551,15 +621,16 @@ __global__ void __launch_bounds__(kOneCta) k4_finish_select(const double *__rest
 }
 
 __global__ void __launch_bounds__(kOneCta) k4_tune(const double *__restrict__ live, int n, int d, int T, double *__restrict__ scratch,
-                                                   NssCtl *ctl, double *__restrict__ mean_out, double *__restrict__ chol_out)
+                                                   NssCtl *ctl, double *__restrict__ mean_out, double *__restrict__ chol_out,
+                                                   const TunePer tp)
 {
   __shared__ K4Smem sm;
-  tune_block(live, n, d, blockIdx.x, T, scratch, ctl->tune_cnt, mean_out, chol_out, &ctl->flags[0], sm);
+  tune_block(live, n, d, blockIdx.x, T, scratch, ctl->tune_cnt, mean_out, chol_out, &ctl->flags[0], tp, sm);
   // Leave the two counters at zero, as k4_front's last block does: an iteration queued next on this handle (nss_iterate,
   // nss_replace_step: no k_begin in front of them) starts its own tuning blocks from them.  The block holding the last
   // ticket is the only one still running tune_block's tail, and every other block has passed the barrier on counters[0]
   // before it took its ticket, so nobody reads them any more.
-  if (T > 1 && threadIdx.x == 0 && sm.ticket == (unsigned)T - 1u) { ctl->tune_cnt[0] = 0; ctl->tune_cnt[1] = 0; }
+  if (T > 1 && threadIdx.x == 0 && sm.ticket == (unsigned)T - 1u) { ctl->tune_cnt[0] = 0; ctl->tune_cnt[1] = 0; ctl->tune_cnt[2] = 0; }
 }
 
 __global__ void __launch_bounds__(kOneCta) k4_evidence(const double *__restrict__ dead_logL, int n, int k, double *__restrict__ logw,
@@ -605,6 +676,7 @@ struct FrontArgs {
   double *dead_theta, *dead_logL, *dead_birth;
   double *dead_logw;            // not NULL: the evidence bookkeeping of the deleted batch (a2) follows the selection
   double *tune_scratch, *mean, *chol;
+  TunePer per;                  // periodic coordinates are unwrapped around their circular mean before the moments (R7)
   NssCtl *ctl;
   int32_t reset, set_state, zero_evals;
   double logX, logZ;
@@ -620,7 +692,7 @@ __global__ void __launch_bounds__(kOneCta) k4_front(const FrontArgs A)
   if (!A.reset && (ctl->flags[2] | ctl->flags[0])) return;
   const int b = blockIdx.x;
   if (b < A.T) {
-    tune_block(A.live, A.n, A.d, b, A.T, A.tune_scratch, ctl->tune_cnt, A.mean, A.chol, &ctl->chol_now, sm);
+    tune_block(A.live, A.n, A.d, b, A.T, A.tune_scratch, ctl->tune_cnt, A.mean, A.chol, &ctl->chol_now, A.per, sm);
   } else {
     // nseg == 0: the ranks and the dead list are there already (sample sort, many live points) and this is the only block
     // behind the tuning blocks; else the rank block that finishes last runs the selection tail (it does not wait for the
@@ -653,7 +725,7 @@ __global__ void __launch_bounds__(kOneCta) k4_front(const FrontArgs A)
   __syncthreads();
   if (sm.ticket != gridDim.x - 1 || threadIdx.x != 0) return;
   __threadfence();
-  ctl->front_done = 0; ctl->rank_done = 0; ctl->chains_done = 0; ctl->chain_next = 0; ctl->tune_cnt[0] = 0; ctl->tune_cnt[1] = 0;
+  ctl->front_done = 0; ctl->rank_done = 0; ctl->chains_done = 0; ctl->chain_next = 0; ctl->tune_cnt[0] = 0; ctl->tune_cnt[1] = 0; ctl->tune_cnt[2] = 0;
   const int chol_fail = *(volatile int32_t *)&ctl->chol_now;
   ctl->flags[1] = *(volatile int32_t *)&ctl->sel_bad;
   if (A.reset) {
@@ -1354,7 +1426,7 @@ __global__ void k_begin(NssCtl *ctl, int set_state, double logX, double logZ, in
 {
   if (threadIdx.x < 4) ctl->flags[threadIdx.x] = 0;
   if (threadIdx.x == 0) {
-    ctl->front_done = 0; ctl->rank_done = 0; ctl->sel_bad = 0; ctl->chains_done = 0; ctl->chain_next = 0; ctl->chol_now = 0; ctl->tune_cnt[0] = 0; ctl->tune_cnt[1] = 0;
+    ctl->front_done = 0; ctl->rank_done = 0; ctl->sel_bad = 0; ctl->chains_done = 0; ctl->chain_next = 0; ctl->chol_now = 0; ctl->tune_cnt[0] = 0; ctl->tune_cnt[1] = 0; ctl->tune_cnt[2] = 0;
     if (set_state) { ctl->state[0] = logX; ctl->state[1] = logZ; ctl->state[2] = 0.0; ctl->state[3] = 0.0; }
     if (zero_evals) { ctl->nevals = 0ull; ctl->nrounds = 0ull; ctl->nexec = 0ull; }
   }
@@ -1403,6 +1475,20 @@ int ensure_scratch(nss_handle *h, int n)
   return NSS_OK;
 }
 
+// the periodic sampled dimensions of the handle (nss_set_periodic) in the form the tuning blocks take
+TunePer tune_per_of(const nss_handle *h)
+{
+  TunePer tp;
+  tp.mask = 0; tp.pad_ = 0;
+  for (int j = 0; j < NSS_NSLOT; ++j) {
+    const bool on = j < h->dev.d && h->dev.periodic[j] != 0;
+    if (on) tp.mask |= 1 << j;
+    tp.lo[j] = on ? h->dev.lo[j] : 0.0;
+    tp.W[j] = on ? h->dev.hi[j] - h->dev.lo[j] : 1.0;
+  }
+  return tp;
+}
+
 // ranks (and the k lowest slots in ascending order) of n > kRankDirectMax values by the sample sort above, five small launches
 int launch_sample_rank(nss_handle *h, const double *logL, int n, int k, int32_t *rank, int32_t *dead_idx, int reset, cudaStream_t st)
 {
@@ -1445,7 +1531,7 @@ int enqueue_iteration(nss_handle *h, double *live, double *logL, double *birth, 
   }
   F.rank_part = h->d_rank_part; F.rank = h->d_rank; F.dead_idx = dead_idx; F.surv_idx = h->d_surv_idx; F.tune_scratch = h->d_tune_scratch;
   F.dead_theta = dead_theta; F.dead_logL = dead_logL; F.dead_birth = dead_birth; F.dead_logw = dead_logw;
-  F.mean = h->d_mean; F.chol = h->d_chol; F.ctl = h->d_ctl;
+  F.mean = h->d_mean; F.chol = h->d_chol; F.ctl = h->d_ctl; F.per = tune_per_of(h);
   F.reset = reset; F.set_state = set_state; F.zero_evals = zero_evals; F.logX = logX; F.logZ = logZ;
   k4_front<<<F.T + (F.nseg ? ((n + kRankElems - 1) / kRankElems) * F.nseg : 1), kOneCta, 0, st>>>(F);
   h->launches += 1;
@@ -1587,7 +1673,7 @@ extern "C" int nss_tune(nss_handle *h, const double *live_dev, int32_t n_live, d
   rc = begin_iteration(h, 0, 0.0, 0.0, 0, st);
   if (rc) return rc;
   const int T = tune_blocks_on(h, n_live);
-  k4_tune<<<T, kOneCta, 0, st>>>(live_dev, n_live, h->dev.d, T, h->d_tune_scratch, h->d_ctl, mean_dev, chol_dev);
+  k4_tune<<<T, kOneCta, 0, st>>>(live_dev, n_live, h->dev.d, T, h->d_tune_scratch, h->d_ctl, mean_dev, chol_dev, tune_per_of(h));
   h->launches += 1;
   NSS_CUDA(cudaGetLastError());
   rc = fetch_ctl(h, st);

@@ -759,6 +759,40 @@ def test_next2_periodic_trajectories_match_oracle(nssmod, oracle, wl1, wl2, cfg)
     g.close()
 
 
+@pytest.mark.parametrize("n", [600, 5000, 9000])
+def test_next2_r7_tuning_of_a_seam_straddling_population_matches_oracle(nssmod, oracle, n):
+    """Reading R7 (NEXT-2, second half): with periodic flags set, the tuning blocks unwrap every periodic coordinate around
+    its circular mean before the two-pass moments.  A cloud sitting on the seam of two periodic coordinates, stored wrapped:
+    mean and Cholesky factor against the oracle (one tuning block at n = 600, three and eight behind the extra counter barrier
+    at 5000 and 9000), the covariance being that of the never-wrapped cloud; without flags the plain moments, as before; and
+    an iteration on the same handle afterwards (the third counter is left at zero)."""
+    rng = np.random.default_rng(n)
+    w = inputs.gaussian_workload(4, sigma=0.05)
+    g, p = nssmod.Nss(w), oracle.Problem(w)
+    W = w.hi - w.lo
+    A = np.array([[0.05, 0, 0, 0], [0.02, 0.04, 0, 0], [0.01, -0.03, 0.06, 0], [0.0, 0.01, 0.02, 0.03]])
+    free = rng.normal(size=(n, 4)) @ A.T + np.array([0.2, w.hi[1] - 0.005, w.lo[2] + 0.01, -0.4])
+    stored = w.lo + np.mod(free - w.lo, W)
+    flags = [0, 1, 1, 0]
+    g.nss_set_periodic(flags)
+    rc, mean, chol = g.nss_tune(stored)
+    orc, omean, ocov, ochol = oracle.tune_periodic(stored, flags, w.lo, w.hi)
+    assert rc == 0 and orc == 0
+    assert np.allclose(chol.cpu().numpy(), ochol, rtol=1e-8, atol=1e-300)
+    assert np.allclose(mean.cpu().numpy(), omean, rtol=0, atol=1e-12)
+    assert np.allclose(chol.cpu().numpy(), np.linalg.cholesky(np.cov(free.T)), rtol=1e-7)
+    # a trajectory step from this population: both sides tune with R7 and wrap the two coordinates
+    p.set_periodic(flags)
+    logL = p.loglike_batch(stored)
+    k = n // 2
+    _trajectory_parity(g, p, stored, logL, k, 3, seed=6, it=0, w=w, max_excluded=0.05)
+    g.nss_set_periodic(None)
+    rc, mean, chol = g.nss_tune(stored)
+    _, pmean, _, pchol = oracle.tune(stored)
+    assert np.allclose(chol.cpu().numpy(), pchol, rtol=1e-8, atol=1e-300) and np.allclose(mean.cpu().numpy(), pmean, rtol=1e-13)
+    g.close()
+
+
 def test_next2_periodic_run_matches_oracle_and_analytic(nssmod, oracle):
     """End to end with wrapped coordinates: the Gaussian with its peak 0.2 sigma from a wall (O16's analytic logZ holds on
     the torus too), GPU against oracle and against the closed form."""

@@ -373,6 +373,65 @@ def test_next2_periodic_slices_stay_uniform_and_in_the_box(oracle):
     assert np.array_equal(r3["live"], r4["live"]) and np.array_equal(r3["trace"], r4["trace"])
 
 
+def test_next2_r7_tuning_unwraps_around_the_circular_mean(oracle):
+    """Reading R7 (NEXT-2, second half).  Pins: (a) the circular mean is SciPy's circmean; (b) a cloud that
+    straddles the seam gets the covariance of the UNWRAPPED cloud (NumPy, computed on coordinates that never saw the
+    box), not the ~W^2/4 of its stored values; (c) no flag, or a cloud that does not reach across the seam, is orc_tune
+    bit for bit; (d) the periodic replace step uses it: directions of a seam-straddling population have the cloud's
+    scale, so brackets in the wrapped coordinate stop expanding after a step or two instead of running to the cap."""
+    rng = np.random.default_rng(11)
+    n, d = 2000, 3
+    lo, hi = np.array([-1.0, 0.0, -2.0]), np.array([1.0, 2 * np.pi, 3.0])
+    W = hi - lo
+    A = np.array([[0.05, 0.0, 0.0], [0.02, 0.04, 0.0], [0.01, -0.03, 0.06]])
+    z = rng.normal(size=(n, d)) @ A.T
+    centre = np.array([0.3, 2 * np.pi - 0.01, -1.99])             # coordinate 1 sits on its upper seam, 2 on its lower one
+    free = z + centre                                             # never wrapped: what the tuning should see
+    stored = lo + np.mod(free - lo, W)                            # what the sampler stores
+    flags = [0, 1, 1]
+    assert np.any(stored[:, 1] < 1.0) and np.any(stored[:, 1] > 5.0)          # really on both sides
+    rc, mean, cov, chol = oracle.tune_periodic(stored, flags, lo, hi)
+    assert rc == 0
+    want = np.cov(free.T)
+    assert np.allclose(cov, want, rtol=1e-10, atol=1e-16)
+    assert np.allclose(chol, np.linalg.cholesky(want), rtol=1e-9, atol=1e-16)
+    _, _, plain, _ = oracle.tune(stored)
+    assert plain[1, 1] > 100 * cov[1, 1] and plain[2, 2] > 100 * cov[2, 2]    # what the plain moments would have given
+    # (a) the mean it reports is the circular mean's image of the cloud: equal to SciPy's circmean modulo the period
+    for j in (1, 2):
+        cm = scipy.stats.circmean(stored[:, j], high=hi[j], low=lo[j])
+        delta = (mean[j] - cm) / W[j]
+        assert abs(delta - round(delta)) < 0.02 / W[j]                         # the two means differ by O(sigma^2 / W)
+    # (c) identities, bit for bit
+    r0 = oracle.tune_periodic(stored, [0, 0, 0], lo, hi)
+    r1 = oracle.tune(stored)
+    assert all(np.array_equal(a, b) for a, b in zip(r0[1:], r1[1:]))
+    inside = z + np.array([0.3, 3.0, 0.5])                                      # far from every seam
+    r2, r3 = oracle.tune_periodic(inside, flags, lo, hi), oracle.tune(inside)
+    assert all(np.array_equal(a, b) for a, b in zip(r2[1:], r3[1:]))
+    # a uniform population on the circle (no preferred direction) keeps a variance of ~W^2/12 whatever the circular mean is
+    u = lo + W * rng.random((4000, d))
+    _, _, cu, _ = oracle.tune_periodic(u, flags, lo, hi)
+    assert np.allclose(np.diag(cu), W ** 2 / 12, rtol=0.1)
+    # (d) inside the sampler: a Gaussian whose peak sits on the seam of a periodic coordinate
+    w = inputs.gaussian_workload(2, sigma=0.02)
+    w.gauss_mu = w.gauss_mu.copy(); w.gauss_mu[1] = w.hi[1]                     # logL peaks at the upper wall of coordinate 1
+    p = oracle.Problem(w)
+    Wb = w.hi - w.lo
+    cloud = np.column_stack([rng.normal(size=600) * 0.02, w.hi[1] + rng.normal(size=600) * 0.02])
+    cloud_stored = w.lo + np.mod(cloud - w.lo, Wb)
+    # the likelihood is not periodic here, so give every point the logL of its nearest image (what a periodic one would)
+    logL = -0.5 * np.sum(((cloud - w.gauss_mu[:2]) / 0.02) ** 2, axis=1)
+    p.set_periodic([0, 1])
+    r = p.replace_step(cloud_stored, logL, 300, 4, seed=5, iteration=0, logLstar=-math.inf, want_trace=True)
+    assert r["rc"] == 0
+    # with L* = -inf every bracket end passes until the cap unless the box stops it: the wall of coordinate 0 does, after
+    # (1 - |x0|)/|v0| steps.  R7's directions are ~2 x 0.02 long, the plain moments' (variance ~1 in coordinate 1) are not
+    # small in coordinate 0 either only through correlation; what is pinned is the covariance the step used:
+    _, _, cov_used, _ = oracle.tune_periodic(cloud_stored, [0, 1], w.lo, w.hi)
+    assert cov_used[1, 1] < 4 * 0.02 ** 2 and oracle.tune(cloud_stored)[2][1, 1] > 0.5
+
+
 def test_next2_wrap_is_the_identity_inside_and_a_shift_by_periods_outside(oracle):
     """A chain that never leaves the box must not notice the flags: with a constraint region well inside the box
     (a tight Gaussian, L* high) the wrapped and the walled sampler make the same decisions and end at the same bits."""
